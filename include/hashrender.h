@@ -1,0 +1,143 @@
+/* hashrender.h -- C ABI of the B200-native recursively executed hash-grid renderer.
+ *
+ * The hot path of "Baking Relightable NeRF for Real-time Direct/Indirect Illumination Rendering"
+ * (arXiv 2409.10327; citations are lines of /root/reference/PAPER.md): for every primary surface point x
+ * and sampled light direction w_i, f = H(x) (multi-resolution hash-grid encoder), n,a,r = B(f)
+ * (BRDF decoder MLP), v,t = I(f, w_i) (implicit ray tracer MLP: hard visibility + expected depth,
+ * PAPER.md:80, 98), x' = x + t*w_i, the recursive re-evaluation at x' and
+ * the Monte-Carlo rendering equation (Eq. 1) with the two-bounce incoming radiance
+ * L = V*L_i + (1-V)*L'_o (Eq. 2).  Readings of points the paper leaves open are the Qn
+ * entries of DESIGN.md.
+ *
+ * Conventions
+ *  - Every function returns an int status (HR_OK = 0, ...); nothing throws or aborts across the ABI.
+ *    hashrender_last_error(h) returns a NUL-terminated string owned by the handle (valid until the next
+ *    failing call on that handle or its destruction).
+ *  - Pointers are DEVICE pointers unless the comment says `host`.  All device work is enqueued
+ *    asynchronously on the caller's cudaStream_t (passed as void*, NULL = legacy default stream); no call
+ *    synchronises except hashrender_create, hashrender_destroy and hashrender_render_frame_host.
+ *  - Outputs are caller-allocated.  The library neither frees nor keeps caller memory after a call
+ *    returns; hashrender_create COPIES (and re-lays-out / converts) tables and weights.
+ *  - No allocation after create, except hashrender_render_frame_host's staging buffers (grown on demand,
+ *    released by destroy).
+ *  - Arrays are row-major, innermost index last; float = IEEE binary32.  Directions and w_o are assumed
+ *    unit length (not re-normalised).  Positions outside [0,1]^3 are clamped per component (Q6).
+ *  - N == 0 is a no-op returning HR_OK.  NULL handle / NULL required pointer / S == 0 where a set is
+ *    needed / unsupported shape => error status BEFORE any launch.
+ *  - A handle is single-threaded; distinct handles are independent.
+ *  - Supported shapes (else HR_ERR_UNSUPPORTED): F == 2, 1 <= L <= 16, 1 <= log2_T <= 28, hidden == 64,
+ *    brdf_out == 7, irt_out == 2, tertiary S <= 64.
+ */
+#ifndef HASHRENDER_H_
+#define HASHRENDER_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum { HR_OK = 0, HR_ERR_INVALID_ARG = 1, HR_ERR_CUDA = 2, HR_ERR_OOM = 3, HR_ERR_UNSUPPORTED = 4 };
+enum { HR_F32 = 0, HR_F16 = 1 };
+enum { HR_DIRECT = 1, HR_SHADOW = 2, HR_INDIRECT = 4 };           /* hr_frame.flags */
+enum { HR_TERM_DIRECT = 1, HR_TERM_INDIRECT = 2 };                /* hashrender_shade terms */
+enum { HR_VIS_SOFT = 0, HR_VIS_HARD = 1 };
+enum { HR_BRDF_LAMBERT = 0, HR_BRDF_DISNEY = 1 };
+
+typedef struct hashrender hashrender_t;                           /* opaque */
+
+/* Model description (14 levels, T = 2^17, F = 2, resolutions 16..131072, two 3-layer MLPs of
+ * hidden width 64; BASELINE.json configs use L = 8/16, T = 2^14..2^24). */
+typedef struct {
+  uint32_t L, F, log2_T;
+  const uint32_t* res;          /* host [L]: integer level resolutions N_l (Q2: given, never recomputed) */
+  uint32_t table_dtype;         /* HR_F32 | HR_F16: storage type of the hash tables on the device */
+  uint32_t mlp_dtype;           /* HR_F32: fp32 weights and activations.  HR_F16: fp16 weights and hidden
+                                   activations, fp32 accumulate; final-layer outputs, t, x' and the whole
+                                   index path stay fp32 (Q34) */
+  uint32_t hidden;              /* 64 */
+  uint32_t brdf_out, irt_out;   /* 7, 2 */
+  float near_t, far_t;          /* 0.05, 1.5 */
+  float rough_min;              /* 0.09 */
+  float fresnel_f0;             /* 0.04 */
+  uint32_t vis_mode;            /* HR_VIS_SOFT v = sigma(z_v) | HR_VIS_HARD v = [z_v > 0] (Q14) */
+  uint32_t brdf_model;          /* HR_BRDF_LAMBERT | HR_BRDF_DISNEY (Q21) */
+  float albedo_scale[3];        /* global albedo rescale; 1,1,1 = none */
+  uint64_t max_points;          /* largest N any call will pass (sizes internal scratch) */
+} hr_config;
+
+/* A direction set (sampled w_i with its pdf).  dir[., S, 3], pdf[., S], optional Lin[., S, 3]
+ * (incoming radiance per direction; NULL => looked up in the env map).  point_stride = number of floats of
+ * `dir` (and of `Lin`) between consecutive points; pdf advances by point_stride / 3.  0 = ONE set shared by
+ * all points (Q19). */
+typedef struct {
+  const float* dir; const float* pdf; const float* Lin;
+  uint32_t S; uint64_t point_stride;
+} hr_dirset;
+
+/* One frame of primary points (the direct renderer G hands over material, normal and the
+ * primary surface coordinate x). */
+typedef struct {
+  uint64_t N;
+  const float* x;               /* [N,3] in [0,1]^3 */
+  const float* brdf;            /* [N,7] = n(3) a(3) r(1), post-activation; NULL => B(H(x)) (Q30) */
+  const float* wo;              /* [N,3] unit, towards the camera */
+  const uint8_t* mask;          /* [N] nullable; 0 => rgb = 0 (Q27) */
+  hr_dirset direct;             /* used with HR_DIRECT */
+  hr_dirset secondary;          /* used with HR_INDIRECT: directions along which x' = x + t w is traced */
+  hr_dirset tertiary;           /* used with HR_INDIRECT: directions sampled at every x' (8);
+                                   point_stride != 0 => row index is i*secondary.S + j */
+  uint32_t flags;               /* HR_DIRECT | HR_SHADOW | HR_INDIRECT */
+} hr_frame;
+
+/* Creates a renderer.  tables: host, fp32 [L][T][F] (every level owns T = 2^log2_T slots; a dense level --
+ * (N_l+1)^3 <= T, Q3 -- uses the first (N_l+1)^3); converted once (RNE) when table_dtype == HR_F16.
+ * brdf_w / irt_w: host, fp32 blobs, per layer W[out][in] row-major then b[out]; layers in->64->64->out with
+ * in = L*F for B and L*F+3 ([f ; w], Q13) for I.  Synchronous.  Errors: INVALID_ARG, UNSUPPORTED, OOM, CUDA. */
+int hashrender_create(const hr_config* cfg, const float* tables, const float* brdf_w, const float* irt_w,
+                      hashrender_t** out);
+int hashrender_destroy(hashrender_t* h);
+
+/* Sets the equirect environment map, fp32 [He][We][3], DEVICE pointer; copied on `stream`. */
+int hashrender_set_env(hashrender_t* h, const float* env, uint32_t He, uint32_t We, void* stream);
+
+/* f = H(x) (steps a1-a4).  feat [N, L*F] fp32; optional idx [N, L, 8] uint32 (corner number
+ * b0 + 2 b1 + 4 b2) and w [N, L, 3] fp32 (fractional position), both bit-exact against the oracle. */
+int hashrender_encode(hashrender_t* h, const float* x, uint64_t N, float* feat, uint32_t* idx, float* w, void* stream);
+
+/* n, a, r = B(f) (step a5).  feat [N, L*F] -> brdf [N, 7]. */
+int hashrender_decode(hashrender_t* h, const float* feat, uint64_t N, float* brdf, void* stream);
+
+/* v, t = I(f, w) for every direction of `ds` (step a6) and x' = clamp(x + t w) (
+ * step a7).  feat NULL => the encode is fused (x required).  vis [N,S] (sigma(z_v) or {0,1}); zv nullable
+ * [N,S] raw logit; t [N,S]; xsec nullable [N,S,3] (x required). ds->pdf and ds->Lin are not read. */
+int hashrender_trace(hashrender_t* h, const float* x, const float* feat, uint64_t N, const hr_dirset* ds,
+                     float* vis, float* zv, float* t, float* xsec, void* stream);
+
+/* Eq. 1 with Eq. 2 per direction on ONE set (steps a9-a11):
+ * rgb = 1/S sum_s [ (terms & DIRECT) v L_i + (terms & INDIRECT) (1-v) Lind ] f_r (n.w)^+ / p.
+ * brdf [N,7]; wo [N,3]; vis [N,S]; Lind nullable [N,S,3] (= L'_o); rgb [N,3]. */
+int hashrender_shade(hashrender_t* h, const float* brdf, const float* wo, uint64_t N, const hr_dirset* ds,
+                     const float* vis, const float* Lind, uint32_t terms, float* rgb, void* stream);
+
+/* The fused, timed path (all steps a1-a11): rgb [N,3] = direct (shadowed) + one-bounce indirect radiance. */
+int hashrender_render_frame(hashrender_t* h, const hr_frame* frame, float* rgb, void* stream);
+
+/* Same as hashrender_render_frame but EVERY pointer in `frame` and `rgb` is a HOST pointer (pinned memory
+ * recommended): copies inputs host->device, renders, copies rgb device->host, synchronises `stream`.
+ * h2d_bytes / d2h_bytes (nullable) receive the bytes moved. */
+int hashrender_render_frame_host(hashrender_t* h, const hr_frame* frame, float* rgb, void* stream,
+                                 uint64_t* h2d_bytes, uint64_t* d2h_bytes);
+
+/* Number of kernels this handle has launched so far (for launch accounting in benchmarks). */
+uint64_t hashrender_launch_count(const hashrender_t* h);
+
+/* Which implementation the last render_frame / trace used: "ffma32" or "tcgen05-f16". Never NULL. */
+const char* hashrender_last_path(const hashrender_t* h);
+
+const char* hashrender_last_error(const hashrender_t* h);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* HASHRENDER_H_ */

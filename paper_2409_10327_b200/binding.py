@@ -1,0 +1,197 @@
+"""ctypes binding of include/hashrender.h.  Same names as the C ABI; marshals torch CUDA tensors (device
+pointers) and numpy arrays (host pointers) into plain pointers + sizes.  No arithmetic happens here, and there
+is NO fallback: if the CUDA library cannot be loaded every call raises."""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from dataclasses import dataclass
+
+import numpy as np
+
+HR_DIRECT, HR_SHADOW, HR_INDIRECT = 1, 2, 4
+HR_TERM_DIRECT, HR_TERM_INDIRECT = 1, 2
+_STATUS = {1: "HR_ERR_INVALID_ARG", 2: "HR_ERR_CUDA", 3: "HR_ERR_OOM", 4: "HR_ERR_UNSUPPORTED"}
+_LIB_PATH = os.path.join(os.path.dirname(os.path.abspath(__file__)), "libhashrender.so")
+
+EXPORTS = ["hashrender_create", "hashrender_destroy", "hashrender_set_env", "hashrender_encode", "hashrender_decode",
+           "hashrender_trace", "hashrender_shade", "hashrender_render_frame", "hashrender_render_frame_host",
+           "hashrender_launch_count", "hashrender_last_path", "hashrender_last_error"]
+
+
+class HashRenderError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__(f"{_STATUS.get(code, code)}: {msg}")
+        self.code = code
+
+
+class hr_config(C.Structure):
+    _fields_ = [("L", C.c_uint32), ("F", C.c_uint32), ("log2_T", C.c_uint32), ("res", C.POINTER(C.c_uint32)),
+                ("table_dtype", C.c_uint32), ("mlp_dtype", C.c_uint32), ("hidden", C.c_uint32), ("brdf_out", C.c_uint32),
+                ("irt_out", C.c_uint32), ("near_t", C.c_float), ("far_t", C.c_float), ("rough_min", C.c_float),
+                ("fresnel_f0", C.c_float), ("vis_mode", C.c_uint32), ("brdf_model", C.c_uint32),
+                ("albedo_scale", C.c_float * 3), ("max_points", C.c_uint64)]
+
+
+class hr_dirset(C.Structure):
+    _fields_ = [("dir", C.c_void_p), ("pdf", C.c_void_p), ("Lin", C.c_void_p), ("S", C.c_uint32), ("point_stride", C.c_uint64)]
+
+
+class hr_frame(C.Structure):
+    _fields_ = [("N", C.c_uint64), ("x", C.c_void_p), ("brdf", C.c_void_p), ("wo", C.c_void_p), ("mask", C.c_void_p),
+                ("direct", hr_dirset), ("secondary", hr_dirset), ("tertiary", hr_dirset), ("flags", C.c_uint32)]
+
+
+_lib = None
+
+
+def load_library(path: str | None = None):
+    """Loads libhashrender.so (must have been built: `python -m paper_2409_10327_b200.build`).  Fails loudly."""
+    global _lib
+    if _lib is None:
+        p = path or _LIB_PATH
+        if not os.path.exists(p):
+            raise ImportError(f"{p} not found: build it with `python -m paper_2409_10327_b200.build` "
+                              "(there is no CPU fallback)")
+        lib = C.CDLL(p)
+        vp, u64, u32 = C.c_void_p, C.c_uint64, C.c_uint32
+        lib.hashrender_create.argtypes = [C.POINTER(hr_config), vp, vp, vp, C.POINTER(vp)]
+        lib.hashrender_destroy.argtypes = [vp]
+        lib.hashrender_set_env.argtypes = [vp, vp, u32, u32, vp]
+        lib.hashrender_encode.argtypes = [vp, vp, u64, vp, vp, vp, vp]
+        lib.hashrender_decode.argtypes = [vp, vp, u64, vp, vp]
+        lib.hashrender_trace.argtypes = [vp, vp, vp, u64, C.POINTER(hr_dirset), vp, vp, vp, vp, vp]
+        lib.hashrender_shade.argtypes = [vp, vp, vp, u64, C.POINTER(hr_dirset), vp, vp, u32, vp, vp]
+        lib.hashrender_render_frame.argtypes = [vp, C.POINTER(hr_frame), vp, vp]
+        lib.hashrender_render_frame_host.argtypes = [vp, C.POINTER(hr_frame), vp, vp, C.POINTER(u64), C.POINTER(u64)]
+        lib.hashrender_launch_count.argtypes = [vp]
+        lib.hashrender_launch_count.restype = u64
+        lib.hashrender_last_path.argtypes = [vp]
+        lib.hashrender_last_path.restype = C.c_char_p
+        lib.hashrender_last_error.argtypes = [vp]
+        lib.hashrender_last_error.restype = C.c_char_p
+        for name in EXPORTS:
+            if name not in ("hashrender_launch_count", "hashrender_last_path", "hashrender_last_error"):
+                getattr(lib, name).restype = C.c_int
+        _lib = lib
+    return _lib
+
+
+def _ptr(a):
+    """torch tensor (any device) or numpy array -> raw pointer; None -> NULL.  Must be contiguous."""
+    if a is None:
+        return None
+    if isinstance(a, np.ndarray):
+        assert a.flags["C_CONTIGUOUS"]
+        return C.c_void_p(a.ctypes.data)
+    assert a.is_contiguous()
+    return C.c_void_p(a.data_ptr())
+
+
+@dataclass
+class DirSet:
+    """dir [N,S,3] (or [S,3] = one shared set), pdf [N,S] (or [S]), optional Lin like dir."""
+    dir: object
+    pdf: object
+    Lin: object = None
+
+    def c(self) -> hr_dirset:
+        shared = self.dir.ndim == 2
+        S = self.dir.shape[-2]
+        return hr_dirset(dir=_ptr(self.dir), pdf=_ptr(self.pdf), Lin=_ptr(self.Lin), S=S, point_stride=0 if shared else 3 * S)
+
+
+class HashRenderer:
+    """Owns one hashrender_t handle.  Methods mirror the C ABI one to one."""
+
+    def __init__(self, *, L, F, log2_T, res, tables, brdf_w, irt_w, table_dtype="f32", mlp_dtype="f32", hidden=64,
+                 near_t=0.05, far_t=1.5, rough_min=0.09, fresnel_f0=0.04, vis_mode=0, brdf_model=1,
+                 albedo_scale=(1.0, 1.0, 1.0), max_points=1 << 20):
+        self._lib = load_library()
+        self._res = np.ascontiguousarray(res, dtype=np.uint32)
+        tables = np.ascontiguousarray(tables, dtype=np.float32)
+        brdf_w = np.ascontiguousarray(brdf_w, dtype=np.float32)
+        irt_w = np.ascontiguousarray(irt_w, dtype=np.float32)
+        assert tables.size == L * (1 << log2_T) * F
+        assert brdf_w.size == hidden * (L * F) + hidden + hidden * hidden + hidden + 7 * hidden + 7
+        assert irt_w.size == hidden * (L * F + 3) + hidden + hidden * hidden + hidden + 2 * hidden + 2
+        self.L, self.F, self.D = L, F, L * F
+        self.cfg = hr_config(L=L, F=F, log2_T=log2_T, res=self._res.ctypes.data_as(C.POINTER(C.c_uint32)),
+                             table_dtype={"f32": 0, "f16": 1}[table_dtype], mlp_dtype={"f32": 0, "f16": 1}[mlp_dtype],
+                             hidden=hidden, brdf_out=7, irt_out=2, near_t=near_t, far_t=far_t, rough_min=rough_min,
+                             fresnel_f0=fresnel_f0, vis_mode=vis_mode, brdf_model=brdf_model,
+                             albedo_scale=(C.c_float * 3)(*albedo_scale), max_points=max_points)
+        self._h = C.c_void_p()
+        rc = self._lib.hashrender_create(C.byref(self.cfg), _ptr(tables), _ptr(brdf_w), _ptr(irt_w), C.byref(self._h))
+        if rc != 0:
+            msg = self._lib.hashrender_last_error(self._h).decode() if self._h else "create failed"
+            if self._h:
+                self._lib.hashrender_destroy(self._h)
+                self._h = C.c_void_p()
+            raise HashRenderError(rc, msg)
+
+    @classmethod
+    def from_gen(cls, cfg, model, **over):
+        kw = dict(L=cfg.L, F=cfg.F, log2_T=cfg.log2_T, res=model["res"], tables=model["tables"], brdf_w=model["brdf_w"],
+                  irt_w=model["irt_w"], table_dtype=cfg.table_dtype, mlp_dtype=cfg.mlp_dtype, hidden=cfg.hidden,
+                  near_t=cfg.near_t, far_t=cfg.far_t, rough_min=cfg.rough_min, fresnel_f0=cfg.fresnel_f0,
+                  max_points=max(cfg.N, 1 << 16))
+        kw.update(over)
+        return cls(**kw)
+
+    def _check(self, rc):
+        if rc != 0:
+            raise HashRenderError(rc, self._lib.hashrender_last_error(self._h).decode())
+
+    def destroy(self):
+        if getattr(self, "_h", None):
+            self._lib.hashrender_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+    # ---- C ABI mirrors (device pointers; stream = int cudaStream_t handle or None) -----------------------
+    def set_env(self, env, stream=None):
+        self._check(self._lib.hashrender_set_env(self._h, _ptr(env), env.shape[0], env.shape[1], stream))
+
+    def encode(self, x, feat, idx=None, w=None, stream=None, N=None):
+        self._check(self._lib.hashrender_encode(self._h, _ptr(x), x.shape[0] if N is None else N, _ptr(feat), _ptr(idx), _ptr(w), stream))
+
+    def decode(self, feat, brdf, stream=None):
+        self._check(self._lib.hashrender_decode(self._h, _ptr(feat), feat.shape[0], _ptr(brdf), stream))
+
+    def trace(self, x, feat, ds: DirSet, vis, zv, t, xsec=None, stream=None, N=None):
+        n = N if N is not None else (x.shape[0] if x is not None else feat.shape[0])
+        d = ds.c()
+        self._check(self._lib.hashrender_trace(self._h, _ptr(x), _ptr(feat), n, C.byref(d), _ptr(vis), _ptr(zv), _ptr(t), _ptr(xsec), stream))
+
+    def shade(self, brdf, wo, ds: DirSet, vis, Lind, terms, rgb, stream=None):
+        d = ds.c()
+        self._check(self._lib.hashrender_shade(self._h, _ptr(brdf), _ptr(wo), brdf.shape[0], C.byref(d), _ptr(vis), _ptr(Lind), terms, _ptr(rgb), stream))
+
+    def make_frame(self, x, wo, direct: DirSet | None, secondary: DirSet | None = None, tertiary: DirSet | None = None,
+                   flags=HR_DIRECT | HR_SHADOW, brdf=None, mask=None, N=None) -> hr_frame:
+        z = hr_dirset()
+        fr = hr_frame(N=x.shape[0] if N is None else N, x=_ptr(x), brdf=_ptr(brdf), wo=_ptr(wo), mask=_ptr(mask),
+                      direct=direct.c() if direct else z, secondary=secondary.c() if secondary else z,
+                      tertiary=tertiary.c() if tertiary else z, flags=flags)
+        fr._keep = (x, wo, direct, secondary, tertiary, brdf, mask)
+        return fr
+
+    def render_frame(self, frame: hr_frame, rgb, stream=None):
+        self._check(self._lib.hashrender_render_frame(self._h, C.byref(frame), _ptr(rgb), stream))
+
+    def render_frame_host(self, frame: hr_frame, rgb, stream=None):
+        up, down = C.c_uint64(), C.c_uint64()
+        self._check(self._lib.hashrender_render_frame_host(self._h, C.byref(frame), _ptr(rgb), stream, C.byref(up), C.byref(down)))
+        return up.value, down.value
+
+    def launch_count(self) -> int:
+        return int(self._lib.hashrender_launch_count(self._h))
+
+    def last_path(self) -> str:
+        return self._lib.hashrender_last_path(self._h).decode()

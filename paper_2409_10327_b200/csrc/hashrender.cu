@@ -1,0 +1,415 @@
+// hashrender.cu -- C-ABI entry points (include/hashrender.h) and host-side launch logic.
+// Argument validation happens before any launch; every kernel is enqueued on the caller's stream.
+#include <cuda_runtime.h>
+
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+#include "../../include/hashrender.h"
+#include "hr_kernels_ffma.cuh"
+#ifndef HR_NO_TC
+#include "hr_kernels_tc.cuh"
+#endif
+
+using namespace hr;
+
+struct hashrender {
+  hr_config cfg;
+  uint32_t res[kMaxL];
+  GridP grid;
+  ShadeP shade;
+  EnvP env;
+  void* d_tables = nullptr;
+  float* d_wts = nullptr;        // prepared fp32 weights (hr_kernels_ffma.cuh layout)
+  void* d_wts_tc = nullptr;      // prepared fp16 UMMA-layout weights (hr_kernels_tc.cuh), mlp_dtype == HR_F16
+  float* d_env = nullptr;
+  size_t env_cap = 0;
+  int num_sms = 148;
+  uint64_t launches = 0;
+  const char* last_path = "none";
+  char err[512];
+  // staging for render_frame_host
+  void* stage[16] = {nullptr};
+  size_t stage_cap[16] = {0};
+  int force_path = 0;            // 0 auto, 1 ffma, 2 tc  (env HASHRENDER_PATH, for A/B tests)
+};
+
+namespace {
+
+int fail(hashrender* h, int code, const char* fmt, ...) {
+  if (h) {
+    va_list ap; va_start(ap, fmt);
+    vsnprintf(h->err, sizeof(h->err), fmt, ap);
+    va_end(ap);
+  }
+  return code;
+}
+
+#define HR_CUDA(h, call)                                                                              \
+  do {                                                                                                \
+    cudaError_t e_ = (call);                                                                          \
+    if (e_ != cudaSuccess)                                                                            \
+      return fail(h, e_ == cudaErrorMemoryAllocation ? HR_ERR_OOM : HR_ERR_CUDA, "%s failed: %s", #call, \
+                  cudaGetErrorString(e_));                                                            \
+  } while (0)
+
+__global__ void k_f32_to_f16(const float* __restrict__ src, __half* __restrict__ dst, size_t n) {
+  for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x)
+    dst[i] = __float2half_rn(src[i]);
+}
+
+constexpr int NT_FFMA = 256;
+
+void prepare_weights_ffma(const hr_config& c, const float* bw, const float* iw, std::vector<float>& out) {
+  const int D = c.L * c.F, H = kH;
+  out.assign(wo_::ALL, 0.f);
+  float* B = out.data();
+  float* I = out.data() + wo_::B_SIZE;
+  {  // B: W1[H][D], b1[H], W2[H][H], b2[H], W3[7][H], b3[7]
+    const float* W1 = bw; const float* b1 = W1 + H * D; const float* W2 = b1 + H; const float* b2 = W2 + H * H;
+    const float* W3 = b2 + H; const float* b3 = W3 + 7 * H;
+    for (int j = 0; j < H; ++j) for (int k = 0; k < D; ++k) B[wo_::B_W1 + k * H + j] = W1[j * D + k];
+    for (int j = 0; j < H; ++j) B[wo_::B_b1 + j] = b1[j];
+    for (int j = 0; j < H; ++j) for (int k = 0; k < H; ++k) B[wo_::B_W2 + k * H + j] = W2[j * H + k];
+    for (int j = 0; j < H; ++j) B[wo_::B_b2 + j] = b2[j];
+    for (int cidx = 0; cidx < 7; ++cidx) for (int k = 0; k < H; ++k) B[wo_::B_W3 + k * 8 + cidx] = W3[cidx * H + k];
+    for (int cidx = 0; cidx < 7; ++cidx) B[wo_::B_b3 + cidx] = b3[cidx];
+  }
+  {  // I: W1[H][D+3], b1[H], W2[H][H], b2[H], W3[2][H], b3[2]
+    const int Din = D + 3;
+    const float* W1 = iw; const float* b1 = W1 + H * Din; const float* W2 = b1 + H; const float* b2 = W2 + H * H;
+    const float* W3 = b2 + H; const float* b3 = W3 + 2 * H;
+    for (int j = 0; j < H; ++j) for (int k = 0; k < D; ++k) I[wo_::I_W1f + k * H + j] = W1[j * Din + k];
+    for (int j = 0; j < H; ++j) for (int d = 0; d < 3; ++d) I[wo_::I_W1w + d * H + j] = W1[j * Din + D + d];
+    for (int j = 0; j < H; ++j) I[wo_::I_b1 + j] = b1[j];
+    for (int j = 0; j < H; ++j) for (int k = 0; k < H; ++k) I[wo_::I_W2 + k * H + j] = W2[j * H + k];
+    for (int j = 0; j < H; ++j) I[wo_::I_b2 + j] = b2[j];
+    for (int cidx = 0; cidx < 2; ++cidx) for (int k = 0; k < H; ++k) I[wo_::I_W3 + k * 2 + cidx] = W3[cidx * H + k];
+    for (int cidx = 0; cidx < 2; ++cidx) I[wo_::I_b3 + cidx] = b3[cidx];
+  }
+}
+
+DirsetP to_dev(const hr_dirset& d) {
+  DirsetP p; p.dir = d.dir; p.pdf = d.pdf; p.Lin = d.Lin; p.S = d.S; p.stride = d.point_stride; return p;
+}
+
+int grid_for(const hashrender* h, uint64_t N, int nt, int blocks_per_sm) {
+  uint64_t need = (N + nt - 1) / nt;
+  uint64_t cap = (uint64_t)h->num_sms * blocks_per_sm;
+  return (int)(need < cap ? need : cap);
+}
+
+int check_dirset(hashrender* h, const hr_dirset* d, const char* name, bool need_pdf) {
+  if (!d) return fail(h, HR_ERR_INVALID_ARG, "%s: NULL direction set", name);
+  if (d->S == 0) return fail(h, HR_ERR_INVALID_ARG, "%s: S == 0", name);
+  if (!d->dir) return fail(h, HR_ERR_INVALID_ARG, "%s: NULL dir", name);
+  if (need_pdf && !d->pdf) return fail(h, HR_ERR_INVALID_ARG, "%s: NULL pdf", name);
+  if (d->point_stride % 3 != 0) return fail(h, HR_ERR_INVALID_ARG, "%s: point_stride must be a multiple of 3", name);
+  if (d->point_stride && d->point_stride < 3ull * d->S) return fail(h, HR_ERR_INVALID_ARG, "%s: point_stride < 3*S", name);
+  return HR_OK;
+}
+
+bool use_tc(const hashrender* h) {
+#ifdef HR_NO_TC
+  return false;
+#else
+  if (h->force_path == 1) return false;
+  if (h->force_path == 2) return h->d_wts_tc != nullptr;
+  return h->cfg.mlp_dtype == HR_F16 && h->d_wts_tc != nullptr;
+#endif
+}
+
+}  // namespace
+
+extern "C" {
+
+int hashrender_create(const hr_config* cfg, const float* tables, const float* brdf_w, const float* irt_w, hashrender_t** out) {
+  if (!out) return HR_ERR_INVALID_ARG;
+  *out = nullptr;
+  if (!cfg || !tables || !brdf_w || !irt_w || !cfg->res) return HR_ERR_INVALID_ARG;
+  hashrender* h = new (std::nothrow) hashrender();
+  if (!h) return HR_ERR_OOM;
+  h->err[0] = 0;
+  *out = h;   // returned even on failure so the caller can read last_error, then destroy
+  h->cfg = *cfg;
+  if (cfg->F != 2 || cfg->L < 1 || cfg->L > kMaxL || cfg->log2_T < 1 || cfg->log2_T > 28 || cfg->hidden != kH ||
+      cfg->brdf_out != 7 || cfg->irt_out != 2)
+    return fail(h, HR_ERR_UNSUPPORTED, "unsupported shape: need F==2, 1<=L<=16, 1<=log2_T<=28, hidden==64, brdf_out==7, irt_out==2");
+  if (cfg->table_dtype > 1 || cfg->mlp_dtype > 1 || cfg->vis_mode > 1 || cfg->brdf_model > 1)
+    return fail(h, HR_ERR_INVALID_ARG, "bad dtype / mode enum");
+  for (uint32_t l = 0; l < cfg->L; ++l) {
+    h->res[l] = cfg->res[l];
+    if (cfg->res[l] < 1 || cfg->res[l] > (1u << 24)) return fail(h, HR_ERR_INVALID_ARG, "res[%u] out of range", l);
+  }
+  h->cfg.res = h->res;
+  int dev = 0;
+  HR_CUDA(h, cudaGetDevice(&dev));
+  HR_CUDA(h, cudaDeviceGetAttribute(&h->num_sms, cudaDevAttrMultiProcessorCount, dev));
+  const char* fp = getenv("HASHRENDER_PATH");
+  if (fp) h->force_path = !strcmp(fp, "ffma") ? 1 : (!strcmp(fp, "tc") ? 2 : 0);
+
+  // grid parameters
+  GridP& g = h->grid;
+  g.L = cfg->L; g.log2_T = cfg->log2_T; g.f16 = cfg->table_dtype; g.dense_mask = 0;
+  for (uint32_t l = 0; l < kMaxL; ++l) g.res[l] = l < cfg->L ? cfg->res[l] : 1;
+  for (uint32_t l = 0; l < cfg->L; ++l) {
+    const uint64_t s = (uint64_t)cfg->res[l] + 1;
+    if (s * s * s <= (1ull << cfg->log2_T)) g.dense_mask |= 1u << l;
+  }
+  // tables: fp32 host -> device float2 / half2
+  const size_t n = (size_t)cfg->L << cfg->log2_T << 1;
+  if (cfg->table_dtype == HR_F32) {
+    HR_CUDA(h, cudaMalloc(&h->d_tables, n * sizeof(float)));
+    HR_CUDA(h, cudaMemcpy(h->d_tables, tables, n * sizeof(float), cudaMemcpyHostToDevice));
+  } else {
+    HR_CUDA(h, cudaMalloc(&h->d_tables, n * sizeof(__half)));
+    const size_t chunk = (size_t)16 << 20;
+    float* st = nullptr;
+    HR_CUDA(h, cudaMalloc(&st, chunk * sizeof(float)));
+    for (size_t o = 0; o < n; o += chunk) {
+      const size_t m = n - o < chunk ? n - o : chunk;
+      cudaError_t e = cudaMemcpy(st, tables + o, m * sizeof(float), cudaMemcpyHostToDevice);
+      if (e == cudaSuccess) {
+        k_f32_to_f16<<<h->num_sms * 8, 256>>>(st, reinterpret_cast<__half*>(h->d_tables) + o, m);
+        e = cudaDeviceSynchronize();
+      }
+      if (e != cudaSuccess) { cudaFree(st); return fail(h, HR_ERR_CUDA, "table conversion failed: %s", cudaGetErrorString(e)); }
+    }
+    cudaFree(st);
+  }
+  g.tables = h->d_tables;
+  // weights
+  std::vector<float> w;
+  prepare_weights_ffma(*cfg, brdf_w, irt_w, w);
+  HR_CUDA(h, cudaMalloc(&h->d_wts, w.size() * sizeof(float)));
+  HR_CUDA(h, cudaMemcpy(h->d_wts, w.data(), w.size() * sizeof(float), cudaMemcpyHostToDevice));
+#ifndef HR_NO_TC
+  if (cfg->mlp_dtype == HR_F16 || h->force_path == 2) {
+    std::vector<uint8_t> wt;
+    tc::prepare_weights(*cfg, brdf_w, irt_w, wt);
+    HR_CUDA(h, cudaMalloc(&h->d_wts_tc, wt.size()));
+    HR_CUDA(h, cudaMemcpy(h->d_wts_tc, wt.data(), wt.size(), cudaMemcpyHostToDevice));
+    HR_CUDA(h, tc::set_attributes());
+  }
+#endif
+  ShadeP& s = h->shade;
+  s.near_t = cfg->near_t; s.far_t = cfg->far_t; s.rough_min = cfg->rough_min; s.f0 = cfg->fresnel_f0;
+  s.vis_mode = cfg->vis_mode; s.brdf_model = cfg->brdf_model;
+  s.as0 = cfg->albedo_scale[0]; s.as1 = cfg->albedo_scale[1]; s.as2 = cfg->albedo_scale[2];
+  h->env.env = nullptr; h->env.He = h->env.We = 0;
+
+  const int smem_full = (int)ffma_smem_bytes(NT_FFMA, true), smem_half = (int)ffma_smem_bytes(NT_FFMA, false);
+  HR_CUDA(h, cudaFuncSetAttribute(k_render_ffma<false, NT_FFMA>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_full));
+  HR_CUDA(h, cudaFuncSetAttribute(k_render_ffma<true, NT_FFMA>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_full));
+  HR_CUDA(h, cudaFuncSetAttribute(k_trace_ffma<false, NT_FFMA>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_half));
+  HR_CUDA(h, cudaFuncSetAttribute(k_trace_ffma<true, NT_FFMA>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_half));
+  HR_CUDA(h, cudaFuncSetAttribute(k_decode_ffma<NT_FFMA>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_half));
+  return HR_OK;
+}
+
+int hashrender_destroy(hashrender_t* h) {
+  if (!h) return HR_ERR_INVALID_ARG;
+  cudaDeviceSynchronize();
+  cudaFree(h->d_tables); cudaFree(h->d_wts); cudaFree(h->d_wts_tc); cudaFree(h->d_env);
+  for (int i = 0; i < 16; ++i) cudaFree(h->stage[i]);
+  delete h;
+  return HR_OK;
+}
+
+int hashrender_set_env(hashrender_t* h, const float* env, uint32_t He, uint32_t We, void* stream) {
+  if (!h) return HR_ERR_INVALID_ARG;
+  if (!env || He == 0 || We == 0 || He > 8192 || We > 16384) return fail(h, HR_ERR_INVALID_ARG, "set_env: bad env / size");
+  const size_t bytes = (size_t)He * We * 3 * sizeof(float);
+  if (bytes > h->env_cap) {
+    cudaFree(h->d_env); h->d_env = nullptr; h->env_cap = 0;
+    HR_CUDA(h, cudaMalloc(&h->d_env, bytes));
+    h->env_cap = bytes;
+  }
+  HR_CUDA(h, cudaMemcpyAsync(h->d_env, env, bytes, cudaMemcpyDeviceToDevice, (cudaStream_t)stream));
+  h->env.env = h->d_env; h->env.He = He; h->env.We = We;
+  return HR_OK;
+}
+
+int hashrender_encode(hashrender_t* h, const float* x, uint64_t N, float* feat, uint32_t* idx, float* w, void* stream) {
+  if (!h) return HR_ERR_INVALID_ARG;
+  if (N == 0) return HR_OK;
+  if (!x || !feat) return fail(h, HR_ERR_INVALID_ARG, "encode: NULL x or feat");
+  if (N > h->cfg.max_points) return fail(h, HR_ERR_INVALID_ARG, "encode: N exceeds max_points");
+  const int grid = grid_for(h, N, 256, 8);
+  if (h->grid.f16) k_encode<true><<<grid, 256, 0, (cudaStream_t)stream>>>(h->grid, x, N, feat, idx, w);
+  else k_encode<false><<<grid, 256, 0, (cudaStream_t)stream>>>(h->grid, x, N, feat, idx, w);
+  h->launches++;
+  HR_CUDA(h, cudaGetLastError());
+  return HR_OK;
+}
+
+int hashrender_decode(hashrender_t* h, const float* feat, uint64_t N, float* brdf, void* stream) {
+  if (!h) return HR_ERR_INVALID_ARG;
+  if (N == 0) return HR_OK;
+  if (!feat || !brdf) return fail(h, HR_ERR_INVALID_ARG, "decode: NULL feat or brdf");
+  if (N > h->cfg.max_points) return fail(h, HR_ERR_INVALID_ARG, "decode: N exceeds max_points");
+  k_decode_ffma<NT_FFMA><<<grid_for(h, N, NT_FFMA, 1), NT_FFMA, ffma_smem_bytes(NT_FFMA, false), (cudaStream_t)stream>>>(
+      h->shade, h->d_wts, h->cfg.L * 2, feat, N, brdf);
+  h->launches++;
+  HR_CUDA(h, cudaGetLastError());
+  return HR_OK;
+}
+
+int hashrender_trace(hashrender_t* h, const float* x, const float* feat, uint64_t N, const hr_dirset* ds, float* vis, float* zv,
+                     float* t, float* xsec, void* stream) {
+  if (!h) return HR_ERR_INVALID_ARG;
+  if (N == 0) return HR_OK;
+  if (int e = check_dirset(h, ds, "trace", false)) return e;
+  if (!vis || !t) return fail(h, HR_ERR_INVALID_ARG, "trace: NULL vis or t");
+  if (!feat && !x) return fail(h, HR_ERR_INVALID_ARG, "trace: need x when feat is NULL (fused encode)");
+  if (xsec && !x) return fail(h, HR_ERR_INVALID_ARG, "trace: xsec needs x");
+  if (N > h->cfg.max_points) return fail(h, HR_ERR_INVALID_ARG, "trace: N exceeds max_points");
+  const DirsetP d = to_dev(*ds);
+#ifndef HR_NO_TC
+  if (use_tc(h) && !feat) {
+    h->last_path = "tcgen05-f16";
+    HR_CUDA(h, tc::launch_trace(h->grid, h->shade, h->d_wts_tc, x, N, d, vis, zv, t, xsec, h->num_sms, (cudaStream_t)stream));
+    h->launches++;
+    return HR_OK;
+  }
+#endif
+  h->last_path = "ffma32";
+  const int grid = grid_for(h, N, NT_FFMA, 1);
+  const size_t smem = ffma_smem_bytes(NT_FFMA, false);
+  if (h->grid.f16) k_trace_ffma<true, NT_FFMA><<<grid, NT_FFMA, smem, (cudaStream_t)stream>>>(h->grid, h->shade, h->d_wts, x, feat, N, d, vis, zv, t, xsec);
+  else k_trace_ffma<false, NT_FFMA><<<grid, NT_FFMA, smem, (cudaStream_t)stream>>>(h->grid, h->shade, h->d_wts, x, feat, N, d, vis, zv, t, xsec);
+  h->launches++;
+  HR_CUDA(h, cudaGetLastError());
+  return HR_OK;
+}
+
+int hashrender_shade(hashrender_t* h, const float* brdf, const float* wo, uint64_t N, const hr_dirset* ds, const float* vis,
+                     const float* Lind, uint32_t terms, float* rgb, void* stream) {
+  if (!h) return HR_ERR_INVALID_ARG;
+  if (N == 0) return HR_OK;
+  if (int e = check_dirset(h, ds, "shade", true)) return e;
+  if (!brdf || !wo || !vis || !rgb) return fail(h, HR_ERR_INVALID_ARG, "shade: NULL brdf / wo / vis / rgb");
+  if ((terms & HR_TERM_DIRECT) && !ds->Lin && !h->env.env) return fail(h, HR_ERR_INVALID_ARG, "shade: no env map set and no Lin");
+  if ((terms & ~3u) || terms == 0) return fail(h, HR_ERR_INVALID_ARG, "shade: bad terms");
+  if (N > h->cfg.max_points) return fail(h, HR_ERR_INVALID_ARG, "shade: N exceeds max_points");
+  k_shade<<<grid_for(h, N, 256, 8), 256, 0, (cudaStream_t)stream>>>(h->env, h->shade, brdf, wo, N, to_dev(*ds), vis, Lind, terms, rgb);
+  h->launches++;
+  HR_CUDA(h, cudaGetLastError());
+  return HR_OK;
+}
+
+static int check_frame(hashrender* h, const hr_frame* f, const float* rgb) {
+  if (!f) return fail(h, HR_ERR_INVALID_ARG, "render_frame: NULL frame");
+  if (f->N == 0) return HR_OK;
+  if (!f->x || !f->wo || !rgb) return fail(h, HR_ERR_INVALID_ARG, "render_frame: NULL x / wo / rgb");
+  if (f->N > h->cfg.max_points) return fail(h, HR_ERR_INVALID_ARG, "render_frame: N exceeds max_points");
+  if (!(f->flags & (HR_DIRECT | HR_INDIRECT)) || (f->flags & ~7u)) return fail(h, HR_ERR_INVALID_ARG, "render_frame: bad flags");
+  bool need_env = false;
+  if (f->flags & HR_DIRECT) {
+    if (int e = check_dirset(h, &f->direct, "render_frame.direct", true)) return e;
+    need_env |= !f->direct.Lin;
+  }
+  if (f->flags & HR_INDIRECT) {
+    if (int e = check_dirset(h, &f->secondary, "render_frame.secondary", true)) return e;
+    if (int e = check_dirset(h, &f->tertiary, "render_frame.tertiary", true)) return e;
+    if (f->tertiary.S > kMaxS2) return fail(h, HR_ERR_UNSUPPORTED, "render_frame: tertiary S > 64");
+    need_env |= !f->tertiary.Lin;
+  }
+  if (need_env && !h->env.env) return fail(h, HR_ERR_INVALID_ARG, "render_frame: no env map set and no Lin");
+  return HR_OK;
+}
+
+int hashrender_render_frame(hashrender_t* h, const hr_frame* f, float* rgb, void* stream) {
+  if (!h) return HR_ERR_INVALID_ARG;
+  if (int e = check_frame(h, f, rgb)) return e;
+  if (f->N == 0) return HR_OK;
+  FrameP fr;
+  fr.N = f->N; fr.x = f->x; fr.brdf = f->brdf; fr.wo = f->wo; fr.mask = f->mask; fr.flags = f->flags;
+  fr.d = to_dev(f->direct); fr.s = to_dev(f->secondary); fr.t = to_dev(f->tertiary);
+  if (!(f->flags & HR_DIRECT)) fr.d.S = 0;
+  if (!(f->flags & HR_INDIRECT)) { fr.s.S = 0; fr.t.S = 0; }
+#ifndef HR_NO_TC
+  if (use_tc(h) && tc::frame_supported(fr)) {
+    h->last_path = "tcgen05-f16";
+    int nl = 0;
+    HR_CUDA(h, tc::launch_render(h->grid, h->env, h->shade, h->d_wts_tc, fr, rgb, h->num_sms, (cudaStream_t)stream, &nl));
+    h->launches += nl;
+    return HR_OK;
+  }
+#endif
+  h->last_path = "ffma32";
+  const int grid = grid_for(h, f->N, NT_FFMA, 1);
+  const size_t smem = ffma_smem_bytes(NT_FFMA, true);
+  if (h->grid.f16) k_render_ffma<true, NT_FFMA><<<grid, NT_FFMA, smem, (cudaStream_t)stream>>>(h->grid, h->env, h->shade, h->d_wts, fr, rgb);
+  else k_render_ffma<false, NT_FFMA><<<grid, NT_FFMA, smem, (cudaStream_t)stream>>>(h->grid, h->env, h->shade, h->d_wts, fr, rgb);
+  h->launches++;
+  HR_CUDA(h, cudaGetLastError());
+  return HR_OK;
+}
+
+int hashrender_render_frame_host(hashrender_t* h, const hr_frame* f, float* rgb, void* stream, uint64_t* h2d_bytes, uint64_t* d2h_bytes) {
+  if (!h) return HR_ERR_INVALID_ARG;
+  if (h2d_bytes) *h2d_bytes = 0;
+  if (d2h_bytes) *d2h_bytes = 0;
+  if (int e = check_frame(h, f, rgb)) return e;
+  if (f->N == 0) return HR_OK;
+  cudaStream_t st = (cudaStream_t)stream;
+  uint64_t up = 0;
+  int slot = 0;
+  int rc = HR_OK;
+  auto stage = [&](const void* src, size_t bytes) -> const void* {
+    if (!src || rc != HR_OK) return nullptr;
+    const int s = slot++;
+    if (bytes > h->stage_cap[s]) {
+      cudaFree(h->stage[s]); h->stage[s] = nullptr; h->stage_cap[s] = 0;
+      cudaError_t e = cudaMalloc(&h->stage[s], bytes);
+      if (e != cudaSuccess) { rc = fail(h, HR_ERR_OOM, "render_frame_host: staging alloc of %zu bytes failed", bytes); return nullptr; }
+      h->stage_cap[s] = bytes;
+    }
+    cudaError_t e = cudaMemcpyAsync(h->stage[s], src, bytes, cudaMemcpyHostToDevice, st);
+    if (e != cudaSuccess) { rc = fail(h, HR_ERR_CUDA, "render_frame_host: H2D failed: %s", cudaGetErrorString(e)); return nullptr; }
+    up += bytes;
+    return h->stage[s];
+  };
+  auto stage_set = [&](const hr_dirset& d, uint64_t rows, bool used) -> hr_dirset {
+    hr_dirset o = d;
+    if (!used) { slot += 3; return o; }
+    const uint64_t R = d.point_stride ? rows : 1;
+    const uint64_t dir_elems = d.point_stride ? (R - 1) * d.point_stride + 3ull * d.S : 3ull * d.S;
+    const uint64_t pdf_elems = d.point_stride ? (R - 1) * (d.point_stride / 3) + d.S : d.S;
+    o.dir = (const float*)stage(d.dir, dir_elems * 4);
+    o.pdf = (const float*)stage(d.pdf, pdf_elems * 4);
+    if (d.Lin) o.Lin = (const float*)stage(d.Lin, dir_elems * 4); else slot++;
+    return o;
+  };
+  hr_frame df = *f;
+  df.x = (const float*)stage(f->x, f->N * 12);
+  if (f->brdf) df.brdf = (const float*)stage(f->brdf, f->N * 28); else slot++;
+  df.wo = (const float*)stage(f->wo, f->N * 12);
+  if (f->mask) df.mask = (const uint8_t*)stage(f->mask, f->N); else slot++;
+  df.direct = stage_set(f->direct, f->N, f->flags & HR_DIRECT);
+  df.secondary = stage_set(f->secondary, f->N, f->flags & HR_INDIRECT);
+  df.tertiary = stage_set(f->tertiary, f->N * (uint64_t)f->secondary.S, f->flags & HR_INDIRECT);
+  if (rc != HR_OK) return rc;
+  const int s_rgb = 15;
+  if (f->N * 12 > h->stage_cap[s_rgb]) {
+    cudaFree(h->stage[s_rgb]); h->stage[s_rgb] = nullptr; h->stage_cap[s_rgb] = 0;
+    HR_CUDA(h, cudaMalloc(&h->stage[s_rgb], f->N * 12));
+    h->stage_cap[s_rgb] = f->N * 12;
+  }
+  if (int e = hashrender_render_frame(h, &df, (float*)h->stage[s_rgb], stream)) return e;
+  HR_CUDA(h, cudaMemcpyAsync(rgb, h->stage[s_rgb], f->N * 12, cudaMemcpyDeviceToHost, st));
+  HR_CUDA(h, cudaStreamSynchronize(st));
+  if (h2d_bytes) *h2d_bytes = up;
+  if (d2h_bytes) *d2h_bytes = f->N * 12;
+  return HR_OK;
+}
+
+uint64_t hashrender_launch_count(const hashrender_t* h) { return h ? h->launches : 0; }
+const char* hashrender_last_path(const hashrender_t* h) { return h ? h->last_path : "none"; }
+const char* hashrender_last_error(const hashrender_t* h) { return h ? h->err : "NULL handle"; }
+
+}  // extern "C"

@@ -1,0 +1,212 @@
+// hr_device.cuh -- parameter blocks and per-thread device math shared by the hashrender kernels:
+// hash-grid encode, output maps, env lookup, BRDF
+// (PAPER.md:62, 122, 128, 252), secondary hit.  fp32 throughout; the index path is kept to
+// single IEEE operations (__fmul_rn / __fsub_rn) so integer outputs are bit-exact (Q4).
+#pragma once
+#include <cuda_fp16.h>
+#include <stdint.h>
+
+namespace hr {
+
+constexpr int kMaxL = 16;   // levels
+constexpr int kD = 32;      // padded feature width (L*F <= 32, F == 2)
+constexpr int kH = 64;      // hidden width
+
+struct GridP {
+  uint32_t L, log2_T, dense_mask, f16;
+  uint32_t res[kMaxL];
+  const void* tables;       // [L][T] of float2 (f16 == 0) or __half2 (f16 == 1)
+};
+struct EnvP { const float* env; uint32_t He, We; };
+struct ShadeP {
+  float near_t, far_t, rough_min, f0;
+  uint32_t vis_mode, brdf_model;
+  float as0, as1, as2;
+};
+struct DirsetP {
+  const float* dir; const float* pdf; const float* Lin;
+  uint32_t S; unsigned long long stride;
+};
+struct FrameP {
+  unsigned long long N;
+  const float* x; const float* brdf; const float* wo; const uint8_t* mask;
+  DirsetP d, s, t;
+  uint32_t flags;
+};
+
+__device__ __forceinline__ const float* dir_of(const DirsetP& d, unsigned long long i, uint32_t s) {
+  return d.dir + i * d.stride + 3ull * s;
+}
+__device__ __forceinline__ float pdf_of(const DirsetP& d, unsigned long long i, uint32_t s) {
+  return __ldg(d.pdf + i * (d.stride / 3ull) + s);
+}
+
+// ---- a1/a2: level scale, corner select, spatial hash / dense index ---------------------------------
+struct Cell { uint32_t c0[3]; float w[3]; };
+
+__device__ __forceinline__ Cell cell_of(uint32_t N, float x, float y, float z) {
+  Cell c;
+  const float fn = (float)N;
+  const float p[3] = {__fmul_rn(fminf(fmaxf(x, 0.f), 1.f), fn), __fmul_rn(fminf(fmaxf(y, 0.f), 1.f), fn),
+                      __fmul_rn(fminf(fmaxf(z, 0.f), 1.f), fn)};
+#pragma unroll
+  for (int d = 0; d < 3; ++d) {
+    int fl = min(__float2int_rd(p[d]), (int)N - 1);          // Q7: x == 1 -> c0 = N-1, w = 1
+    c.c0[d] = (uint32_t)fl;
+    c.w[d] = __fsub_rn(p[d], (float)fl);
+  }
+  return c;
+}
+
+__device__ __forceinline__ void corner_indices(const Cell& c, uint32_t N, bool dense, uint32_t log2_T, uint32_t (&idx)[8]) {
+  if (dense) {                                                // (N+1)^3 <= T (Q3)
+    const uint32_t s = N + 1, s2 = s * s;
+    const uint32_t base = c.c0[0] + c.c0[1] * s + c.c0[2] * s2;
+#pragma unroll
+    for (int k = 0; k < 8; ++k) idx[k] = base + (k & 1) + ((k >> 1) & 1) * s + ((k >> 2) & 1) * s2;
+  } else {                                                    // hash of [14], primes (1, 2654435761, 805459861) (Q1)
+    const uint32_t mask = (1u << log2_T) - 1u;
+    const uint32_t hx[2] = {c.c0[0], c.c0[0] + 1u};
+    const uint32_t hy[2] = {c.c0[1] * 2654435761u, (c.c0[1] + 1u) * 2654435761u};
+    const uint32_t hz[2] = {c.c0[2] * 805459861u, (c.c0[2] + 1u) * 805459861u};
+#pragma unroll
+    for (int k = 0; k < 8; ++k) idx[k] = (hx[k & 1] ^ hy[(k >> 1) & 1] ^ hz[(k >> 2) & 1]) & mask;
+  }
+}
+
+template <bool F16>
+__device__ __forceinline__ float2 table_load(const void* tables, uint32_t log2_T, int l, uint32_t idx) {
+  const size_t off = ((size_t)l << log2_T) + idx;
+  if (F16) {
+    const __half2 v = __ldg(reinterpret_cast<const __half2*>(tables) + off);
+    return __half22float2(v);
+  } else {
+    return __ldg(reinterpret_cast<const float2*>(tables) + off);
+  }
+}
+
+// a3/a4: gather 8 corners of one level and interpolate.  Corner number b0 + 2 b1 + 4 b2 (Q9).
+template <bool F16>
+__device__ __forceinline__ float2 encode_level(const GridP& g, int l, float x, float y, float z,
+                                               uint32_t* idx_out, float* w_out) {
+  const uint32_t N = g.res[l];
+  const Cell c = cell_of(N, x, y, z);
+  uint32_t idx[8];
+  corner_indices(c, N, (g.dense_mask >> l) & 1u, g.log2_T, idx);
+  float2 v[8];
+#pragma unroll
+  for (int k = 0; k < 8; ++k) v[k] = table_load<F16>(g.tables, g.log2_T, l, idx[k]);
+  if (idx_out) {
+#pragma unroll
+    for (int k = 0; k < 8; ++k) idx_out[k] = idx[k];
+  }
+  if (w_out) { w_out[0] = c.w[0]; w_out[1] = c.w[1]; w_out[2] = c.w[2]; }
+  const float wx[2] = {1.f - c.w[0], c.w[0]}, wy[2] = {1.f - c.w[1], c.w[1]}, wz[2] = {1.f - c.w[2], c.w[2]};
+  float2 f = make_float2(0.f, 0.f);
+#pragma unroll
+  for (int k = 0; k < 8; ++k) {
+    const float wt = wx[k & 1] * wy[(k >> 1) & 1] * wz[(k >> 2) & 1];
+    f.x = fmaf(wt, v[k].x, f.x);
+    f.y = fmaf(wt, v[k].y, f.y);
+  }
+  return f;
+}
+
+// f = H(x), zero-padded to kD entries.
+template <bool F16>
+__device__ __forceinline__ void encode_point(const GridP& g, float x, float y, float z, float (&f)[kD]) {
+#pragma unroll
+  for (int l = 0; l < kMaxL; ++l) {
+    if (l < (int)g.L) {
+      const float2 v = encode_level<F16>(g, l, x, y, z, nullptr, nullptr);
+      f[2 * l] = v.x; f[2 * l + 1] = v.y;
+    } else {
+      f[2 * l] = 0.f; f[2 * l + 1] = 0.f;
+    }
+  }
+}
+
+// ---- output maps ------------------------------------------------------------------------------------
+__device__ __forceinline__ float sigmoidf_(float z) { return 1.f / (1.f + expf(-z)); }
+
+// o[0..6] raw B outputs -> n/||n||, sigma(a)*scale, rough_min + sigma(r)(1 - rough_min)  (Q12)
+__device__ __forceinline__ void brdf_maps(const ShadeP& sp, const float (&o)[8], float (&b)[7]) {
+  const float nn = fmaxf(sqrtf(o[0] * o[0] + o[1] * o[1] + o[2] * o[2]), 1e-12f);
+  const float inv = 1.f / nn;
+  b[0] = o[0] * inv; b[1] = o[1] * inv; b[2] = o[2] * inv;
+  b[3] = sigmoidf_(o[3]) * sp.as0; b[4] = sigmoidf_(o[4]) * sp.as1; b[5] = sigmoidf_(o[5]) * sp.as2;
+  b[6] = sp.rough_min + sigmoidf_(o[6]) * (1.f - sp.rough_min);
+}
+
+// (z_v, z_t) -> v, t  (Q14, Q15).  softplus(z) >= 1 iff z >= ln(e-1), so the clamp
+// removes the large-z branch.
+__device__ __forceinline__ void irt_maps(const ShadeP& sp, float zv, float zt, float& v, float& t) {
+  v = sp.vis_mode ? (zv > 0.f ? 1.f : 0.f) : sigmoidf_(zv);
+  const float d = zt > 0.6f ? 1.f : fminf(log1pf(expf(zt)), 1.f);
+  t = sp.near_t + d * (sp.far_t - sp.near_t);
+}
+
+// a7: x' = clamp(x + t w, 0, 1)  (Q6, Q20)
+__device__ __forceinline__ float sec_hit(float x, float t, float w) { return fminf(fmaxf(fmaf(t, w, x), 0.f), 1.f); }
+
+// ---- a9: equirect bilinear env lookup (Q25) ------------------------------------------------
+__device__ __forceinline__ float3 env_lookup(const EnvP& e, float wx, float wy, float wz) {
+  const float theta = acosf(fminf(fmaxf(wz, -1.f), 1.f));
+  const float phi = atan2f(wy, wx);
+  const float u = (phi * 0.15915494309189535f + 0.5f) * (float)e.We - 0.5f;
+  const float s = (theta * 0.3183098861837907f) * (float)e.He - 0.5f;
+  const float u0 = floorf(u), s0 = floorf(s);
+  const float fu = u - u0, fs = s - s0;
+  const int We = (int)e.We, He = (int)e.He;
+  int x0 = (int)u0 % We; if (x0 < 0) x0 += We;
+  int x1 = x0 + 1; if (x1 == We) x1 = 0;
+  const int y0 = min(max((int)s0, 0), He - 1), y1 = min(max((int)s0 + 1, 0), He - 1);
+  const float* r0 = e.env + (size_t)y0 * We * 3;
+  const float* r1 = e.env + (size_t)y1 * We * 3;
+  float out[3];
+#pragma unroll
+  for (int ch = 0; ch < 3; ++ch) {
+    const float e00 = __ldg(r0 + x0 * 3 + ch), e01 = __ldg(r0 + x1 * 3 + ch);
+    const float e10 = __ldg(r1 + x0 * 3 + ch), e11 = __ldg(r1 + x1 * 3 + ch);
+    out[ch] = (1.f - fs) * ((1.f - fu) * e00 + fu * e01) + fs * ((1.f - fu) * e10 + fu * e11);
+  }
+  return make_float3(out[0], out[1], out[2]);
+}
+
+// ---- a10: f_r (n.w_i)^+ / p per channel (Q21-Q23) ---------------------------
+__device__ __forceinline__ float3 brdf_cos_over_pdf(const ShadeP& sp, const float (&b)[7], float wix, float wiy, float wiz,
+                                                    float wox, float woy, float woz, float pdf) {
+  const float NoL = b[0] * wix + b[1] * wiy + b[2] * wiz;
+  if (!(NoL > 0.f) || !(pdf > 0.f)) return make_float3(0.f, 0.f, 0.f);
+  float spec = 0.f;
+  if (sp.brdf_model == 1) {
+    const float NoV = fmaxf(b[0] * wox + b[1] * woy + b[2] * woz, 1e-4f);
+    float hx = wix + wox, hy = wiy + woy, hz = wiz + woz;
+    const float hn = 1.f / fmaxf(sqrtf(hx * hx + hy * hy + hz * hz), 1e-12f);
+    hx *= hn; hy *= hn; hz *= hn;
+    const float NoH = fmaxf(b[0] * hx + b[1] * hy + b[2] * hz, 0.f);
+    const float VoH = fmaxf(wox * hx + woy * hy + woz * hz, 0.f);
+    const float alpha = b[6] * b[6], k = alpha * alpha;
+    const float dd = NoH * NoH * (k - 1.f) + 1.f;
+    const float D = k / (3.14159265358979f * dd * dd);
+    const float m = 1.f - VoH, m2 = m * m;
+    const float F = sp.f0 + (1.f - sp.f0) * (m2 * m2 * m);
+    const float Gv = 0.5f / (NoL * sqrtf(NoV * NoV * (1.f - k) + k) + NoV * sqrtf(NoL * NoL * (1.f - k) + k));
+    spec = D * F * Gv;
+  }
+  const float sc = NoL / pdf;
+  const float ipi = 0.3183098861837907f;
+  return make_float3((b[3] * ipi + spec) * sc, (b[4] * ipi + spec) * sc, (b[5] * ipi + spec) * sc);
+}
+
+// incoming radiance for direction s of point-row i (Lin if supplied, else the env map)
+__device__ __forceinline__ float3 incoming(const EnvP& e, const DirsetP& d, unsigned long long i, uint32_t s,
+                                           float wx, float wy, float wz) {
+  if (d.Lin) {
+    const float* p = d.Lin + i * d.stride + 3ull * s;
+    return make_float3(__ldg(p), __ldg(p + 1), __ldg(p + 2));
+  }
+  return env_lookup(e, wx, wy, wz);
+}
+
+}  // namespace hr

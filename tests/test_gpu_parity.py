@@ -1,0 +1,302 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle on identical seeded inputs.
+
+Bars (BASELINE.json north_star; Q32/Q33): hash indices / corner selection / fractional weights
+bit-exact; floating point within 1e-4 relative (fp32) or 3e-3 (fp16 tables/weights), relative to
+max(|o|, mean|o|); hard visibility may flip only where |z_v| < delta (flipbound rule).
+"""
+import numpy as np
+import pytest
+
+import gen
+from hr_testutil import check_close, gpu_render, make_renderer, oracle_render, to_dev
+
+pytestmark = pytest.mark.gpu
+
+TOL32, TOL16 = 1e-4, 3e-3
+DELTA32, DELTA16 = 2e-5, 4e-3      # |z_v| band in which a hard-visibility flip is legitimate (Q33)
+
+
+@pytest.fixture(scope="module")
+def torch():
+    import torch
+    assert torch.cuda.is_available()
+    return torch
+
+
+def _oracle(cfg, model, **kw):
+    from oracle.oracle import Oracle
+    return Oracle.from_gen(cfg, model, **kw)
+
+
+def _edge_points(rng, n):
+    x = rng.random((n, 3)).astype(np.float32)
+    x[:8] = [[0, 0, 0], [1, 1, 1], [0.5, 0.25, 0.125], [1, 0, 0.5], [3 / 16, 5 / 16, 1.0], [1e-8, 1 - 1e-7, 0.999999],
+             [-0.5, 2.0, 0.3], [0.0625, 0.9375, 0.5]]
+    return x
+
+
+# ---------------------------------------------------------------------------------------------- encode
+@pytest.mark.parametrize("name,n", [("C0", 4096), ("C1", 3001), ("C3", 1537)])
+def test_encode_bit_exact_indices_and_features(torch, name, n):
+    cfg = gen.make_config(name)
+    m = gen.make_model(cfg)
+    o = _oracle(cfg, m)
+    rng = np.random.default_rng(100)
+    x = _edge_points(rng, n)
+    if name == "C0":
+        x[8:] = gen.make_points(cfg)[0][8:n]
+    feat_o, idx_o, w_o = o.encode(x)
+    r = make_renderer(cfg, m)
+    feat = torch.empty((n, cfg.D), device="cuda"); idx = torch.empty((n, cfg.L, 8), device="cuda", dtype=torch.int32)
+    w = torch.empty((n, cfg.L, 3), device="cuda")
+    r.encode(to_dev(x), feat, idx, w)
+    torch.cuda.synchronize()
+    assert np.array_equal(idx.cpu().numpy().view(np.uint32), idx_o), "hash / dense indices must be bit-exact"
+    assert np.array_equal(w.cpu().numpy(), w_o), "fractional positions must be bit-exact"
+    check_close(feat.cpu().numpy(), feat_o, 2e-6, what=f"encode {name}")
+    # vertex reproduction on the GPU too: x on a level-0 vertex returns the table row exactly
+    v = np.array([[3 / 16, 5 / 16, 9 / 16]], np.float32)
+    f1 = torch.empty((1, cfg.D), device="cuda")
+    r.encode(to_dev(v), f1)
+    row = 3 + 5 * 17 + 9 * 17 * 17
+    assert np.array_equal(f1.cpu().numpy()[0, :2], m["tables"][0, row])
+
+
+def test_encode_empty_and_errors(torch):
+    from paper_2409_10327_b200 import HashRenderError
+    cfg = gen.make_config("C0")
+    m = gen.make_model(cfg)
+    r = make_renderer(cfg, m)
+    feat = torch.empty((4, cfg.D), device="cuda")
+    r.encode(to_dev(np.zeros((0, 3), np.float32)), feat)            # N == 0: no-op
+    with pytest.raises(HashRenderError) as e:
+        r.encode(None, feat, N=4)
+    assert e.value.code == 1
+    with pytest.raises(HashRenderError):
+        r.encode(to_dev(np.zeros((4, 3), np.float32)), feat, N=cfg.N * 1000)     # N > max_points
+    with pytest.raises(HashRenderError) as e:
+        make_renderer(cfg, m, F=4, tables=np.zeros((cfg.L, cfg.T, 4), np.float32),
+                      brdf_w=np.zeros(64 * 32 + 64 + 64 * 64 + 64 + 7 * 64 + 7, np.float32),
+                      irt_w=np.zeros(64 * 35 + 64 + 64 * 64 + 64 + 2 * 64 + 2, np.float32))
+    assert e.value.code == 4
+
+
+# ---------------------------------------------------------------------------------------------- decode / trace / shade
+@pytest.mark.parametrize("name", ["C0", "C1", "C3"])
+def test_decode_trace_shade_stagewise(torch, name):
+    """Stage-wise parity on ORACLE-supplied inputs (the strict test, SURVEY 8(c) conditioning note)."""
+    cfg = gen.make_config(name)
+    m = gen.make_model(cfg)
+    n = 777
+    pix = np.arange(0, cfg.N, cfg.N // n)[:n]
+    fr = gen.make_frame(cfg, m["env"], pix)
+    tol = TOL16 if cfg.mlp_dtype == "f16" else TOL32
+    o = _oracle(cfg, m)
+    feat_o, _, _ = o.encode(fr["x"])
+    brdf_o = o.decode(feat_o)
+    vis_o, zv_o, t_o, xs_o = o.trace(fr["x"], feat_o, fr["dir_d"])
+    r = make_renderer(cfg, m)
+    featd = to_dev(feat_o.astype(np.float32))
+    S = cfg.S_d
+    # decode
+    brdf = torch.empty((n, 7), device="cuda")
+    r.decode(featd, brdf)
+    check_close(brdf.cpu().numpy(), brdf_o, tol, what="decode")
+    # trace on oracle features, then with the encode fused
+    from paper_2409_10327_b200 import DirSet
+    ds = DirSet(to_dev(fr["dir_d"]), to_dev(fr["pdf_d"]))
+    for fused in (False, True):
+        vis = torch.empty((n, S), device="cuda"); zv = torch.empty((n, S), device="cuda"); t = torch.empty((n, S), device="cuda")
+        xs = torch.empty((n, S, 3), device="cuda")
+        r.trace(to_dev(fr["x"]), None if fused else featd, ds, vis, zv, t, xs)
+        torch.cuda.synchronize()
+        check_close(vis.cpu().numpy(), vis_o, tol, what="trace vis")
+        check_close(t.cpu().numpy(), t_o, tol, what="trace t")
+        check_close(zv.cpu().numpy(), zv_o, tol, extra=tol * 0.05, what="trace zv")
+        check_close(xs.cpu().numpy(), xs_o, tol, what="trace x'")
+    # hard mode: bits agree wherever |z_v| >= delta
+    oh = _oracle(cfg, m, vis_mode=1)
+    vh_o, zvh_o, _, _ = oh.trace(fr["x"], feat_o, fr["dir_d"])
+    rh = make_renderer(cfg, m, vis_mode=1)
+    vis = torch.empty((n, S), device="cuda"); t = torch.empty((n, S), device="cuda")
+    rh.trace(to_dev(fr["x"]), featd, ds, vis, None, t)
+    vh = vis.cpu().numpy()
+    assert set(np.unique(vh)) <= {0.0, 1.0}
+    delta = DELTA16 if cfg.mlp_dtype == "f16" else DELTA32
+    sure = np.abs(zvh_o) >= delta
+    assert np.array_equal(vh[sure], vh_o[sure])
+    assert sure.mean() > 0.9
+    # shade: direct only, then Eq. 2 on one set with a synthetic L'_o
+    rng = np.random.default_rng(5)
+    Lind = rng.random((n, S, 3)).astype(np.float32)
+    for terms, li in ((1, None), (3, Lind), (2, Lind)):
+        rgb_o = o.shade(brdf_o, fr["wo"], fr["dir_d"], fr["pdf_d"], vis_o, Lind=li, terms=terms)
+        rgb = torch.empty((n, 3), device="cuda")
+        r.shade(to_dev(brdf_o.astype(np.float32)), to_dev(fr["wo"]), ds, to_dev(vis_o.astype(np.float32)),
+                None if li is None else to_dev(li), terms, rgb)
+        check_close(rgb.cpu().numpy(), rgb_o, TOL32, what=f"shade terms={terms}")
+
+
+def test_trace_shared_set_and_ragged(torch):
+    cfg = gen.make_config("C0")
+    m = gen.make_model(cfg)
+    o = _oracle(cfg, m)
+    from paper_2409_10327_b200 import DirSet
+    for n in (1, 31, 257, 1000):
+        fr = gen.make_frame(cfg, m["env"], np.arange(n))
+        feat_o, _, _ = o.encode(fr["x"])
+        vis_o, zv_o, t_o, xs_o = o.trace(fr["x"], feat_o, fr["dir_t"], shared=True)
+        r = make_renderer(cfg, m)
+        S = cfg.S_2
+        vis = torch.empty((n, S), device="cuda"); t = torch.empty((n, S), device="cuda"); xs = torch.empty((n, S, 3), device="cuda")
+        r.trace(to_dev(fr["x"]), None, DirSet(to_dev(fr["dir_t"]), to_dev(fr["pdf_t"])), vis, None, t, xs)
+        check_close(vis.cpu().numpy(), vis_o, TOL32, what="trace shared vis")
+        check_close(xs.cpu().numpy(), xs_o, TOL32, what="trace shared x'")
+
+
+# ---------------------------------------------------------------------------------------------- whole frames
+def _frame_case(torch, name, pix, vis_mode, flags=None, over=None, tol=None, delta=None, brdf=None, mask=None):
+    cfg = gen.make_config(name, **(over or {}))
+    m = gen.make_model(cfg)
+    fr = gen.make_frame(cfg, m["env"], pix)
+    f16 = cfg.mlp_dtype == "f16"
+    tol = tol or (TOL16 if f16 else TOL32)
+    delta = delta if delta is not None else (DELTA16 if f16 else DELTA32)
+    o = _oracle(cfg, m, vis_mode=vis_mode)
+    ref = oracle_render(o, cfg, fr, flags=flags, delta=delta if vis_mode else 0.0, brdf=brdf, mask=mask)
+    r = make_renderer(cfg, m, vis_mode=vis_mode)
+    got = gpu_render(r, cfg, fr, flags=flags, brdf=brdf, mask=mask)
+    worst = check_close(got, ref["rgb"], tol, extra=ref["flipbound"] if vis_mode else None, what=f"{name} vis_mode={vis_mode}")
+    return cfg, ref, got, worst, r
+
+
+@pytest.mark.parametrize("vis_mode", [0, 1])
+def test_frame_C0_full(torch, vis_mode):
+    cfg, ref, got, worst, _ = _frame_case(torch, "C0", None, vis_mode)
+    assert np.abs(ref["rgb"]).max() > 0.1
+    if vis_mode:          # the flip allowance must stay a rare exception, not the rule
+        assert (ref["flipbound"].max(axis=1) > 0).mean() < 0.05
+
+
+@pytest.mark.parametrize("vis_mode", [0, 1])
+def test_frame_C1_subset(torch, vis_mode):
+    pix = np.concatenate([np.arange(0, 640000, 313), [0, 799, 639200, 639999]])
+    _frame_case(torch, "C1", pix, vis_mode)
+
+
+@pytest.mark.parametrize("vis_mode", [0, 1])
+def test_frame_C2_subset(torch, vis_mode):
+    """One-bounce indirect, fp32: 1e-4 (soft); hard adds the flip allowance."""
+    pix = np.concatenate([np.arange(0, 640000, 1259), [0, 799, 639200, 639999]])
+    cfg, ref, got, worst, _ = _frame_case(torch, "C2", pix, vis_mode)
+    assert ref["n_sec"] == len(pix) * 64
+
+
+@pytest.mark.parametrize("name", ["C3", "C3a"])
+@pytest.mark.parametrize("vis_mode", [0, 1])
+def test_frame_C3_fp16_subset(torch, name, vis_mode):
+    pix = np.concatenate([np.arange(0, 640000, 1259), [0, 799, 639200, 639999]])
+    _frame_case(torch, name, pix, vis_mode)
+
+
+def test_frame_variants_small(torch):
+    """External BRDF (Q30), mask (Q27), Lambert model, flag subsets, per-secondary-point tertiary sets, ragged N."""
+    rng = np.random.default_rng(9)
+    n = 333
+    pix = np.arange(n)
+    over = dict(S_i=4, S_2=3, flags=7)
+    cfg = gen.make_config("C0", **over)
+    brdf = np.concatenate([gen._normalize(rng.standard_normal((n, 3))), rng.random((n, 3)), 0.09 + 0.91 * rng.random((n, 1))], 1).astype(np.float32)
+    mask = (rng.random(n) > 0.3).astype(np.uint8)
+    _frame_case(torch, "C0", pix, 0, over=over, brdf=brdf, mask=mask)
+    for flags in (1, 3, 4, 6, 5):
+        _frame_case(torch, "C0", pix, 0, flags=flags, over=over)
+    # Lambert
+    m = gen.make_model(cfg); fr = gen.make_frame(cfg, m["env"], pix)
+    o = _oracle(cfg, m, brdf_model=0)
+    ref = oracle_render(o, cfg, fr, flags=7)
+    got = gpu_render(make_renderer(cfg, m, brdf_model=0), cfg, fr, flags=7)
+    check_close(got, ref["rgb"], TOL32, what="lambert")
+    # per-secondary-point tertiary sets (point_stride != 0, the paper's literal reading of PAPER.md:344)
+    dt = gen._normalize(rng.standard_normal((n * 4, 3, 3))).astype(np.float32)
+    dt = gen._normalize(dt.astype(np.float64)).astype(np.float32)
+    pt = np.full((n * 4, 3), 1 / (4 * np.pi), np.float32)
+    fr2 = dict(fr); fr2["dir_t"], fr2["pdf_t"] = dt, pt
+    o = _oracle(cfg, m)
+    ref = oracle_render(o, cfg, fr2, flags=7)
+    got = gpu_render(make_renderer(cfg, m), cfg, fr2, flags=7)
+    check_close(got, ref["rgb"], TOL32, what="per-point tertiary")
+
+
+def test_frame_closed_form_on_gpu(torch):
+    """The a*L closed form (Eq. 1) evaluated by the CUDA path itself: Lambert, v == 1, constant env,
+    cosine pdf => every pixel equals albedo * L."""
+    cfg = gen.make_config("C0")
+    m = gen.make_model(cfg)
+    m = {**m, "env": np.full((16, 32, 3), 1.75, np.float32)}
+    fr = gen.make_frame(cfg, m["env"], np.arange(500))
+    rng = np.random.default_rng(2)
+    a = rng.random((500, 3)).astype(np.float32)
+    brdf = np.concatenate([fr["n_g"], a, np.full((500, 1), 0.5, np.float32)], 1)
+    # pdf consistent with the fp32 directions and normals actually passed
+    fr["pdf_d"] = (np.einsum("nsk,nk->ns", fr["dir_d"].astype(np.float64), fr["n_g"].astype(np.float64)) / np.pi).astype(np.float32)
+    got = gpu_render(make_renderer(cfg, m, brdf_model=0), cfg, fr, flags=1, brdf=brdf)
+    np.testing.assert_allclose(got, a * 1.75, rtol=2e-5)
+
+
+def test_render_frame_host_matches_device(torch):
+    cfg = gen.make_config("C0", S_i=4, S_2=3, flags=7)
+    m = gen.make_model(cfg)
+    fr = gen.make_frame(cfg, m["env"], np.arange(1000))
+    r = make_renderer(cfg, m)
+    a = gpu_render(r, cfg, fr)
+    b = gpu_render(r, cfg, fr, host=True)
+    assert np.array_equal(a, b)
+    assert r.launch_count() >= 2
+
+
+def test_frame_errors(torch):
+    from paper_2409_10327_b200 import DirSet, HashRenderError
+    cfg = gen.make_config("C0")
+    m = gen.make_model(cfg)
+    fr = gen.make_frame(cfg, m["env"], np.arange(64))
+    from paper_2409_10327_b200 import HashRenderer
+    r = HashRenderer.from_gen(cfg, m)                       # no env set
+    x, wo = to_dev(fr["x"]), to_dev(fr["wo"])
+    d = DirSet(to_dev(fr["dir_d"]), to_dev(fr["pdf_d"]))
+    rgb = torch.empty((64, 3), device="cuda")
+    with pytest.raises(HashRenderError) as e:
+        r.render_frame(r.make_frame(x, wo, d), rgb)
+    assert e.value.code == 1 and "env" in str(e.value)
+    r.set_env(to_dev(m["env"]))
+    with pytest.raises(HashRenderError):
+        r.render_frame(r.make_frame(x, wo, d, flags=0), rgb)
+    with pytest.raises(HashRenderError):
+        r.render_frame(r.make_frame(x, wo, d, flags=7), rgb)            # INDIRECT without secondary set
+    r.render_frame(r.make_frame(x, wo, d, N=0), rgb)                    # N == 0 no-op
+    r.render_frame(r.make_frame(x, wo, d), rgb)
+    torch.cuda.synchronize()
+
+
+# ---------------------------------------------------------------------------------------------- full size, bench configuration
+@pytest.mark.parametrize("name", ["C2", "C3"])
+def test_full_size_sampled_pixels(torch, name):
+    """BASELINE full size (800x800, 128 + 64x8 directions) in the launch configuration bench.py times; the oracle
+    checks a seeded sample of pixels one by one (it needs ~6 ms per pixel)."""
+    cfg = gen.make_config(name)
+    m = gen.make_model(cfg)
+    fr = gen.make_frame(cfg, m["env"])
+    r = make_renderer(cfg, m, vis_mode=1)
+    got = gpu_render(r, cfg, fr)
+    assert np.all(np.isfinite(got)) and got.shape == (cfg.N, 3)
+    rng = np.random.default_rng(77)
+    pix = np.sort(np.concatenate([rng.choice(cfg.N, 188, replace=False), [0, 799, 639200, 639999]]))
+    sub = {k: (v[pix] if k not in ("dir_t", "pdf_t") else v) for k, v in fr.items()}
+    f16 = cfg.mlp_dtype == "f16"
+    o = _oracle(cfg, m, vis_mode=1)
+    ref = oracle_render(o, cfg, sub, delta=DELTA16 if f16 else DELTA32)
+    # tolerance scale s (mean |o|) from the sample itself
+    check_close(got[pix], ref["rgb"], TOL16 if f16 else TOL32, extra=ref["flipbound"], what=f"{name} full-size sample")
+    # a generator subset reproduces the same inputs as the full frame (so bench's CPU sample is the same workload)
+    fr_sub = gen.make_frame(cfg, m["env"], pix)
+    assert np.array_equal(fr_sub["dir_d"], sub["dir_d"]) and np.array_equal(fr_sub["x"], sub["x"])
