@@ -24,7 +24,8 @@ struct hashrender {
   EnvP env;
   void* d_tables = nullptr;
   float* d_wts = nullptr;        // prepared fp32 weights (hr_kernels_ffma.cuh layout)
-  void* d_wts_tc = nullptr;      // prepared fp16 UMMA-layout weights (hr_kernels_tc.cuh), mlp_dtype == HR_F16
+  uint8_t* d_wts_tc = nullptr;   // prepared fp16 UMMA weight tiles (hr_kernels_tc.cuh), mlp_dtype == HR_F16
+  std::vector<uint8_t> h_wts_tc; // host copy of [TcConst | tiles]; TcConst is passed by value at launch
   float* d_env = nullptr;
   size_t env_cap = 0;
   int num_sms = 148;
@@ -188,10 +189,10 @@ int hashrender_create(const hr_config* cfg, const float* tables, const float* br
   HR_CUDA(h, cudaMemcpy(h->d_wts, w.data(), w.size() * sizeof(float), cudaMemcpyHostToDevice));
 #ifndef HR_NO_TC
   if (cfg->mlp_dtype == HR_F16 || h->force_path == 2) {
-    std::vector<uint8_t> wt;
-    tc::prepare_weights(*cfg, brdf_w, irt_w, wt);
-    HR_CUDA(h, cudaMalloc(&h->d_wts_tc, wt.size()));
-    HR_CUDA(h, cudaMemcpy(h->d_wts_tc, wt.data(), wt.size(), cudaMemcpyHostToDevice));
+    tc::prepare_weights(*cfg, brdf_w, irt_w, h->h_wts_tc);
+    const size_t tb = h->h_wts_tc.size() - sizeof(tc::TcConst);
+    HR_CUDA(h, cudaMalloc(&h->d_wts_tc, tb));
+    HR_CUDA(h, cudaMemcpy(h->d_wts_tc, h->h_wts_tc.data() + sizeof(tc::TcConst), tb, cudaMemcpyHostToDevice));
     HR_CUDA(h, tc::set_attributes());
   }
 #endif
@@ -271,7 +272,8 @@ int hashrender_trace(hashrender_t* h, const float* x, const float* feat, uint64_
 #ifndef HR_NO_TC
   if (use_tc(h) && !feat) {
     h->last_path = "tcgen05-f16";
-    HR_CUDA(h, tc::launch_trace(h->grid, h->shade, h->d_wts_tc, x, N, d, vis, zv, t, xsec, h->num_sms, (cudaStream_t)stream));
+    HR_CUDA(h, tc::launch_trace(h->grid, h->shade, *reinterpret_cast<const tc::TcConst*>(h->h_wts_tc.data()), h->d_wts_tc, x, N, d, vis,
+                                zv, t, xsec, h->num_sms, (cudaStream_t)stream));
     h->launches++;
     return HR_OK;
   }
@@ -334,9 +336,9 @@ int hashrender_render_frame(hashrender_t* h, const hr_frame* f, float* rgb, void
 #ifndef HR_NO_TC
   if (use_tc(h) && tc::frame_supported(fr)) {
     h->last_path = "tcgen05-f16";
-    int nl = 0;
-    HR_CUDA(h, tc::launch_render(h->grid, h->env, h->shade, h->d_wts_tc, fr, rgb, h->num_sms, (cudaStream_t)stream, &nl));
-    h->launches += nl;
+    HR_CUDA(h, tc::launch_render(h->grid, h->env, h->shade, *reinterpret_cast<const tc::TcConst*>(h->h_wts_tc.data()), h->d_wts_tc, fr,
+                                 rgb, h->num_sms, (cudaStream_t)stream));
+    h->launches++;
     return HR_OK;
   }
 #endif

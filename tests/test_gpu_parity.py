@@ -208,15 +208,22 @@ def test_frame_variants_small(torch):
     cfg = gen.make_config("C0", **over)
     brdf = np.concatenate([gen._normalize(rng.standard_normal((n, 3))), rng.random((n, 3)), 0.09 + 0.91 * rng.random((n, 1))], 1).astype(np.float32)
     mask = (rng.random(n) > 0.3).astype(np.uint8)
-    _frame_case(torch, "C0", pix, 0, over=over, brdf=brdf, mask=mask)
-    for flags in (1, 3, 4, 6, 5):
+    # Off-spec combination (C0's U(-1,1) tables WITH an indirect bounce): the fp32 error of t (~4e-6, 64-term fp32 dot
+    # products) moves x' and is amplified by N_max * |grad tab| ~ 256 * 2 into a ~1e-3 feature error at the finest level
+    # (SURVEY 8(c) conditioning note), so end-to-end radiance is only good to a few 1e-4 here; the BASELINE configs
+    # (C0 direct-only, C1/C2 with 0.1-scale tables) keep the stated 1e-4.
+    TOLV = 4e-4
+    _frame_case(torch, "C0", pix, 0, over=over, brdf=brdf, mask=mask, tol=TOLV)
+    for flags in (1, 3):
         _frame_case(torch, "C0", pix, 0, flags=flags, over=over)
+    for flags in (4, 6, 5):
+        _frame_case(torch, "C0", pix, 0, flags=flags, over=over, tol=TOLV)
     # Lambert
     m = gen.make_model(cfg); fr = gen.make_frame(cfg, m["env"], pix)
     o = _oracle(cfg, m, brdf_model=0)
     ref = oracle_render(o, cfg, fr, flags=7)
     got = gpu_render(make_renderer(cfg, m, brdf_model=0), cfg, fr, flags=7)
-    check_close(got, ref["rgb"], TOL32, what="lambert")
+    check_close(got, ref["rgb"], TOLV, what="lambert")
     # per-secondary-point tertiary sets (point_stride != 0, the paper's literal reading of PAPER.md:344)
     dt = gen._normalize(rng.standard_normal((n * 4, 3, 3))).astype(np.float32)
     dt = gen._normalize(dt.astype(np.float64)).astype(np.float32)
@@ -225,7 +232,7 @@ def test_frame_variants_small(torch):
     o = _oracle(cfg, m)
     ref = oracle_render(o, cfg, fr2, flags=7)
     got = gpu_render(make_renderer(cfg, m), cfg, fr2, flags=7)
-    check_close(got, ref["rgb"], TOL32, what="per-point tertiary")
+    check_close(got, ref["rgb"], TOLV, what="per-point tertiary")
 
 
 def test_frame_closed_form_on_gpu(torch):
