@@ -29,7 +29,7 @@ constexpr int kTileBytes = 64 * 128;          // one 64 x 64 fp16 K-major SW128 
 constexpr int kNumTiles = 4;                  // I.W1f(+b1), B.W1(+b1), I.W2, B.W2
 constexpr int kMaxS2 = 16;                    // shared tertiary set staged in smem
 // TMEM column map (per CTA): A operand (fp16 pairs) | constant bias K-step | accumulator
-constexpr uint32_t kColA = 0, kColOne = 32, kColD = 64;
+constexpr uint32_t kColA = 0, kColOne = 56, kColD = 64;   // a split-precision 64-wide A (cols 0..63) overwrites the bias step
 
 struct __align__(16) TcConst {                // lives in the kernel-parameter constant bank
   float w1w[3][kH];                           // I layer 1, direction columns
@@ -122,8 +122,10 @@ struct Ctx {
 };
 
 // One 128 x 64 layer: D = A[:, 0:16*ksteps] * W^T (+ bias K-step from tile columns 32..47 when with_bias).
+// split: A holds a hi block (columns 0..8*ksteps) and a lo block (the next 8*ksteps columns) of an error-compensated
+// fp16 pair; both are multiplied by the same (exact fp16) weights, so the layer input is good to ~2^-22.
 // Every thread must have issued its tcgen05.st of A before calling.  Returns when D is readable.
-__device__ __forceinline__ void mma_layer(Ctx& c, int tile, int ksteps, bool with_bias) {
+__device__ __forceinline__ void mma_layer(Ctx& c, int tile, int ksteps, bool with_bias, bool split = false) {
   wait_st();
   fence_before();
   __syncthreads();
@@ -131,6 +133,8 @@ __device__ __forceinline__ void mma_layer(Ctx& c, int tile, int ksteps, bool wit
     fence_after();
     const uint64_t bd = make_bdesc(c.tile[tile]);
     for (int k = 0; k < ksteps; ++k) mma_f16_ts(c.tD0, c.tA0 + 8 * k, bd + 2 * k, kIdesc, k > 0);
+    if (split)
+      for (int k = 0; k < ksteps; ++k) mma_f16_ts(c.tD0, c.tA0 + 8 * (ksteps + k), bd + 2 * k, kIdesc, 1u);
     if (with_bias) mma_f16_ts(c.tD0, c.tOne0, bd + 2 * 2, kIdesc, 1u);
     mma_commit(c.mbar);
   }
@@ -146,6 +150,28 @@ __device__ __forceinline__ void store_feat(const Ctx& c, const float (&f)[kD]) {
 #pragma unroll
   for (int k = 0; k < 16; ++k) r[k] = pack_rn(f[2 * k], f[2 * k + 1]);
   tmem_st16(c.tA, r);
+}
+
+// residual of an fp16x2 pack: (a - fp16(a), b - fp16(b)) packed again (the "lo" half of a hi/lo split)
+__device__ __forceinline__ uint32_t pack_lo(uint32_t hi, float a, float b) {
+  const float2 h = __half22float2(*reinterpret_cast<const __half2*>(&hi));
+  return pack_rn(a - h.x, b - h.y);
+}
+
+// f[32] -> A columns 0..15 (hi) and 16..31 (lo): split-precision features for the primary layer-1 partial P
+__device__ __forceinline__ void store_feat_split(const Ctx& c, const float (&f)[kD]) {
+  uint32_t r[32];
+#pragma unroll
+  for (int k = 0; k < 16; ++k) {
+    r[k] = pack_rn(f[2 * k], f[2 * k + 1]);
+    r[16 + k] = pack_lo(r[k], f[2 * k], f[2 * k + 1]);
+  }
+  tmem_st32(c.tA, r);
+}
+
+__device__ __forceinline__ void restore_one(const Ctx& c) {
+  uint32_t one[8] = {0x3C003C00u, 0u, 0u, 0u, 0u, 0u, 0u, 0u};     // bias K-step of A: [1, 1, 0, ... 0]
+  tmem_st8(c.tOne, one);
 }
 
 // epilogue of I: (z_v, z_t) = b3 + W3 relu(D + b2)
@@ -223,6 +249,26 @@ __device__ __forceinline__ void h1_from_smem(const Ctx& c, const TcConst& cw, co
       p[k] = pack_relu(a0, a1);
     }
     tmem_st16(c.tA + 16 * h, p);
+  }
+}
+// split-precision variant for the secondary set (its z_t becomes t and moves x': SURVEY 8(c) conditioning note):
+// h1 in fp32 -> hi (columns 0..31) + lo (columns 32..63)
+__device__ __forceinline__ void h1_from_smem_split(const Ctx& c, const TcConst& cw, const float* Ps, float wx, float wy, float wz) {
+#pragma unroll
+  for (int h = 0; h < 2; ++h) {
+    uint32_t p[16], q[16];
+#pragma unroll
+    for (int k = 0; k < 16; ++k) {
+      const int j = 32 * h + 2 * k;
+      float a0 = fmaf(cw.w1w[0][j], wx, Ps[j * kThreads]);
+      a0 = fmaf(cw.w1w[1][j], wy, a0); a0 = fmaxf(fmaf(cw.w1w[2][j], wz, a0), 0.f);
+      float a1 = fmaf(cw.w1w[0][j + 1], wx, Ps[(j + 1) * kThreads]);
+      a1 = fmaf(cw.w1w[1][j + 1], wy, a1); a1 = fmaxf(fmaf(cw.w1w[2][j + 1], wz, a1), 0.f);
+      p[k] = pack_rn(a0, a1);
+      q[k] = pack_lo(p[k], a0, a1);
+    }
+    tmem_st16(c.tA + 16 * h, p);
+    tmem_st16(c.tA + 32 + 16 * h, q);
   }
 }
 // ... or from registers (secondary point)
@@ -317,8 +363,7 @@ __device__ __forceinline__ void setup(const Smem& s, const uint8_t* __restrict__
   c.mbar = smem_u32(s.mbar); c.phase = 0;
 #pragma unroll
   for (int t = 0; t < kNumTiles; ++t) c.tile[t] = smem_u32(s.tiles + t * kTileBytes);
-  uint32_t one[8] = {0x3C003C00u, 0u, 0u, 0u, 0u, 0u, 0u, 0u};     // bias K-step of A: [1, 1, 0, ... 0]
-  tmem_st8(c.tOne, one);
+  restore_one(c);
   wait_st();
 }
 
@@ -370,9 +415,9 @@ __global__ void __launch_bounds__(kThreads, 3) k_render_tc(GridP g, EnvP env, Sh
     {
       float f[kD];
       encode_point<F16>(g, px, py, pz, f);
-      store_feat(c, f);
+      store_feat_split(c, f);
     }
-    mma_layer(c, 0, 2, true);                   // P = W1f f + b1
+    mma_layer(c, 0, 2, true, true);             // P = W1f f + b1 (split-precision f: P feeds the t that moves x')
     {
       float P[kH];
       load_D(c, P);
@@ -416,11 +461,12 @@ __global__ void __launch_bounds__(kThreads, 3) k_render_tc(GridP g, EnvP env, Sh
         const float* dp = dir_of(fr.s, i, j);
         const float wx = __ldg(dp), wy = __ldg(dp + 1), wz = __ldg(dp + 2);
         const float pdf = pdf_of(fr.s, i, j);
-        h1_from_smem(c, cw, Ps, wx, wy, wz);
-        mma_layer(c, 2, 4, false);
+        h1_from_smem_split(c, cw, Ps, wx, wy, wz);
+        mma_layer(c, 2, 4, false, true);
         float zv, zt, v, t;
         irt_epilogue(c, cw, zv, zt);
         irt_maps(sp, zv, zt, v, t);
+        restore_one(c);                         // the split A block overwrote the bias K-step columns
         // a7 + a8: secondary point, re-encode, B, I over the tertiary set
         float b2[7];
         float P2[kH];
@@ -483,9 +529,9 @@ __global__ void __launch_bounds__(kThreads, 3) k_trace_tc(GridP g, ShadeP sp, co
     {
       float f[kD];
       encode_point<F16>(g, px, py, pz, f);
-      store_feat(c, f);
+      store_feat_split(c, f);
     }
-    mma_layer(c, 0, 2, true);
+    mma_layer(c, 0, 2, true, true);
     float P[kH];
     load_D(c, P);
     for (uint32_t sidx = 0; sidx < ds.S; ++sidx) {
