@@ -35,6 +35,7 @@ struct __align__(16) TcConst {                // lives in the kernel-parameter c
   float w1w[3][kH];                           // I layer 1, direction columns
   float b2[kH]; float w3[2][kH]; float b3[2]; float pad0[2];
   float Bb2[kH]; float BW3[7][kH]; float Bb3[8];
+  uint32_t w3v_h2[kH / 2];                    // fp16x2 pairs of w3[0] (visibility row) for the fast epilogue
 };
 
 // ---------------------------------------------------------------------------------------------------- PTX wrappers
@@ -89,6 +90,10 @@ __device__ __forceinline__ void tmem_st8(uint32_t taddr, const uint32_t (&r)[8])
                : "memory");
 }
 
+__device__ __forceinline__ void tmem_st1(uint32_t taddr, uint32_t r) {
+  asm volatile("tcgen05.st.sync.aligned.32x32b.x1.b32 [%0], {%1};" ::"r"(taddr), "r"(r) : "memory");
+}
+
 // two floats -> packed fp16x2 (lo = a, hi = b), optionally with ReLU fused into the conversion
 __device__ __forceinline__ uint32_t pack_relu(float a, float b) {
   uint32_t r;
@@ -121,11 +126,12 @@ struct Ctx {
   uint32_t tile[kNumTiles];    // smem addresses of the weight tiles
 };
 
-// One 128 x 64 layer: D = A[:, 0:16*ksteps] * W^T (+ bias K-step from tile columns 32..47 when with_bias).
+// One 128 x 64 layer: D = A[:, 0:16*ksteps] * W^T (+ a bias K-step: A = [1,1,0..] times K-step `bias_kstep` of tile
+// `bias_tile`, whose first two columns hold the bias as an fp16 hi/lo pair; bias_tile < 0 = none).
 // split: A holds a hi block (columns 0..8*ksteps) and a lo block (the next 8*ksteps columns) of an error-compensated
 // fp16 pair; both are multiplied by the same (exact fp16) weights, so the layer input is good to ~2^-22.
 // Every thread must have issued its tcgen05.st of A before calling.  Returns when D is readable.
-__device__ __forceinline__ void mma_layer(Ctx& c, int tile, int ksteps, bool with_bias, bool split = false) {
+__device__ __forceinline__ void mma_layer(Ctx& c, int tile, int ksteps, int bias_tile, int bias_kstep, bool split = false) {
   wait_st();
   fence_before();
   __syncthreads();
@@ -135,7 +141,7 @@ __device__ __forceinline__ void mma_layer(Ctx& c, int tile, int ksteps, bool wit
     for (int k = 0; k < ksteps; ++k) mma_f16_ts(c.tD0, c.tA0 + 8 * k, bd + 2 * k, kIdesc, k > 0);
     if (split)
       for (int k = 0; k < ksteps; ++k) mma_f16_ts(c.tD0, c.tA0 + 8 * (ksteps + k), bd + 2 * k, kIdesc, 1u);
-    if (with_bias) mma_f16_ts(c.tD0, c.tOne0, bd + 2 * 2, kIdesc, 1u);
+    if (bias_tile >= 0) mma_f16_ts(c.tD0, c.tOne0, make_bdesc(c.tile[bias_tile]) + 2 * bias_kstep, kIdesc, 1u);
     mma_commit(c.mbar);
   }
   mbar_wait(c.mbar, c.phase);
@@ -144,29 +150,28 @@ __device__ __forceinline__ void mma_layer(Ctx& c, int tile, int ksteps, bool wit
 }
 
 // ---------------------------------------------------------------------------------------------------- per-row stages
-// f[32] -> A columns 0..15
-__device__ __forceinline__ void store_feat(const Ctx& c, const float (&f)[kD]) {
-  uint32_t r[16];
-#pragma unroll
-  for (int k = 0; k < 16; ++k) r[k] = pack_rn(f[2 * k], f[2 * k + 1]);
-  tmem_st16(c.tA, r);
-}
-
 // residual of an fp16x2 pack: (a - fp16(a), b - fp16(b)) packed again (the "lo" half of a hi/lo split)
 __device__ __forceinline__ uint32_t pack_lo(uint32_t hi, float a, float b) {
   const float2 h = __half22float2(*reinterpret_cast<const __half2*>(&hi));
   return pack_rn(a - h.x, b - h.y);
 }
 
-// f[32] -> A columns 0..15 (hi) and 16..31 (lo): split-precision features for the primary layer-1 partial P
-__device__ __forceinline__ void store_feat_split(const Ctx& c, const float (&f)[kD]) {
-  uint32_t r[32];
-#pragma unroll
-  for (int k = 0; k < 16; ++k) {
-    r[k] = pack_rn(f[2 * k], f[2 * k + 1]);
-    r[16 + k] = pack_lo(r[k], f[2 * k], f[2 * k + 1]);
+// f = H(x) straight into the A operand: level l -> TMEM column l (fp16 pair) and its fp16 residual into column
+// 16 + l (split-precision features for the layer-1 partial P, which feeds the t that moves x').  The level loop stays
+// rolled (x2) to keep the kernel inside the instruction cache; 16 gathers per thread are in flight.
+template <bool F16>
+__device__ __forceinline__ void encode_to_A(const GridP& g, const Ctx& c, float x, float y, float z) {
+#pragma unroll 2
+  for (int l = 0; l < kMaxL; ++l) {
+    uint32_t hi = 0u, lo = 0u;
+    if (l < (int)g.L) {
+      const float2 v = encode_level<F16>(g, l, x, y, z, nullptr, nullptr);
+      hi = pack_rn(v.x, v.y);
+      lo = pack_lo(hi, v.x, v.y);
+    }
+    tmem_st1(c.tA + l, hi);
+    tmem_st1(c.tA + 16 + l, lo);
   }
-  tmem_st32(c.tA, r);
 }
 
 __device__ __forceinline__ void restore_one(const Ctx& c) {
@@ -174,8 +179,8 @@ __device__ __forceinline__ void restore_one(const Ctx& c) {
   tmem_st8(c.tOne, one);
 }
 
-// epilogue of I: (z_v, z_t) = b3 + W3 relu(D + b2)
-__device__ __forceinline__ void irt_epilogue(const Ctx& c, const TcConst& cw, float& zv, float& zt) {
+// Precise epilogue of I (secondary set: z_t becomes t): (z_v, z_t) = b3 + W3 relu(D + b2), all fp32.
+__device__ __forceinline__ void irt_epilogue_precise(const Ctx& c, const TcConst& cw, float& zv, float& zt) {
   float z0 = cw.b3[0], z1 = cw.b3[1];
 #pragma unroll
   for (int h = 0; h < 2; ++h) {
@@ -192,26 +197,32 @@ __device__ __forceinline__ void irt_epilogue(const Ctx& c, const TcConst& cw, fl
   zv = z0; zt = z1;
 }
 
-// layers 2+3 of B with relu(hB1) already in A: -> brdf (post-activation)
-__device__ __forceinline__ void brdf_tail(Ctx& c, const TcConst& cw, const ShadeP& sp, float (&b)[7]) {
-  mma_layer(c, 3, 4, false);
-  float o[8];
+// Fast epilogue of I (direct and tertiary queries need only visibility): b2 already rode in the MMA (bias K-step),
+// h2 = relu(D) is rounded to fp16 by the packing conversion, z_v = b3 + w3v . h2 with fp16x2 FMAs into four short
+// accumulators summed in fp32.
+__device__ __forceinline__ float irt_epilogue_fast(const Ctx& c, const TcConst& cw) {
+  __half2 acc[4];
 #pragma unroll
-  for (int q = 0; q < 8; ++q) o[q] = cw.Bb3[q];
+  for (int q = 0; q < 4; ++q) acc[q] = __float2half2_rn(0.f);
 #pragma unroll
   for (int h = 0; h < 2; ++h) {
     uint32_t r[32];
     tmem_ld32(c.tD + 32 * h, r);
     wait_ld();
 #pragma unroll
-    for (int k = 0; k < 32; ++k) {
-      const float a = fmaxf(__uint_as_float(r[k]) + cw.Bb2[32 * h + k], 0.f);
-#pragma unroll
-      for (int q = 0; q < 7; ++q) o[q] = fmaf(a, cw.BW3[q][32 * h + k], o[q]);
+    for (int k = 0; k < 16; ++k) {
+      const uint32_t p = pack_relu(__uint_as_float(r[2 * k]), __uint_as_float(r[2 * k + 1]));
+      const uint32_t w = cw.w3v_h2[16 * h + k];
+      acc[k & 3] = __hfma2(*reinterpret_cast<const __half2*>(&p), *reinterpret_cast<const __half2*>(&w), acc[k & 3]);
     }
   }
-  brdf_maps(sp, o, b);
+  float z = cw.b3[0];
+#pragma unroll
+  for (int q = 0; q < 4; ++q) { const float2 f = __half22float2(acc[q]); z += f.x + f.y; }
+  return z;
 }
+
+__device__ __forceinline__ float vis_of(const ShadeP& sp, float zv) { return sp.vis_mode ? (zv > 0.f ? 1.f : 0.f) : sigmoidf_(zv); }
 
 // D (= W1 f + b1 of B) -> relu -> fp16 -> A columns 0..31
 __device__ __forceinline__ void hidden_to_A(const Ctx& c) {
@@ -227,24 +238,40 @@ __device__ __forceinline__ void hidden_to_A(const Ctx& c) {
   }
 }
 
-// full B(f) with f already in A[0..15]: layer 1 (bias in the MMA), relu, layers 2+3
+// B(f) with f already in A[0..15]: layer 1 and layer 2 biases ride in the MMAs, layer 3 in fp32 registers
 __device__ __forceinline__ void brdf_from_A(Ctx& c, const TcConst& cw, const ShadeP& sp, float (&b)[7]) {
-  mma_layer(c, 1, 2, true);
+  mma_layer(c, 1, 2, 1, 2);
   hidden_to_A(c);
-  brdf_tail(c, cw, sp, b);
+  mma_layer(c, 3, 4, 1, 3);
+  float o[8];
+#pragma unroll
+  for (int q = 0; q < 8; ++q) o[q] = cw.Bb3[q];
+#pragma unroll
+  for (int h = 0; h < 2; ++h) {
+    uint32_t r[32];
+    tmem_ld32(c.tD + 32 * h, r);
+    wait_ld();
+#pragma unroll
+    for (int k = 0; k < 32; ++k) {
+      const float a = fmaxf(__uint_as_float(r[k]), 0.f);
+#pragma unroll
+      for (int q = 0; q < 7; ++q) o[q] = fmaf(a, cw.BW3[q][32 * h + k], o[q]);
+    }
+  }
+  brdf_maps(sp, o, b);
 }
 
-// h1 = relu(P + W1w . w) -> A, P from a strided smem column (primary) ...
-__device__ __forceinline__ void h1_from_smem(const Ctx& c, const TcConst& cw, const float* Ps, float wx, float wy, float wz) {
+// h1 = relu(P + W1w . w) -> A columns 0..31 (P in registers)
+__device__ __forceinline__ void h1_from_regs(const Ctx& c, const TcConst& cw, const float (&P)[kH], float wx, float wy, float wz) {
 #pragma unroll
   for (int h = 0; h < 2; ++h) {
     uint32_t p[16];
 #pragma unroll
     for (int k = 0; k < 16; ++k) {
       const int j = 32 * h + 2 * k;
-      float a0 = fmaf(cw.w1w[0][j], wx, Ps[j * kThreads]);
+      float a0 = fmaf(cw.w1w[0][j], wx, P[j]);
       a0 = fmaf(cw.w1w[1][j], wy, a0); a0 = fmaf(cw.w1w[2][j], wz, a0);
-      float a1 = fmaf(cw.w1w[0][j + 1], wx, Ps[(j + 1) * kThreads]);
+      float a1 = fmaf(cw.w1w[0][j + 1], wx, P[j + 1]);
       a1 = fmaf(cw.w1w[1][j + 1], wy, a1); a1 = fmaf(cw.w1w[2][j + 1], wz, a1);
       p[k] = pack_relu(a0, a1);
     }
@@ -252,7 +279,7 @@ __device__ __forceinline__ void h1_from_smem(const Ctx& c, const TcConst& cw, co
   }
 }
 // split-precision variant for the secondary set (its z_t becomes t and moves x': SURVEY 8(c) conditioning note):
-// h1 in fp32 -> hi (columns 0..31) + lo (columns 32..63)
+// h1 in fp32 -> hi (columns 0..31) + lo (columns 32..63); P from this thread's shared-memory column
 __device__ __forceinline__ void h1_from_smem_split(const Ctx& c, const TcConst& cw, const float* Ps, float wx, float wy, float wz) {
 #pragma unroll
   for (int h = 0; h < 2; ++h) {
@@ -271,24 +298,7 @@ __device__ __forceinline__ void h1_from_smem_split(const Ctx& c, const TcConst& 
     tmem_st16(c.tA + 32 + 16 * h, q);
   }
 }
-// ... or from registers (secondary point)
-__device__ __forceinline__ void h1_from_regs(const Ctx& c, const TcConst& cw, const float (&P)[kH], float wx, float wy, float wz) {
-#pragma unroll
-  for (int h = 0; h < 2; ++h) {
-    uint32_t p[16];
-#pragma unroll
-    for (int k = 0; k < 16; ++k) {
-      const int j = 32 * h + 2 * k;
-      float a0 = fmaf(cw.w1w[0][j], wx, P[j]);
-      a0 = fmaf(cw.w1w[1][j], wy, a0); a0 = fmaf(cw.w1w[2][j], wz, a0);
-      float a1 = fmaf(cw.w1w[0][j + 1], wx, P[j + 1]);
-      a1 = fmaf(cw.w1w[1][j + 1], wy, a1); a1 = fmaf(cw.w1w[2][j + 1], wz, a1);
-      p[k] = pack_relu(a0, a1);
-    }
-    tmem_st16(c.tA + 16 * h, p);
-  }
-}
-// ... or with the direction part precomputed for a shared set: h1 = relu(P + Q)
+// shared direction set: the direction part Q = W1w . w'_k is precomputed per CTA, h1 = relu(P + Q)
 __device__ __forceinline__ void h1_from_regs_shared(const Ctx& c, const float (&P)[kH], const float* __restrict__ Q) {
 #pragma unroll
   for (int h = 0; h < 2; ++h) {
@@ -329,7 +339,7 @@ constexpr size_t kSmemBytes = 1024 + kNumTiles * kTileBytes + kH * kThreads * 4 
 
 __device__ __forceinline__ Smem carve(uint8_t* raw) {
   Smem s;
-  uint8_t* p = reinterpret_cast<uint8_t*>((reinterpret_cast<uintptr_t>(raw) + 1023) & ~uintptr_t(1023));
+  uint8_t* p = raw + ((1024u - (smem_u32(raw) & 1023u)) & 1023u);      // pointer arithmetic keeps the shared address space
   s.tiles = p; p += kNumTiles * kTileBytes;
   s.Ps = reinterpret_cast<float*>(p); p += kH * kThreads * 4;
   s.Qt = reinterpret_cast<float*>(p); p += kMaxS2 * kH * 4;
@@ -377,9 +387,10 @@ __device__ __forceinline__ void teardown(const Ctx& c) {
 }
 
 // ---------------------------------------------------------------------------------------------------- kernels
-// render_frame (a1-a11), tensor-core path.
+// render_frame (a1-a11), tensor-core path.  The point loop `j` runs -1 (the primary point itself) .. S_i-1 (its
+// secondary points) so that encode + layer-1 partial + BRDF decoder exist once in the instruction stream.
 template <bool F16>
-__global__ void __launch_bounds__(kThreads, 3) k_render_tc(GridP g, EnvP env, ShadeP sp, const __grid_constant__ TcConst cw,
+__global__ void __launch_bounds__(kThreads, 3) k_render_tc(const __grid_constant__ GridP g, EnvP env, ShadeP sp, const __grid_constant__ TcConst cw,
                                                            const uint8_t* __restrict__ wtiles, FrameP fr, float* __restrict__ rgb) {
   extern __shared__ uint8_t smem_raw[];
   const Smem s = carve(smem_raw);
@@ -404,6 +415,7 @@ __global__ void __launch_bounds__(kThreads, 3) k_render_tc(GridP g, EnvP env, Sh
   __syncthreads();
   float* Ps = s.Ps + threadIdx.x;
   const unsigned long long ntiles = (fr.N + kThreads - 1) / kThreads;
+  const int jend = indirect ? (int)fr.s.S : 0;
   for (unsigned long long tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
     const unsigned long long i_raw = tile * kThreads + threadIdx.x;
     const bool valid = i_raw < fr.N;
@@ -411,97 +423,88 @@ __global__ void __launch_bounds__(kThreads, 3) k_render_tc(GridP g, EnvP env, Sh
     const bool live = valid && !(fr.mask && !fr.mask[i]);
     const float px = __ldg(fr.x + 3 * i), py = __ldg(fr.x + 3 * i + 1), pz = __ldg(fr.x + 3 * i + 2);
     const float ox = __ldg(fr.wo + 3 * i), oy = __ldg(fr.wo + 3 * i + 1), oz = __ldg(fr.wo + 3 * i + 2);
-    float b[7];
-    {
-      float f[kD];
-      encode_point<F16>(g, px, py, pz, f);
-      store_feat_split(c, f);
-    }
-    mma_layer(c, 0, 2, true, true);             // P = W1f f + b1 (split-precision f: P feeds the t that moves x')
-    {
+    float b[7];                                                     // primary BRDF
+    float r = 0.f, gch = 0.f, bch = 0.f;                            // direct term of Eq. 1
+    float ir = 0.f, ig = 0.f, ib = 0.f;                             // (1 - V) L'_o term of Eq. 2
+    for (int j = -1; j < jend; ++j) {
+      float ex = px, ey = py, ez = pz, wx = 0.f, wy = 0.f, wz = 0.f, pdf = 0.f, v = 0.f;
+      if (j >= 0) {                                                 // a6/a7 along secondary direction j (split precision)
+        const float* dp = dir_of(fr.s, i, j);
+        wx = __ldg(dp); wy = __ldg(dp + 1); wz = __ldg(dp + 2);
+        pdf = pdf_of(fr.s, i, j);
+        h1_from_smem_split(c, cw, Ps, wx, wy, wz);
+        mma_layer(c, 2, 4, -1, 0, true);
+        float zv, zt, t;
+        irt_epilogue_precise(c, cw, zv, zt);
+        irt_maps(sp, zv, zt, v, t);
+        restore_one(c);                                             // the split A block overwrote the bias K-step columns
+        ex = sec_hit(px, t, wx); ey = sec_hit(py, t, wy); ez = sec_hit(pz, t, wz);
+      }
+      // a1-a5 at the point: f -> A, P = W1f f + b1, B(f)
+      encode_to_A<F16>(g, c, ex, ey, ez);
+      mma_layer(c, 0, 2, 0, 2, true);
       float P[kH];
       load_D(c, P);
+      float bb[7];
+      if (j < 0 && fr.brdf) {
 #pragma unroll
-      for (int k = 0; k < kH; ++k) Ps[k * kThreads] = P[k];
-    }
-    if (fr.brdf) {
-#pragma unroll
-      for (int k = 0; k < 7; ++k) b[k] = __ldg(fr.brdf + i * 7 + k);
-    } else {
-      brdf_from_A(c, cw, sp, b);                // A still holds f
-    }
-    float r = 0.f, gch = 0.f, bch = 0.f;
-    if ((fr.flags & 1u) && fr.d.S) {            // direct term of Eq. 1
-      float ar = 0.f, ag = 0.f, ab = 0.f;
-      const float* dp = dir_of(fr.d, i, 0);
-      float wx = __ldg(dp), wy = __ldg(dp + 1), wz = __ldg(dp + 2), pdf = pdf_of(fr.d, i, 0);
-      for (uint32_t sidx = 0; sidx < fr.d.S; ++sidx) {
-        const uint32_t sn = sidx + 1 < fr.d.S ? sidx + 1 : sidx;          // prefetch the next direction
-        const float* dn = dir_of(fr.d, i, sn);
-        const float nwx = __ldg(dn), nwy = __ldg(dn + 1), nwz = __ldg(dn + 2), npdf = pdf_of(fr.d, i, sn);
-        float v = 1.f;
-        if (fr.flags & 2u) {
-          h1_from_smem(c, cw, Ps, wx, wy, wz);
-          mma_layer(c, 2, 4, false);
-          float zv, zt, t;
-          irt_epilogue(c, cw, zv, zt);
-          irt_maps(sp, zv, zt, v, t);
-        }
-        const float3 gg = brdf_cos_over_pdf(sp, b, wx, wy, wz, ox, oy, oz, pdf);
-        const float3 L = incoming(env, fr.d, i, sidx, wx, wy, wz);
-        ar = fmaf(v * L.x, gg.x, ar); ag = fmaf(v * L.y, gg.y, ag); ab = fmaf(v * L.z, gg.z, ab);
-        wx = nwx; wy = nwy; wz = nwz; pdf = npdf;
+        for (int k = 0; k < 7; ++k) bb[k] = __ldg(fr.brdf + i * 7 + k);
+      } else {
+        brdf_from_A(c, cw, sp, bb);                                 // A[0..15] still holds f (hi)
       }
-      const float inv = 1.f / (float)fr.d.S;
-      r = ar * inv; gch = ag * inv; bch = ab * inv;
-    }
-    if (indirect) {                             // (1 - V) L'_o term of Eq. 2
-      float ar = 0.f, ag = 0.f, ab = 0.f;
-      for (uint32_t j = 0; j < fr.s.S; ++j) {
-        const float* dp = dir_of(fr.s, i, j);
-        const float wx = __ldg(dp), wy = __ldg(dp + 1), wz = __ldg(dp + 2);
-        const float pdf = pdf_of(fr.s, i, j);
-        h1_from_smem_split(c, cw, Ps, wx, wy, wz);
-        mma_layer(c, 2, 4, false, true);
-        float zv, zt, v, t;
-        irt_epilogue(c, cw, zv, zt);
-        irt_maps(sp, zv, zt, v, t);
-        restore_one(c);                         // the split A block overwrote the bias K-step columns
-        // a7 + a8: secondary point, re-encode, B, I over the tertiary set
-        float b2[7];
-        float P2[kH];
-        {
-          float f[kD];
-          encode_point<F16>(g, sec_hit(px, t, wx), sec_hit(py, t, wy), sec_hit(pz, t, wz), f);
-          store_feat(c, f);
+      if (j < 0) {
+#pragma unroll
+        for (int k = 0; k < 7; ++k) b[k] = bb[k];
+        if (jend > 0) {
+#pragma unroll
+          for (int k = 0; k < kH; ++k) Ps[k * kThreads] = P[k];
         }
-        mma_layer(c, 0, 2, true);
-        load_D(c, P2);
-        brdf_from_A(c, cw, sp, b2);
+        if ((fr.flags & 1u) && fr.d.S) {                            // direct term of Eq. 1 over the direct set
+          float ar = 0.f, ag = 0.f, ab = 0.f;
+          const float* dp = dir_of(fr.d, i, 0);
+          float dx = __ldg(dp), dy = __ldg(dp + 1), dz = __ldg(dp + 2), dpdf = pdf_of(fr.d, i, 0);
+          for (uint32_t sidx = 0; sidx < fr.d.S; ++sidx) {
+            const uint32_t sn = sidx + 1 < fr.d.S ? sidx + 1 : sidx;      // prefetch the next direction
+            const float* dn = dir_of(fr.d, i, sn);
+            const float nx = __ldg(dn), ny = __ldg(dn + 1), nz = __ldg(dn + 2), npdf = pdf_of(fr.d, i, sn);
+            float vd = 1.f;
+            if (fr.flags & 2u) {
+              h1_from_regs(c, cw, P, dx, dy, dz);
+              mma_layer(c, 2, 4, 0, 3);
+              vd = vis_of(sp, irt_epilogue_fast(c, cw));
+            }
+            const float3 gg = brdf_cos_over_pdf(sp, bb, dx, dy, dz, ox, oy, oz, dpdf);
+            const float3 L = incoming(env, fr.d, i, sidx, dx, dy, dz);
+            ar = fmaf(vd * L.x, gg.x, ar); ag = fmaf(vd * L.y, gg.y, ag); ab = fmaf(vd * L.z, gg.z, ab);
+            dx = nx; dy = ny; dz = nz; dpdf = npdf;
+          }
+          const float inv = 1.f / (float)fr.d.S;
+          r = ar * inv; gch = ag * inv; bch = ab * inv;
+        }
+      } else {                                                      // a8: Eq. 1 at x' over the tertiary set, w_o' = -w_j
         float lr = 0.f, lg = 0.f, lb = 0.f;
         const unsigned long long trow = tshared ? 0ull : i * fr.s.S + j;
         for (uint32_t k = 0; k < fr.t.S; ++k) {
           const float* tp = dir_of(fr.t, trow, k);
           const float tx = __ldg(tp), ty = __ldg(tp + 1), tz = __ldg(tp + 2);
-          if (tshared) h1_from_regs_shared(c, P2, s.Qt + k * kH);
-          else h1_from_regs(c, cw, P2, tx, ty, tz);
-          mma_layer(c, 2, 4, false);
-          float zv2, zt2, v2, t2;
-          irt_epilogue(c, cw, zv2, zt2);
-          irt_maps(sp, zv2, zt2, v2, t2);
-          const float3 gg = brdf_cos_over_pdf(sp, b2, tx, ty, tz, -wx, -wy, -wz, pdf_of(fr.t, trow, k));
+          if (tshared) h1_from_regs_shared(c, P, s.Qt + k * kH);
+          else h1_from_regs(c, cw, P, tx, ty, tz);
+          mma_layer(c, 2, 4, 0, 3);
+          const float v2 = vis_of(sp, irt_epilogue_fast(c, cw));
+          const float3 gg = brdf_cos_over_pdf(sp, bb, tx, ty, tz, -wx, -wy, -wz, pdf_of(fr.t, trow, k));
           float3 L;
           if (tshared) L = make_float3(s.Lt[4 * k], s.Lt[4 * k + 1], s.Lt[4 * k + 2]);
           else L = incoming(env, fr.t, trow, k, tx, ty, tz);
           lr = fmaf(v2 * L.x, gg.x, lr); lg = fmaf(v2 * L.y, gg.y, lg); lb = fmaf(v2 * L.z, gg.z, lb);
         }
-        const float invt = 1.f / (float)fr.t.S;
         const float3 gg = brdf_cos_over_pdf(sp, b, wx, wy, wz, ox, oy, oz, pdf);
-        const float m = (1.f - v) * invt;
-        ar = fmaf(m * lr, gg.x, ar); ag = fmaf(m * lg, gg.y, ag); ab = fmaf(m * lb, gg.z, ab);
+        const float m = (1.f - v) / (float)fr.t.S;
+        ir = fmaf(m * lr, gg.x, ir); ig = fmaf(m * lg, gg.y, ig); ib = fmaf(m * lb, gg.z, ib);
       }
-      const float inv = 1.f / (float)fr.s.S;
-      r = fmaf(ar, inv, r); gch = fmaf(ag, inv, gch); bch = fmaf(ab, inv, bch);
+    }
+    if (jend > 0) {
+      const float inv = 1.f / (float)jend;
+      r = fmaf(ir, inv, r); gch = fmaf(ig, inv, gch); bch = fmaf(ib, inv, bch);
     }
     if (valid) {
       rgb[3 * i] = live ? r : 0.f; rgb[3 * i + 1] = live ? gch : 0.f; rgb[3 * i + 2] = live ? bch : 0.f;
@@ -510,9 +513,9 @@ __global__ void __launch_bounds__(kThreads, 3) k_render_tc(GridP g, EnvP env, Sh
   teardown(c);
 }
 
-// trace with the encode fused (a1-a4, a6, a7), tensor-core path.
+// trace with the encode fused (a1-a4, a6, a7), tensor-core path (t is an output: precise epilogue).
 template <bool F16>
-__global__ void __launch_bounds__(kThreads, 3) k_trace_tc(GridP g, ShadeP sp, const __grid_constant__ TcConst cw,
+__global__ void __launch_bounds__(kThreads, 3) k_trace_tc(const __grid_constant__ GridP g, ShadeP sp, const __grid_constant__ TcConst cw,
                                                           const uint8_t* __restrict__ wtiles, const float* __restrict__ x,
                                                           unsigned long long N, DirsetP ds, float* __restrict__ vis,
                                                           float* __restrict__ zvo, float* __restrict__ to, float* __restrict__ xsec) {
@@ -526,21 +529,17 @@ __global__ void __launch_bounds__(kThreads, 3) k_trace_tc(GridP g, ShadeP sp, co
     const bool valid = i_raw < N;
     const unsigned long long i = valid ? i_raw : N - 1;
     const float px = __ldg(x + 3 * i), py = __ldg(x + 3 * i + 1), pz = __ldg(x + 3 * i + 2);
-    {
-      float f[kD];
-      encode_point<F16>(g, px, py, pz, f);
-      store_feat_split(c, f);
-    }
-    mma_layer(c, 0, 2, true, true);
+    encode_to_A<F16>(g, c, px, py, pz);
+    mma_layer(c, 0, 2, 0, 2, true);
     float P[kH];
     load_D(c, P);
     for (uint32_t sidx = 0; sidx < ds.S; ++sidx) {
       const float* dp = dir_of(ds, i, sidx);
       const float wx = __ldg(dp), wy = __ldg(dp + 1), wz = __ldg(dp + 2);
       h1_from_regs(c, cw, P, wx, wy, wz);
-      mma_layer(c, 2, 4, false);
+      mma_layer(c, 2, 4, -1, 0);
       float zv, zt, v, t;
-      irt_epilogue(c, cw, zv, zt);
+      irt_epilogue_precise(c, cw, zv, zt);
       irt_maps(sp, zv, zt, v, t);
       if (valid) {
         const unsigned long long o = i * ds.S + sidx;
@@ -567,10 +566,10 @@ inline void prepare_weights(const hr_config& cfg, const float* bw, const float* 
   auto put = [&](int t, int j, int k, float v) {
     *reinterpret_cast<__half*>(reinterpret_cast<uint8_t*>(tiles) + (size_t)t * kTileBytes + tile_off(j, k)) = __float2half_rn(v);
   };
-  auto put_bias = [&](int t, int j, float b) {            // hi + lo split in columns 32, 33 (bias K-step)
+  auto put_bias = [&](int t, int j, int col, float b) {   // hi + lo split in columns col, col+1 (one bias K-step)
     const __half hi = __float2half_rn(b);
-    put(t, j, 32, __half2float(hi));
-    put(t, j, 33, b - __half2float(hi));
+    put(t, j, col, __half2float(hi));
+    put(t, j, col + 1, b - __half2float(hi));
   };
   const float* BW1 = bw; const float* Bb1 = BW1 + H * D; const float* BW2 = Bb1 + H; const float* Bb2 = BW2 + H * H;
   const float* BW3 = Bb2 + H; const float* Bb3 = BW3 + 7 * H;
@@ -578,7 +577,8 @@ inline void prepare_weights(const hr_config& cfg, const float* bw, const float* 
   const float* IW3 = Ib2 + H; const float* Ib3 = IW3 + 2 * H;
   for (int j = 0; j < H; ++j) {
     for (int k = 0; k < D; ++k) { put(0, j, k, IW1[j * Din + k]); put(1, j, k, BW1[j * D + k]); }
-    put_bias(0, j, Ib1[j]); put_bias(1, j, Bb1[j]);
+    put_bias(0, j, 32, Ib1[j]); put_bias(1, j, 32, Bb1[j]);       // K-step 2: layer-1 biases
+    put_bias(0, j, 48, Ib2[j]); put_bias(1, j, 48, Bb2[j]);       // K-step 3: layer-2 biases (spare columns of the K=32 tiles)
     for (int k = 0; k < H; ++k) { put(2, j, k, IW2[j * H + k]); put(3, j, k, BW2[j * H + k]); }
     for (int d = 0; d < 3; ++d) cw.w1w[d][j] = IW1[j * Din + D + d];
     cw.b2[j] = Ib2[j]; cw.w3[0][j] = IW3[j]; cw.w3[1][j] = IW3[H + j];
@@ -586,6 +586,10 @@ inline void prepare_weights(const hr_config& cfg, const float* bw, const float* 
     for (int q = 0; q < 7; ++q) cw.BW3[q][j] = BW3[q * H + j];
   }
   cw.b3[0] = Ib3[0]; cw.b3[1] = Ib3[1];
+  for (int k = 0; k < H / 2; ++k) {
+    const __half2 w = __floats2half2_rn(IW3[2 * k], IW3[2 * k + 1]);
+    cw.w3v_h2[k] = *reinterpret_cast<const uint32_t*>(&w);
+  }
   for (int q = 0; q < 8; ++q) cw.Bb3[q] = q < 7 ? Bb3[q] : 0.f;
 }
 
