@@ -7,7 +7,9 @@
 // the A operand is read from TMEM), weights sit in shared memory as K-major SWIZZLE_128B UMMA tiles, the fp32
 // accumulator comes back with tcgen05.ld and the bias/ReLU/last-layer dot products run from constant-bank
 // operands.  Layer-1 biases ride in the MMA as an extra K step (hi + lo fp16 split => exact to 2^-22).
-// Several CTAs per SM overlap one tile's MMA round trip with the others' ALU work.
+// The query loops are software-pipelined two deep over two (A, D) TMEM buffer pairs, and the gathers of the next
+// secondary point are spread over the tertiary loop of the current one, so a thread's gathers, packing, MMA and
+// epilogue overlap; two CTAs per SM cover the remaining serial phases.
 //
 // Precision contract (Q34): tables/weights fp16 (rounded once by the caller's generator), hidden activations
 // rounded to fp16 (RNE), accumulation fp32, final-layer outputs / t / x' / the index path / shading fp32.
@@ -24,12 +26,18 @@ namespace hr {
 namespace tc {
 
 constexpr int kThreads = 128;
-constexpr int kTmemCols = 128;
+constexpr int kTmemCols = 256;                // per CTA; two CTAs per SM own the whole TMEM
 constexpr int kTileBytes = 64 * 128;          // one 64 x 64 fp16 K-major SW128 weight tile
-constexpr int kNumTiles = 4;                  // I.W1f(+b1), B.W1(+b1), I.W2, B.W2
+constexpr int kNumTiles = 4;                  // I.W1f(+b1,b2), B.W1(+b1,b2), I.W2, B.W2  (64 x 64 each)
+constexpr int kTile3Bytes = 16 * 128;         // B.W3 zero-padded to 16 x 64 (N = 16 MMA)
+constexpr int kAllTileBytes = kNumTiles * kTileBytes + kTile3Bytes;
+constexpr int kCtasPerSm = 2;
 constexpr int kMaxS2 = 16;                    // shared tertiary set staged in smem
-// TMEM column map (per CTA): A operand (fp16 pairs) | constant bias K-step | accumulator
-constexpr uint32_t kColA = 0, kColOne = 56, kColD = 64;   // a split-precision 64-wide A (cols 0..63) overwrites the bias step
+// TMEM column map (per CTA).  Two (A, D) buffer pairs let one query's MMA run under the next query's packing and
+// the previous query's epilogue.  A buffer b: columns 64 b .. 64 b + 31 (fp16 pairs); the split-precision layers use
+// A0 columns 0..63 (hi | lo).  Columns 32..47 stage the NEXT secondary point's features while the tertiary loop of
+// the current one runs.  Columns 96..103 hold the constant bias K-step [1, 1, 0 .. 0].  D buffer b: 128 + 64 b.
+constexpr uint32_t kColA = 0, kColNext = 32, kColOne = 96, kColD = 128, kBufStride = 64;
 
 struct __align__(16) TcConst {                // lives in the kernel-parameter constant bank
   float w1w[3][kH];                           // I layer 1, direction columns
@@ -73,6 +81,10 @@ __device__ __forceinline__ void tmem_ld32(uint32_t taddr, uint32_t (&r)[32]) {
       "tcgen05.ld.sync.aligned.32x32b.x32.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16,%17,%18,%19,%20,%21,%22,%23,%24,%25,"
       "%26,%27,%28,%29,%30,%31}, [%32];"
       : HR_R16(r, 0), HR_R16(r, 16) : "r"(taddr) : "memory");
+}
+__device__ __forceinline__ void tmem_ld8(uint32_t taddr, uint32_t (&r)[8]) {
+  asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+               : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]) : "r"(taddr) : "memory");
 }
 __device__ __forceinline__ void tmem_st16(uint32_t taddr, const uint32_t (&r)[16]) {
   asm volatile("tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16};" ::"r"(taddr), HR_W16(r, 0)
@@ -118,49 +130,59 @@ __device__ __forceinline__ uint64_t make_bdesc(uint32_t smem_addr) {
 }
 // kind::f16, A/B = F16 K-major, D = F32, M = 128, N = 64
 constexpr uint32_t kIdesc = (1u << 4) | ((64u >> 3) << 17) | ((128u >> 4) << 24);
+constexpr uint32_t kIdescN16 = (1u << 4) | ((16u >> 3) << 17) | ((128u >> 4) << 24);
+
 
 struct Ctx {
-  uint32_t tA, tOne, tD;       // TMEM addresses incl. this warp's lane base
-  uint32_t tA0, tOne0, tD0;    // lane-0 addresses (MMA operands)
-  uint32_t mbar, phase;
-  uint32_t tile[kNumTiles];    // smem addresses of the weight tiles
+  uint32_t lane;               // this warp's TMEM lane base (bits 31..16)
+  uint32_t base;               // TMEM base of the CTA's allocation (lane 0, column 0)
+  uint32_t mbar;               // smem address of mbarrier 0 (mbarrier 1 at +8)
+  uint32_t phase;              // bit b = parity to wait for on mbarrier b
+  uint32_t tile0;              // smem address of weight tile 0 (tile t at + t * kTileBytes)
 };
+__device__ __forceinline__ uint32_t colA(const Ctx& c, int buf) { return c.base + c.lane + kColA + kBufStride * buf; }
+__device__ __forceinline__ uint32_t colD(const Ctx& c, int buf) { return c.base + c.lane + kColD + kBufStride * buf; }
+__device__ __forceinline__ uint32_t colNext(const Ctx& c) { return c.base + c.lane + kColNext; }
 
-// One 128 x 64 layer: D = A[:, 0:16*ksteps] * W^T (+ a bias K-step: A = [1,1,0..] times K-step `bias_kstep` of tile
-// `bias_tile`, whose first two columns hold the bias as an fp16 hi/lo pair; bias_tile < 0 = none).
-// split: A holds a hi block (columns 0..8*ksteps) and a lo block (the next 8*ksteps columns) of an error-compensated
-// fp16 pair; both are multiplied by the same (exact fp16) weights, so the layer input is good to ~2^-22.
-// Every thread must have issued its tcgen05.st of A before calling.  Returns when D is readable.
-__device__ __forceinline__ void mma_layer(Ctx& c, int tile, int ksteps, int bias_tile, int bias_kstep, bool split = false) {
+// Issue one 128 x N layer on buffer pair `buf`: D[buf] = A * W^T where A starts `a_off` columns into the CTA's TMEM
+// (lane 0 address), `ksteps` K-steps of 16; optional split lo block right after the hi block; optional bias K-step
+// (A = [1,1,0..] times K-step `bias_kstep` of tile `bias_tile`).  Every thread must have issued its tcgen05.st of A.
+// Does NOT wait for the MMA: wait_layer(c, buf) does.
+__device__ __forceinline__ void issue_layer(Ctx& c, int buf, uint32_t a_off, int tile, int ksteps, int bias_tile, int bias_kstep,
+                                            bool split = false, uint32_t idesc = kIdesc) {
   wait_st();
   fence_before();
   __syncthreads();
   if (threadIdx.x == 0) {
     fence_after();
-    const uint64_t bd = make_bdesc(c.tile[tile]);
-    for (int k = 0; k < ksteps; ++k) mma_f16_ts(c.tD0, c.tA0 + 8 * k, bd + 2 * k, kIdesc, k > 0);
+    const uint32_t d = c.base + kColD + kBufStride * buf;
+    const uint32_t a = c.base + a_off;
+    const uint64_t bd = make_bdesc(c.tile0 + tile * kTileBytes);
+    for (int k = 0; k < ksteps; ++k) mma_f16_ts(d, a + 8 * k, bd + 2 * k, idesc, k > 0);
     if (split)
-      for (int k = 0; k < ksteps; ++k) mma_f16_ts(c.tD0, c.tA0 + 8 * (ksteps + k), bd + 2 * k, kIdesc, 1u);
-    if (bias_tile >= 0) mma_f16_ts(c.tD0, c.tOne0, make_bdesc(c.tile[bias_tile]) + 2 * bias_kstep, kIdesc, 1u);
-    mma_commit(c.mbar);
+      for (int k = 0; k < ksteps; ++k) mma_f16_ts(d, a + 8 * (ksteps + k), bd + 2 * k, idesc, 1u);
+    if (bias_tile >= 0) mma_f16_ts(d, c.base + kColOne, make_bdesc(c.tile0 + bias_tile * kTileBytes) + 2 * bias_kstep, idesc, 1u);
+    mma_commit(c.mbar + 8 * buf);
   }
-  mbar_wait(c.mbar, c.phase);
-  c.phase ^= 1u;
+}
+__device__ __forceinline__ void wait_layer(Ctx& c, int buf) {
+  mbar_wait(c.mbar + 8 * buf, (c.phase >> buf) & 1u);
+  c.phase ^= 1u << buf;
   fence_after();
 }
 
-// ---------------------------------------------------------------------------------------------------- per-row stages
+// ---------------------------------------------------------------------------------------------------- encode pieces
 // residual of an fp16x2 pack: (a - fp16(a), b - fp16(b)) packed again (the "lo" half of a hi/lo split)
 __device__ __forceinline__ uint32_t pack_lo(uint32_t hi, float a, float b) {
   const float2 h = __half22float2(*reinterpret_cast<const __half2*>(&hi));
   return pack_rn(a - h.x, b - h.y);
 }
 
-// f = H(x) straight into the A operand: level l -> TMEM column l (fp16 pair) and its fp16 residual into column
-// 16 + l (split-precision features for the layer-1 partial P, which feeds the t that moves x').  The level loop stays
-// rolled (x2) to keep the kernel inside the instruction cache; 16 gathers per thread are in flight.
+// Primary point: f = H(x) in fp32, level l -> A0 column l (fp16 pair) and its fp16 residual -> column 16 + l
+// (split-precision features for the layer-1 partial P, which feeds the t that moves x').
 template <bool F16>
-__device__ __forceinline__ void encode_to_A(const GridP& g, const Ctx& c, float x, float y, float z) {
+__device__ __forceinline__ void encode_split_to_A(const GridP& g, const Ctx& c, float x, float y, float z) {
+  const uint32_t tA = colA(c, 0);
 #pragma unroll 2
   for (int l = 0; l < kMaxL; ++l) {
     uint32_t hi = 0u, lo = 0u;
@@ -169,45 +191,109 @@ __device__ __forceinline__ void encode_to_A(const GridP& g, const Ctx& c, float 
       hi = pack_rn(v.x, v.y);
       lo = pack_lo(hi, v.x, v.y);
     }
-    tmem_st1(c.tA + l, hi);
-    tmem_st1(c.tA + 16 + l, lo);
+    tmem_st1(tA + l, hi);
+    tmem_st1(tA + 16 + l, lo);
   }
 }
 
-__device__ __forceinline__ void restore_one(const Ctx& c) {
-  uint32_t one[8] = {0x3C003C00u, 0u, 0u, 0u, 0u, 0u, 0u, 0u};     // bias K-step of A: [1, 1, 0, ... 0]
-  tmem_st8(c.tOne, one);
+// Secondary points: the gathers of one level (issued early) and their interpolation (consumed late) are separate so
+// the caller can put a whole tertiary query between them.  fp16 tables: the 8 half2 rows are interpolated with fp16x2
+// lerps (x, y, z: 7 sub + 7 fma) and the result IS the packed A-operand word.  The cell / index path is fp32 + integer,
+// identical to encode_level.
+template <bool F16> struct LevelTaps;
+template <> struct LevelTaps<true> { __half2 v[8]; __half2 w[3]; };
+template <> struct LevelTaps<false> { float2 v[8]; float w[3]; };
+
+template <bool F16>
+__device__ __forceinline__ void gather_level(const GridP& g, int l, float x, float y, float z, LevelTaps<F16>& t) {
+  const uint32_t N = g.res[l];
+  const Cell cl = cell_of(N, x, y, z);
+  uint32_t idx[8];
+  corner_indices(cl, N, (g.dense_mask >> l) & 1u, g.log2_T, idx);
+  if constexpr (F16) {
+    const __half2* tb = reinterpret_cast<const __half2*>(g.tables) + ((size_t)l << g.log2_T);
+#pragma unroll
+    for (int k = 0; k < 8; ++k) t.v[k] = __ldg(tb + idx[k]);
+#pragma unroll
+    for (int d = 0; d < 3; ++d) t.w[d] = __float2half2_rn(cl.w[d]);
+  } else {
+    const float2* tb = reinterpret_cast<const float2*>(g.tables) + ((size_t)l << g.log2_T);
+#pragma unroll
+    for (int k = 0; k < 8; ++k) t.v[k] = __ldg(tb + idx[k]);
+#pragma unroll
+    for (int d = 0; d < 3; ++d) t.w[d] = cl.w[d];
+  }
+}
+__device__ __forceinline__ uint32_t lerp_level(const LevelTaps<true>& t) {
+  __half2 a[4];
+#pragma unroll
+  for (int k = 0; k < 4; ++k) a[k] = __hfma2(t.w[0], __hsub2(t.v[2 * k + 1], t.v[2 * k]), t.v[2 * k]);
+  const __half2 b0 = __hfma2(t.w[1], __hsub2(a[1], a[0]), a[0]);
+  const __half2 b1 = __hfma2(t.w[1], __hsub2(a[3], a[2]), a[2]);
+  const __half2 r = __hfma2(t.w[2], __hsub2(b1, b0), b0);
+  return *reinterpret_cast<const uint32_t*>(&r);
+}
+__device__ __forceinline__ uint32_t lerp_level(const LevelTaps<false>& t) {
+  float2 a[4];
+#pragma unroll
+  for (int k = 0; k < 4; ++k) {
+    a[k].x = fmaf(t.w[0], t.v[2 * k + 1].x - t.v[2 * k].x, t.v[2 * k].x);
+    a[k].y = fmaf(t.w[0], t.v[2 * k + 1].y - t.v[2 * k].y, t.v[2 * k].y);
+  }
+  const float b0x = fmaf(t.w[1], a[1].x - a[0].x, a[0].x), b0y = fmaf(t.w[1], a[1].y - a[0].y, a[0].y);
+  const float b1x = fmaf(t.w[1], a[3].x - a[2].x, a[2].x), b1y = fmaf(t.w[1], a[3].y - a[2].y, a[2].y);
+  return pack_rn(fmaf(t.w[2], b1x - b0x, b0x), fmaf(t.w[2], b1y - b0y, b0y));
 }
 
+// whole fast encode of one secondary point into the staging columns (used for the first secondary point of a pixel
+// and whenever the tertiary loop cannot carry the gathers)
+template <bool F16>
+__device__ __forceinline__ void encode_next_plain(const GridP& g, const Ctx& c, float x, float y, float z) {
+  const uint32_t tN = colNext(c);
+#pragma unroll 1
+  for (int l0 = 0; l0 < kMaxL; l0 += 2) {
+    LevelTaps<F16> t0, t1;
+    const bool on0 = l0 < (int)g.L, on1 = l0 + 1 < (int)g.L;
+    if (on0) gather_level<F16>(g, l0, x, y, z, t0);
+    if (on1) gather_level<F16>(g, l0 + 1, x, y, z, t1);
+    tmem_st1(tN + l0, on0 ? lerp_level(t0) : 0u);
+    tmem_st1(tN + l0 + 1, on1 ? lerp_level(t1) : 0u);
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------- per-row stages
 // Precise epilogue of I (secondary set: z_t becomes t): (z_v, z_t) = b3 + W3 relu(D + b2), all fp32.
-__device__ __forceinline__ void irt_epilogue_precise(const Ctx& c, const TcConst& cw, float& zv, float& zt) {
-  float z0 = cw.b3[0], z1 = cw.b3[1];
+__device__ __forceinline__ void irt_epilogue_precise(const Ctx& c, const TcConst& cw, int buf, float& zv, float& zt) {
+  float z0[4] = {cw.b3[0], 0.f, 0.f, 0.f}, z1[4] = {cw.b3[1], 0.f, 0.f, 0.f};
+  const uint32_t tD = colD(c, buf);
 #pragma unroll
   for (int h = 0; h < 2; ++h) {
     uint32_t r[32];
-    tmem_ld32(c.tD + 32 * h, r);
+    tmem_ld32(tD + 32 * h, r);
     wait_ld();
 #pragma unroll
     for (int k = 0; k < 32; ++k) {
       const float a = fmaxf(__uint_as_float(r[k]) + cw.b2[32 * h + k], 0.f);
-      z0 = fmaf(a, cw.w3[0][32 * h + k], z0);
-      z1 = fmaf(a, cw.w3[1][32 * h + k], z1);
+      z0[k & 3] = fmaf(a, cw.w3[0][32 * h + k], z0[k & 3]);
+      z1[k & 3] = fmaf(a, cw.w3[1][32 * h + k], z1[k & 3]);
     }
   }
-  zv = z0; zt = z1;
+  zv = (z0[0] + z0[1]) + (z0[2] + z0[3]);
+  zt = (z1[0] + z1[1]) + (z1[2] + z1[3]);
 }
 
 // Fast epilogue of I (direct and tertiary queries need only visibility): b2 already rode in the MMA (bias K-step),
 // h2 = relu(D) is rounded to fp16 by the packing conversion, z_v = b3 + w3v . h2 with fp16x2 FMAs into four short
 // accumulators summed in fp32.
-__device__ __forceinline__ float irt_epilogue_fast(const Ctx& c, const TcConst& cw) {
+__device__ __forceinline__ float irt_epilogue_fast(const Ctx& c, const TcConst& cw, int buf) {
   __half2 acc[4];
 #pragma unroll
   for (int q = 0; q < 4; ++q) acc[q] = __float2half2_rn(0.f);
+  const uint32_t tD = colD(c, buf);
 #pragma unroll
   for (int h = 0; h < 2; ++h) {
     uint32_t r[32];
-    tmem_ld32(c.tD + 32 * h, r);
+    tmem_ld32(tD + 32 * h, r);
     wait_ld();
 #pragma unroll
     for (int k = 0; k < 16; ++k) {
@@ -224,45 +310,44 @@ __device__ __forceinline__ float irt_epilogue_fast(const Ctx& c, const TcConst& 
 
 __device__ __forceinline__ float vis_of(const ShadeP& sp, float zv) { return sp.vis_mode ? (zv > 0.f ? 1.f : 0.f) : sigmoidf_(zv); }
 
-// D (= W1 f + b1 of B) -> relu -> fp16 -> A columns 0..31
+// D0 -> relu -> fp16 -> A0 columns 0..31
 __device__ __forceinline__ void hidden_to_A(const Ctx& c) {
+  const uint32_t tD = colD(c, 0), tA = colA(c, 0);
 #pragma unroll
   for (int h = 0; h < 2; ++h) {
     uint32_t r[32];
-    tmem_ld32(c.tD + 32 * h, r);
+    tmem_ld32(tD + 32 * h, r);
     wait_ld();
     uint32_t p[16];
 #pragma unroll
     for (int k = 0; k < 16; ++k) p[k] = pack_relu(__uint_as_float(r[2 * k]), __uint_as_float(r[2 * k + 1]));
-    tmem_st16(c.tA + 16 * h, p);
+    tmem_st16(tA + 16 * h, p);
   }
 }
 
-// B(f) with f already in A[0..15]: layer 1 and layer 2 biases ride in the MMAs, layer 3 in fp32 registers
-__device__ __forceinline__ void brdf_from_A(Ctx& c, const TcConst& cw, const ShadeP& sp, float (&b)[7]) {
-  mma_layer(c, 1, 2, 1, 2);
+// B(f) with the fp16 features at column offset f_off: all three layers on the tensor core (layer-1/2 biases ride in
+// the MMAs, layer 3 is an N = 16 MMA over the zero-padded 7-row W3; b3 is added in registers).  Buffer pair 0.
+__device__ __forceinline__ void brdf_from_A(Ctx& c, const TcConst& cw, const ShadeP& sp, uint32_t f_off, float (&b)[7]) {
+  issue_layer(c, 0, f_off, 1, 2, 1, 2);
+  wait_layer(c, 0);
   hidden_to_A(c);
-  mma_layer(c, 3, 4, 1, 3);
+  issue_layer(c, 0, kColA, 3, 4, 1, 3);
+  wait_layer(c, 0);
+  hidden_to_A(c);
+  issue_layer(c, 0, kColA, 4, 4, -1, 0, false, kIdescN16);
+  wait_layer(c, 0);
+  uint32_t r[8];
+  tmem_ld8(colD(c, 0), r);
+  wait_ld();
   float o[8];
 #pragma unroll
-  for (int q = 0; q < 8; ++q) o[q] = cw.Bb3[q];
-#pragma unroll
-  for (int h = 0; h < 2; ++h) {
-    uint32_t r[32];
-    tmem_ld32(c.tD + 32 * h, r);
-    wait_ld();
-#pragma unroll
-    for (int k = 0; k < 32; ++k) {
-      const float a = fmaxf(__uint_as_float(r[k]), 0.f);
-#pragma unroll
-      for (int q = 0; q < 7; ++q) o[q] = fmaf(a, cw.BW3[q][32 * h + k], o[q]);
-    }
-  }
+  for (int q = 0; q < 8; ++q) o[q] = __uint_as_float(r[q]) + cw.Bb3[q];
   brdf_maps(sp, o, b);
 }
 
-// h1 = relu(P + W1w . w) -> A columns 0..31 (P in registers)
-__device__ __forceinline__ void h1_from_regs(const Ctx& c, const TcConst& cw, const float (&P)[kH], float wx, float wy, float wz) {
+// h1 = relu(P + W1w . w) -> A[buf] columns 0..31 (P in registers)
+__device__ __forceinline__ void h1_from_regs(const Ctx& c, const TcConst& cw, int buf, const float (&P)[kH], float wx, float wy, float wz) {
+  const uint32_t tA = colA(c, buf);
 #pragma unroll
   for (int h = 0; h < 2; ++h) {
     uint32_t p[16];
@@ -275,12 +360,13 @@ __device__ __forceinline__ void h1_from_regs(const Ctx& c, const TcConst& cw, co
       a1 = fmaf(cw.w1w[1][j + 1], wy, a1); a1 = fmaf(cw.w1w[2][j + 1], wz, a1);
       p[k] = pack_relu(a0, a1);
     }
-    tmem_st16(c.tA + 16 * h, p);
+    tmem_st16(tA + 16 * h, p);
   }
 }
 // split-precision variant for the secondary set (its z_t becomes t and moves x': SURVEY 8(c) conditioning note):
-// h1 in fp32 -> hi (columns 0..31) + lo (columns 32..63); P from this thread's shared-memory column
+// h1 in fp32 -> hi (A0 columns 0..31) + lo (columns 32..63); P from this thread's shared-memory column
 __device__ __forceinline__ void h1_from_smem_split(const Ctx& c, const TcConst& cw, const float* Ps, float wx, float wy, float wz) {
+  const uint32_t tA = colA(c, 0);
 #pragma unroll
   for (int h = 0; h < 2; ++h) {
     uint32_t p[16], q[16];
@@ -294,12 +380,13 @@ __device__ __forceinline__ void h1_from_smem_split(const Ctx& c, const TcConst& 
       p[k] = pack_rn(a0, a1);
       q[k] = pack_lo(p[k], a0, a1);
     }
-    tmem_st16(c.tA + 16 * h, p);
-    tmem_st16(c.tA + 32 + 16 * h, q);
+    tmem_st16(tA + 16 * h, p);
+    tmem_st16(tA + 32 + 16 * h, q);
   }
 }
 // shared direction set: the direction part Q = W1w . w'_k is precomputed per CTA, h1 = relu(P + Q)
-__device__ __forceinline__ void h1_from_regs_shared(const Ctx& c, const float (&P)[kH], const float* __restrict__ Q) {
+__device__ __forceinline__ void h1_from_regs_shared(const Ctx& c, int buf, const float (&P)[kH], const float* __restrict__ Q) {
+  const uint32_t tA = colA(c, buf);
 #pragma unroll
   for (int h = 0; h < 2; ++h) {
     uint32_t p[16];
@@ -310,16 +397,17 @@ __device__ __forceinline__ void h1_from_regs_shared(const Ctx& c, const float (&
       p[2 * k] = pack_relu(P[j] + q.x, P[j + 1] + q.y);
       p[2 * k + 1] = pack_relu(P[j + 2] + q.z, P[j + 3] + q.w);
     }
-    tmem_st16(c.tA + 16 * h, p);
+    tmem_st16(tA + 16 * h, p);
   }
 }
 
-// D -> registers (64 fp32)
+// D0 -> registers (64 fp32)
 __device__ __forceinline__ void load_D(const Ctx& c, float (&P)[kH]) {
+  const uint32_t tD = colD(c, 0);
 #pragma unroll
   for (int h = 0; h < 2; ++h) {
     uint32_t r[32];
-    tmem_ld32(c.tD + 32 * h, r);
+    tmem_ld32(tD + 32 * h, r);
     wait_ld();
 #pragma unroll
     for (int k = 0; k < 32; ++k) P[32 * h + k] = __uint_as_float(r[k]);
@@ -328,22 +416,22 @@ __device__ __forceinline__ void load_D(const Ctx& c, float (&P)[kH]) {
 
 // ---------------------------------------------------------------------------------------------------- shared setup
 struct Smem {
-  uint8_t* tiles;      // 4 x 8 KB, 1024-aligned
+  uint8_t* tiles;      // 4 x 8 KB + 2 KB, 1024-aligned
   float* Ps;           // [64][128]
   float* Qt;           // [kMaxS2][64]
-  float* Lt;           // [kMaxS2][4]
-  uint64_t* mbar;
+  float* Lt;           // [kMaxS2][8]: radiance rgb, pdf, direction xyz, pad
+  uint64_t* mbar;      // [2]
   uint32_t* tmem_slot;
 };
-constexpr size_t kSmemBytes = 1024 + kNumTiles * kTileBytes + kH * kThreads * 4 + kMaxS2 * kH * 4 + kMaxS2 * 4 * 4 + 64;
+constexpr size_t kSmemBytes = 1024 + kAllTileBytes + kH * kThreads * 4 + kMaxS2 * kH * 4 + kMaxS2 * 8 * 4 + 64;
 
 __device__ __forceinline__ Smem carve(uint8_t* raw) {
   Smem s;
   uint8_t* p = raw + ((1024u - (smem_u32(raw) & 1023u)) & 1023u);      // pointer arithmetic keeps the shared address space
-  s.tiles = p; p += kNumTiles * kTileBytes;
+  s.tiles = p; p += kAllTileBytes;
   s.Ps = reinterpret_cast<float*>(p); p += kH * kThreads * 4;
   s.Qt = reinterpret_cast<float*>(p); p += kMaxS2 * kH * 4;
-  s.Lt = reinterpret_cast<float*>(p); p += kMaxS2 * 4 * 4;
+  s.Lt = reinterpret_cast<float*>(p); p += kMaxS2 * 8 * 4;
   s.mbar = reinterpret_cast<uint64_t*>(p); p += 16;
   s.tmem_slot = reinterpret_cast<uint32_t*>(p);
   return s;
@@ -357,23 +445,22 @@ __device__ __forceinline__ void setup(const Smem& s, const uint8_t* __restrict__
   }
   if (threadIdx.x == 0) {
     asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(smem_u32(s.mbar)) : "memory");
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(smem_u32(s.mbar + 1)) : "memory");
     asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
   }
   const uint4* src = reinterpret_cast<const uint4*>(wtiles);
   uint4* dst = reinterpret_cast<uint4*>(s.tiles);
-  for (int i = threadIdx.x; i < kNumTiles * kTileBytes / 16; i += kThreads) dst[i] = __ldg(src + i);
+  for (int i = threadIdx.x; i < kAllTileBytes / 16; i += kThreads) dst[i] = __ldg(src + i);
   asm volatile("fence.proxy.async.shared::cta;" ::: "memory");     // generic-proxy writes -> visible to the tensor core
   fence_before();
   __syncthreads();
   fence_after();
-  const uint32_t base = *s.tmem_slot;
-  const uint32_t lane_base = (uint32_t)(warp * 32) << 16;
-  c.tA0 = base + kColA; c.tOne0 = base + kColOne; c.tD0 = base + kColD;
-  c.tA = c.tA0 + lane_base; c.tOne = c.tOne0 + lane_base; c.tD = c.tD0 + lane_base;
+  c.base = *s.tmem_slot;
+  c.lane = (uint32_t)(warp * 32) << 16;
   c.mbar = smem_u32(s.mbar); c.phase = 0;
-#pragma unroll
-  for (int t = 0; t < kNumTiles; ++t) c.tile[t] = smem_u32(s.tiles + t * kTileBytes);
-  restore_one(c);
+  c.tile0 = smem_u32(s.tiles);
+  uint32_t one[8] = {0x3C003C00u, 0u, 0u, 0u, 0u, 0u, 0u, 0u};     // bias K-step of A: [1, 1, 0, ... 0]
+  tmem_st8(c.base + c.lane + kColOne, one);
   wait_st();
 }
 
@@ -382,23 +469,25 @@ __device__ __forceinline__ void teardown(const Ctx& c) {
   __syncthreads();
   if ((threadIdx.x >> 5) == 0) {
     fence_after();
-    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(c.tA0), "r"((uint32_t)kTmemCols) : "memory");
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(c.base), "r"((uint32_t)kTmemCols) : "memory");
   }
 }
 
 // ---------------------------------------------------------------------------------------------------- kernels
-// render_frame (a1-a11), tensor-core path.  The point loop `j` runs -1 (the primary point itself) .. S_i-1 (its
-// secondary points) so that encode + layer-1 partial + BRDF decoder exist once in the instruction stream.
+struct SecRay { float v, wx, wy, wz, pdf, x, y, z; };   // one secondary direction of a pixel: visibility, direction, pdf, hit x'
+
+// render_frame (a1-a11), tensor-core path.
 template <bool F16>
-__global__ void __launch_bounds__(kThreads, 3) k_render_tc(const __grid_constant__ GridP g, EnvP env, ShadeP sp, const __grid_constant__ TcConst cw,
-                                                           const uint8_t* __restrict__ wtiles, FrameP fr, float* __restrict__ rgb) {
+__global__ void __launch_bounds__(kThreads, kCtasPerSm) k_render_tc(const __grid_constant__ GridP g, EnvP env, ShadeP sp,
+                                                                    const __grid_constant__ TcConst cw, const uint8_t* __restrict__ wtiles,
+                                                                    FrameP fr, float* __restrict__ rgb) {
   extern __shared__ uint8_t smem_raw[];
   const Smem s = carve(smem_raw);
   Ctx c;
   setup(s, wtiles, c);
   const bool indirect = (fr.flags & 4u) && fr.s.S && fr.t.S;
   const bool tshared = fr.t.stride == 0;
-  if (indirect && tshared) {                    // shared tertiary set: Q_k = W1w . w'_k, L_k = env(w'_k)
+  if (indirect && tshared) {                    // shared tertiary set: Q_k = W1w . w'_k; per k: radiance, pdf, direction
     for (int e = threadIdx.x; e < (int)fr.t.S * kH; e += kThreads) {
       const int k = e / kH, q = e % kH;
       const float* dp = fr.t.dir + 3 * k;
@@ -406,16 +495,21 @@ __global__ void __launch_bounds__(kThreads, 3) k_render_tc(const __grid_constant
     }
     for (int k = threadIdx.x; k < (int)fr.t.S; k += kThreads) {
       const float* dp = fr.t.dir + 3 * k;
+      const float tx = __ldg(dp), ty = __ldg(dp + 1), tz = __ldg(dp + 2);
       float3 L;
       if (fr.t.Lin) L = make_float3(__ldg(fr.t.Lin + 3 * k), __ldg(fr.t.Lin + 3 * k + 1), __ldg(fr.t.Lin + 3 * k + 2));
-      else L = env_lookup(env, __ldg(dp), __ldg(dp + 1), __ldg(dp + 2));
-      s.Lt[4 * k] = L.x; s.Lt[4 * k + 1] = L.y; s.Lt[4 * k + 2] = L.z;
+      else L = env_lookup(env, tx, ty, tz);
+      float* o = s.Lt + 8 * k;
+      o[0] = L.x; o[1] = L.y; o[2] = L.z; o[3] = __ldg(fr.t.pdf + k); o[4] = tx; o[5] = ty; o[6] = tz; o[7] = 0.f;
     }
   }
   __syncthreads();
   float* Ps = s.Ps + threadIdx.x;
   const unsigned long long ntiles = (fr.N + kThreads - 1) / kThreads;
   const int jend = indirect ? (int)fr.s.S : 0;
+  // levels of the NEXT secondary point gathered per tertiary iteration (0 = the tertiary loop cannot carry them)
+  const int lpi = (indirect && fr.t.S >= 4 && fr.t.S <= 16 && (16 % fr.t.S) == 0) ? 16 / (int)fr.t.S : 0;
+
   for (unsigned long long tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
     const unsigned long long i_raw = tile * kThreads + threadIdx.x;
     const bool valid = i_raw < fr.N;
@@ -425,84 +519,138 @@ __global__ void __launch_bounds__(kThreads, 3) k_render_tc(const __grid_constant
     const float ox = __ldg(fr.wo + 3 * i), oy = __ldg(fr.wo + 3 * i + 1), oz = __ldg(fr.wo + 3 * i + 2);
     float b[7];                                                     // primary BRDF
     float r = 0.f, gch = 0.f, bch = 0.f;                            // direct term of Eq. 1
-    float ir = 0.f, ig = 0.f, ib = 0.f;                             // (1 - V) L'_o term of Eq. 2
-    for (int j = -1; j < jend; ++j) {
-      float ex = px, ey = py, ez = pz, wx = 0.f, wy = 0.f, wz = 0.f, pdf = 0.f, v = 0.f;
-      if (j >= 0) {                                                 // a6/a7 along secondary direction j (split precision)
-        const float* dp = dir_of(fr.s, i, j);
-        wx = __ldg(dp); wy = __ldg(dp + 1); wz = __ldg(dp + 2);
-        pdf = pdf_of(fr.s, i, j);
-        h1_from_smem_split(c, cw, Ps, wx, wy, wz);
-        mma_layer(c, 2, 4, -1, 0, true);
-        float zv, zt, t;
-        irt_epilogue_precise(c, cw, zv, zt);
-        irt_maps(sp, zv, zt, v, t);
-        restore_one(c);                                             // the split A block overwrote the bias K-step columns
-        ex = sec_hit(px, t, wx); ey = sec_hit(py, t, wy); ez = sec_hit(pz, t, wz);
-      }
-      // a1-a5 at the point: f -> A, P = W1f f + b1, B(f)
-      encode_to_A<F16>(g, c, ex, ey, ez);
-      mma_layer(c, 0, 2, 0, 2, true);
+
+    // ---- primary point: a1-a5, then the direct set -------------------------------------------------------------
+    {
+      encode_split_to_A<F16>(g, c, px, py, pz);
+      issue_layer(c, 0, kColA, 0, 2, 0, 2, true);                   // P = W1f f + b1, split-precision f
+      wait_layer(c, 0);
       float P[kH];
       load_D(c, P);
-      float bb[7];
-      if (j < 0 && fr.brdf) {
+      if (fr.brdf) {
 #pragma unroll
-        for (int k = 0; k < 7; ++k) bb[k] = __ldg(fr.brdf + i * 7 + k);
+        for (int k = 0; k < 7; ++k) b[k] = __ldg(fr.brdf + i * 7 + k);
       } else {
-        brdf_from_A(c, cw, sp, bb);                                 // A[0..15] still holds f (hi)
+        brdf_from_A(c, cw, sp, kColA, b);                           // A0[0..15] still holds f (hi)
       }
-      if (j < 0) {
+      if (jend > 0) {
 #pragma unroll
-        for (int k = 0; k < 7; ++k) b[k] = bb[k];
-        if (jend > 0) {
-#pragma unroll
-          for (int k = 0; k < kH; ++k) Ps[k * kThreads] = P[k];
-        }
-        if ((fr.flags & 1u) && fr.d.S) {                            // direct term of Eq. 1 over the direct set
-          float ar = 0.f, ag = 0.f, ab = 0.f;
-          const float* dp = dir_of(fr.d, i, 0);
-          float dx = __ldg(dp), dy = __ldg(dp + 1), dz = __ldg(dp + 2), dpdf = pdf_of(fr.d, i, 0);
-          for (uint32_t sidx = 0; sidx < fr.d.S; ++sidx) {
-            const uint32_t sn = sidx + 1 < fr.d.S ? sidx + 1 : sidx;      // prefetch the next direction
-            const float* dn = dir_of(fr.d, i, sn);
-            const float nx = __ldg(dn), ny = __ldg(dn + 1), nz = __ldg(dn + 2), npdf = pdf_of(fr.d, i, sn);
-            float vd = 1.f;
-            if (fr.flags & 2u) {
-              h1_from_regs(c, cw, P, dx, dy, dz);
-              mma_layer(c, 2, 4, 0, 3);
-              vd = vis_of(sp, irt_epilogue_fast(c, cw));
-            }
-            const float3 gg = brdf_cos_over_pdf(sp, bb, dx, dy, dz, ox, oy, oz, dpdf);
-            const float3 L = incoming(env, fr.d, i, sidx, dx, dy, dz);
-            ar = fmaf(vd * L.x, gg.x, ar); ag = fmaf(vd * L.y, gg.y, ag); ab = fmaf(vd * L.z, gg.z, ab);
-            dx = nx; dy = ny; dz = nz; dpdf = npdf;
+        for (int k = 0; k < kH; ++k) Ps[k * kThreads] = P[k];
+      }
+      if ((fr.flags & 1u) && fr.d.S) {                              // direct term of Eq. 1, two queries in flight
+        const uint32_t S = fr.d.S;
+        const bool shadow = fr.flags & 2u;
+        float ar = 0.f, ag = 0.f, ab = 0.f;
+        const float* dp = dir_of(fr.d, i, 0);
+        float d0x = __ldg(dp), d0y = __ldg(dp + 1), d0z = __ldg(dp + 2), d0p = pdf_of(fr.d, i, 0);
+        const uint32_t s1 = S > 1 ? 1u : 0u;
+        dp = dir_of(fr.d, i, s1);
+        float d1x = __ldg(dp), d1y = __ldg(dp + 1), d1z = __ldg(dp + 2), d1p = pdf_of(fr.d, i, s1);
+        if (shadow) { h1_from_regs(c, cw, 0, P, d0x, d0y, d0z); issue_layer(c, 0, kColA, 2, 4, 0, 3); }
+        for (uint32_t k = 0; k < S; ++k) {
+          const int bf = k & 1;
+          const uint32_t s2 = k + 2 < S ? k + 2 : S - 1;            // prefetch direction k + 2
+          dp = dir_of(fr.d, i, s2);
+          const float d2x = __ldg(dp), d2y = __ldg(dp + 1), d2z = __ldg(dp + 2), d2p = pdf_of(fr.d, i, s2);
+          float vd = 1.f;
+          if (shadow) {
+            if (k + 1 < S) { h1_from_regs(c, cw, bf ^ 1, P, d1x, d1y, d1z); issue_layer(c, bf ^ 1, kColA + kBufStride * (bf ^ 1), 2, 4, 0, 3); }
+            wait_layer(c, bf);
+            vd = vis_of(sp, irt_epilogue_fast(c, cw, bf));
           }
-          const float inv = 1.f / (float)fr.d.S;
-          r = ar * inv; gch = ag * inv; bch = ab * inv;
+          const float3 gg = brdf_cos_over_pdf(sp, b, d0x, d0y, d0z, ox, oy, oz, d0p);
+          const float3 L = incoming(env, fr.d, i, k, d0x, d0y, d0z);
+          ar = fmaf(vd * L.x, gg.x, ar); ag = fmaf(vd * L.y, gg.y, ag); ab = fmaf(vd * L.z, gg.z, ab);
+          d0x = d1x; d0y = d1y; d0z = d1z; d0p = d1p;
+          d1x = d2x; d1y = d2y; d1z = d2z; d1p = d2p;
         }
-      } else {                                                      // a8: Eq. 1 at x' over the tertiary set, w_o' = -w_j
-        float lr = 0.f, lg = 0.f, lb = 0.f;
-        const unsigned long long trow = tshared ? 0ull : i * fr.s.S + j;
-        for (uint32_t k = 0; k < fr.t.S; ++k) {
-          const float* tp = dir_of(fr.t, trow, k);
-          const float tx = __ldg(tp), ty = __ldg(tp + 1), tz = __ldg(tp + 2);
-          if (tshared) h1_from_regs_shared(c, P, s.Qt + k * kH);
-          else h1_from_regs(c, cw, P, tx, ty, tz);
-          mma_layer(c, 2, 4, 0, 3);
-          const float v2 = vis_of(sp, irt_epilogue_fast(c, cw));
-          const float3 gg = brdf_cos_over_pdf(sp, bb, tx, ty, tz, -wx, -wy, -wz, pdf_of(fr.t, trow, k));
-          float3 L;
-          if (tshared) L = make_float3(s.Lt[4 * k], s.Lt[4 * k + 1], s.Lt[4 * k + 2]);
-          else L = incoming(env, fr.t, trow, k, tx, ty, tz);
-          lr = fmaf(v2 * L.x, gg.x, lr); lg = fmaf(v2 * L.y, gg.y, lg); lb = fmaf(v2 * L.z, gg.z, lb);
-        }
-        const float3 gg = brdf_cos_over_pdf(sp, b, wx, wy, wz, ox, oy, oz, pdf);
-        const float m = (1.f - v) / (float)fr.t.S;
-        ir = fmaf(m * lr, gg.x, ir); ig = fmaf(m * lg, gg.y, ig); ib = fmaf(m * lb, gg.z, ib);
+        const float inv = 1.f / (float)S;
+        r = ar * inv; gch = ag * inv; bch = ab * inv;
       }
     }
+
+    // ---- secondary set: (1 - V) L'_o term of Eq. 2 ---------------------------------------------------------------
     if (jend > 0) {
+      float ir = 0.f, ig = 0.f, ib = 0.f;
+      // a6/a7 along secondary direction j, split precision (buffer pair 0)
+      auto trace_secondary = [&](int j) -> SecRay {
+        SecRay q;
+        const float* dp = dir_of(fr.s, i, j);
+        q.wx = __ldg(dp); q.wy = __ldg(dp + 1); q.wz = __ldg(dp + 2);
+        q.pdf = pdf_of(fr.s, i, j);
+        h1_from_smem_split(c, cw, Ps, q.wx, q.wy, q.wz);
+        issue_layer(c, 0, kColA, 2, 4, -1, 0, true);
+        wait_layer(c, 0);
+        float zv, zt, t;
+        irt_epilogue_precise(c, cw, 0, zv, zt);
+        irt_maps(sp, zv, zt, q.v, t);
+        q.x = sec_hit(px, t, q.wx); q.y = sec_hit(py, t, q.wy); q.z = sec_hit(pz, t, q.wz);
+        return q;
+      };
+      SecRay nxt = trace_secondary(0);
+      encode_next_plain<F16>(g, c, nxt.x, nxt.y, nxt.z);
+      for (int j = 0; j < jend; ++j) {
+        const SecRay cur = nxt;
+        // a1-a5 at x'_j: its features wait in the staging columns
+        issue_layer(c, 0, kColNext, 0, 2, 0, 2);
+        wait_layer(c, 0);
+        float P2[kH];
+        load_D(c, P2);
+        float bb[7];
+        brdf_from_A(c, cw, sp, kColNext, bb);
+        const bool have_next = j + 1 < jend;
+        if (have_next) nxt = trace_secondary(j + 1);                // overwrites the staging columns: they are consumed
+        // a8: Eq. 1 at x'_j over the tertiary set (w_o' = -w_j), two queries in flight; each iteration also carries
+        // `lpi` levels of the gathers of x'_{j+1}
+        const uint32_t S2 = fr.t.S;
+        const unsigned long long trow = tshared ? 0ull : i * fr.s.S + j;
+        float lr = 0.f, lg = 0.f, lb = 0.f;
+        auto h1t = [&](uint32_t k, int bf) {
+          if (tshared) h1_from_regs_shared(c, bf, P2, s.Qt + k * kH);
+          else { const float* tp = dir_of(fr.t, trow, k); h1_from_regs(c, cw, bf, P2, __ldg(tp), __ldg(tp + 1), __ldg(tp + 2)); }
+        };
+        h1t(0, 0);
+        issue_layer(c, 0, kColA, 2, 4, 0, 3);
+        const uint32_t tN = colNext(c);
+        for (uint32_t k = 0; k < S2; ++k) {
+          const int bf = k & 1;
+          LevelTaps<F16> taps[4];
+          const bool carry = have_next && lpi > 0;
+          if (carry) {
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+              const int l = (int)k * lpi + q;
+              if (q < lpi && l < (int)g.L) gather_level<F16>(g, l, nxt.x, nxt.y, nxt.z, taps[q]);
+            }
+          }
+          if (k + 1 < S2) { h1t(k + 1, bf ^ 1); issue_layer(c, bf ^ 1, kColA + kBufStride * (bf ^ 1), 2, 4, 0, 3); }
+          wait_layer(c, bf);
+          const float v2 = vis_of(sp, irt_epilogue_fast(c, cw, bf));
+          float tx, ty, tz, tpdf;
+          float3 L;
+          if (tshared) {
+            const float4 a = reinterpret_cast<const float4*>(s.Lt)[2 * k], d = reinterpret_cast<const float4*>(s.Lt)[2 * k + 1];
+            L = make_float3(a.x, a.y, a.z); tpdf = a.w; tx = d.x; ty = d.y; tz = d.z;
+          } else {
+            const float* tp = dir_of(fr.t, trow, k);
+            tx = __ldg(tp); ty = __ldg(tp + 1); tz = __ldg(tp + 2); tpdf = pdf_of(fr.t, trow, k);
+            L = incoming(env, fr.t, trow, k, tx, ty, tz);
+          }
+          const float3 gg = brdf_cos_over_pdf(sp, bb, tx, ty, tz, -cur.wx, -cur.wy, -cur.wz, tpdf);
+          lr = fmaf(v2 * L.x, gg.x, lr); lg = fmaf(v2 * L.y, gg.y, lg); lb = fmaf(v2 * L.z, gg.z, lb);
+          if (carry) {
+#pragma unroll
+            for (int q = 0; q < 4; ++q) {
+              const int l = (int)k * lpi + q;
+              if (q < lpi) tmem_st1(tN + l, l < (int)g.L ? lerp_level(taps[q]) : 0u);
+            }
+          }
+        }
+        if (have_next && lpi == 0) encode_next_plain<F16>(g, c, nxt.x, nxt.y, nxt.z);
+        const float3 gg = brdf_cos_over_pdf(sp, b, cur.wx, cur.wy, cur.wz, ox, oy, oz, cur.pdf);
+        const float m = (1.f - cur.v) / (float)S2;
+        ir = fmaf(m * lr, gg.x, ir); ig = fmaf(m * lg, gg.y, ig); ib = fmaf(m * lb, gg.z, ib);
+      }
       const float inv = 1.f / (float)jend;
       r = fmaf(ir, inv, r); gch = fmaf(ig, inv, gch); bch = fmaf(ib, inv, bch);
     }
@@ -515,10 +663,10 @@ __global__ void __launch_bounds__(kThreads, 3) k_render_tc(const __grid_constant
 
 // trace with the encode fused (a1-a4, a6, a7), tensor-core path (t is an output: precise epilogue).
 template <bool F16>
-__global__ void __launch_bounds__(kThreads, 3) k_trace_tc(const __grid_constant__ GridP g, ShadeP sp, const __grid_constant__ TcConst cw,
-                                                          const uint8_t* __restrict__ wtiles, const float* __restrict__ x,
-                                                          unsigned long long N, DirsetP ds, float* __restrict__ vis,
-                                                          float* __restrict__ zvo, float* __restrict__ to, float* __restrict__ xsec) {
+__global__ void __launch_bounds__(kThreads, kCtasPerSm) k_trace_tc(const __grid_constant__ GridP g, ShadeP sp, const __grid_constant__ TcConst cw,
+                                                                   const uint8_t* __restrict__ wtiles, const float* __restrict__ x,
+                                                                   unsigned long long N, DirsetP ds, float* __restrict__ vis,
+                                                                   float* __restrict__ zvo, float* __restrict__ to, float* __restrict__ xsec) {
   extern __shared__ uint8_t smem_raw[];
   const Smem s = carve(smem_raw);
   Ctx c;
@@ -529,17 +677,19 @@ __global__ void __launch_bounds__(kThreads, 3) k_trace_tc(const __grid_constant_
     const bool valid = i_raw < N;
     const unsigned long long i = valid ? i_raw : N - 1;
     const float px = __ldg(x + 3 * i), py = __ldg(x + 3 * i + 1), pz = __ldg(x + 3 * i + 2);
-    encode_to_A<F16>(g, c, px, py, pz);
-    mma_layer(c, 0, 2, 0, 2, true);
+    encode_split_to_A<F16>(g, c, px, py, pz);
+    issue_layer(c, 0, kColA, 0, 2, 0, 2, true);
+    wait_layer(c, 0);
     float P[kH];
     load_D(c, P);
     for (uint32_t sidx = 0; sidx < ds.S; ++sidx) {
       const float* dp = dir_of(ds, i, sidx);
       const float wx = __ldg(dp), wy = __ldg(dp + 1), wz = __ldg(dp + 2);
-      h1_from_regs(c, cw, P, wx, wy, wz);
-      mma_layer(c, 2, 4, -1, 0);
+      h1_from_regs(c, cw, 0, P, wx, wy, wz);
+      issue_layer(c, 0, kColA, 2, 4, -1, 0);
+      wait_layer(c, 0);
       float zv, zt, v, t;
-      irt_epilogue_precise(c, cw, zv, zt);
+      irt_epilogue_precise(c, cw, 0, zv, zt);
       irt_maps(sp, zv, zt, v, t);
       if (valid) {
         const unsigned long long o = i * ds.S + sidx;
@@ -560,7 +710,7 @@ inline size_t tile_off(int j, int k) { return (size_t)(j / 8) * 1024 + (j % 8) *
 // Blob = [ TcConst | 4 UMMA tiles ].  The TcConst part is passed by value at launch, the tiles stay in HBM/L2.
 inline void prepare_weights(const hr_config& cfg, const float* bw, const float* iw, std::vector<uint8_t>& out) {
   const int D = cfg.L * cfg.F, H = kH, Din = D + 3;
-  out.assign(sizeof(TcConst) + kNumTiles * kTileBytes, 0);
+  out.assign(sizeof(TcConst) + kAllTileBytes, 0);
   TcConst& cw = *reinterpret_cast<TcConst*>(out.data());
   __half* tiles = reinterpret_cast<__half*>(out.data() + sizeof(TcConst));
   auto put = [&](int t, int j, int k, float v) {
@@ -583,7 +733,7 @@ inline void prepare_weights(const hr_config& cfg, const float* bw, const float* 
     for (int d = 0; d < 3; ++d) cw.w1w[d][j] = IW1[j * Din + D + d];
     cw.b2[j] = Ib2[j]; cw.w3[0][j] = IW3[j]; cw.w3[1][j] = IW3[H + j];
     cw.Bb2[j] = Bb2[j];
-    for (int q = 0; q < 7; ++q) cw.BW3[q][j] = BW3[q * H + j];
+    for (int q = 0; q < 7; ++q) { cw.BW3[q][j] = BW3[q * H + j]; put(4, q, j, BW3[q * H + j]); }
   }
   cw.b3[0] = Ib3[0]; cw.b3[1] = Ib3[1];
   for (int k = 0; k < H / 2; ++k) {
@@ -606,7 +756,7 @@ inline bool frame_supported(const FrameP& fr) { return !(fr.flags & 4u) || fr.t.
 
 inline int grid_size(unsigned long long N, int num_sms) {
   const unsigned long long tiles = (N + kThreads - 1) / kThreads;
-  const unsigned long long cap = (unsigned long long)num_sms * 3;
+  const unsigned long long cap = (unsigned long long)num_sms * kCtasPerSm;
   return (int)(tiles < cap ? tiles : cap);
 }
 
