@@ -131,6 +131,50 @@ def run_reference(args, cfg):
     }))
 
 
+def run_c4_sweep(args):
+    """BASELINE.json configs[4]: encode + IRT throughput (hashrender_trace, encode fused, 1 direction / point) over
+    N = 2^20..2^26 uniform random points x T = 2^16, 2^19, 2^22, 2^24 (fp16, F=2, L=16): where the gather leaves L2."""
+    import torch
+    from paper_2409_10327_b200 import DirSet, HashRenderer
+    dev = torch.device("cuda", 0)
+    peaks = load_peaks()
+    rows = []
+    Ns = [1 << 20, 1 << 22, 1 << 24] + ([1 << 26] if args.full_sweep else [])
+    for log2_T in (16, 19, 22, 24):
+        cfg = gen.make_config("C4", log2_T=log2_T, N=max(Ns))
+        model = gen.make_model(cfg)
+        r = HashRenderer.from_gen(cfg, model, vis_mode=args.vis_mode, max_points=max(Ns))
+        del model
+        g = torch.Generator(device=dev); g.manual_seed(4)
+        x = torch.rand((max(Ns), 3), device=dev, generator=g)
+        d = torch.randn((max(Ns), 1, 3), device=dev, generator=g); d = (d / d.norm(dim=2, keepdim=True)).contiguous()
+        pdf = torch.ones((max(Ns), 1), device=dev)
+        vis = torch.empty((max(Ns), 1), device=dev); t = torch.empty((max(Ns), 1), device=dev)
+        for N in Ns:
+            ds = DirSet(d[:N], pdf[:N])
+            for _ in range(3):
+                r.trace(x[:N], None, ds, vis, None, t, N=N)
+            torch.cuda.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            for _ in range(args.steps):
+                r.trace(x[:N], None, ds, vis, None, t, N=N)
+            e1.record(); torch.cuda.synchronize()
+            ms = e0.elapsed_time(e1) / args.steps
+            useful = N * 16 * 8 * 4            # bytes actually used: 8 corners x 16 levels x one fp16 pair
+            rows.append({"log2_T": log2_T, "table_MiB": 16 * (1 << log2_T) * 4 / 2 ** 20, "N": N, "ms": ms, "points_per_s": N / (ms * 1e-3),
+                         "useful_gather_GBps": useful / (ms * 1e-3) / 1e9, "sector_GBps_upper": useful * 8 / (ms * 1e-3) / 1e9,
+                         "path": r.last_path()})
+        r.destroy(); del x, d, pdf, vis, t
+        torch.cuda.empty_cache()
+    best = max(rows, key=lambda q: q["points_per_s"])
+    print(json.dumps({"metric": "encode+IRT points/s (BASELINE.json configs[4] sweep)", "value": best["points_per_s"], "unit": "points/s", "n_gpus": 1,
+                      "steps": args.steps, "warmup": 3, "ms_per_step": best["ms"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+                      "dtype": "f16", "data": "synthetic", "config": {"workload": "C4 sweep: uniform random points x 1 direction, fp16 L=16 F=2",
+                      "points": "generated on device (torch Philox); parity of this path is covered by tests at C0/C1/C3 shapes"},
+                      "hbm_peak_GBps": peaks["hbm"], "sweep": rows}))
+
+
 def workload_name(cfg):
     ind = f" + {cfg.S_i} secondary x {cfg.S_2} tertiary (one-bounce indirect)" if cfg.flags & gen.HR_INDIRECT else ""
     return (f"{cfg.name}: 800x800 = {cfg.N} primary points, {cfg.S_d} direct directions{ind}; L={cfg.L} F={cfg.F} T=2^{cfg.log2_T} "
@@ -142,7 +186,8 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--workload", default="C2", choices=["C1", "C2", "C3", "C3a"])
+    ap.add_argument("--workload", default="C2", choices=["C1", "C2", "C3", "C3a", "C4"])
+    ap.add_argument("--full-sweep", action="store_true", help="C4: include 2^26 points")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--vis-mode", type=int, default=1, help="1 = hard visibility (paper-faithful), 0 = soft")
     ap.add_argument("--e2e-steps", type=int, default=3)
@@ -154,7 +199,9 @@ def main():
     args.warmup = max(args.warmup, 0)
     cfg = gen.make_config(args.workload)
     if args.impl == "reference":
-        return run_reference(args, cfg)
+        return run_reference(args, gen.make_config("C2") if args.workload == "C4" else cfg)
+    if args.workload == "C4":
+        return run_c4_sweep(args)
 
     import torch
     import torch.distributed as dist
@@ -168,6 +215,7 @@ def main():
     dev = torch.device("cuda", local)
 
     from paper_2409_10327_b200 import DirSet, HashRenderer
+    from paper_2409_10327_b200 import dist as hd
 
     def measure(cfg, steps, warmup, e2e_steps, clocks):
         model = gen.make_model(cfg)
@@ -204,10 +252,7 @@ def main():
         launches = r.launch_count() - l0
         total_ms = ev[0].elapsed_time(ev[-1])
         per = [ev[k].elapsed_time(ev[k + 1]) for k in range(steps)]
-        tt = torch.tensor([total_ms], device=dev)
-        if world > 1:
-            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-        total_ms = float(tt.item())
+        total_ms = hd.max_over_ranks(total_ms, dev)
         assert torch.isfinite(rgb).all()
         out = dict(total_ms=total_ms, per=per, launches=launches, clk=clk, path=r.last_path(), mean_rgb=float(rgb.mean().item()))
         # end to end through the public host-buffer entry point: pinned host inputs, H2D + D2H inside the timed region
@@ -229,10 +274,7 @@ def main():
                 upb, downb = r.render_frame_host(hframe, hrgb, stream)
             e1.record()
             torch.cuda.synchronize()
-            te = torch.tensor([e0.elapsed_time(e1)], device=dev)
-            if world > 1:
-                dist.all_reduce(te, op=dist.ReduceOp.MAX)
-            out.update(e2e_ms=float(te.item()) / e2e_steps, h2d=upb, d2h=downb,
+            out.update(e2e_ms=hd.max_over_ranks(e0.elapsed_time(e1), dev) / e2e_steps, h2d=upb, d2h=downb,
                        e2e_matches=bool(np.allclose(hrgb, rgb.cpu().numpy(), rtol=1e-6, atol=1e-7)))
         r.destroy()
         del x, wo, d, s, t, rgb

@@ -58,6 +58,20 @@ __device__ __forceinline__ Cell cell_of(uint32_t N, float x, float y, float z) {
   return c;
 }
 
+// same for a position already clamped to [0,1]^3 (x' = sec_hit(...) is)
+__device__ __forceinline__ Cell cell_of_clamped(uint32_t N, float x, float y, float z) {
+  Cell c;
+  const float fn = (float)N;
+  const float p[3] = {__fmul_rn(x, fn), __fmul_rn(y, fn), __fmul_rn(z, fn)};
+#pragma unroll
+  for (int d = 0; d < 3; ++d) {
+    int fl = min(__float2int_rd(p[d]), (int)N - 1);
+    c.c0[d] = (uint32_t)fl;
+    c.w[d] = __fsub_rn(p[d], (float)fl);
+  }
+  return c;
+}
+
 __device__ __forceinline__ void corner_indices(const Cell& c, uint32_t N, bool dense, uint32_t log2_T, uint32_t (&idx)[8]) {
   if (dense) {                                                // (N+1)^3 <= T (Q3)
     const uint32_t s = N + 1, s2 = s * s;
@@ -67,10 +81,11 @@ __device__ __forceinline__ void corner_indices(const Cell& c, uint32_t N, bool d
   } else {                                                    // hash of [14], primes (1, 2654435761, 805459861) (Q1)
     const uint32_t mask = (1u << log2_T) - 1u;
     const uint32_t hx[2] = {c.c0[0], c.c0[0] + 1u};
-    const uint32_t hy[2] = {c.c0[1] * 2654435761u, (c.c0[1] + 1u) * 2654435761u};
-    const uint32_t hz[2] = {c.c0[2] * 805459861u, (c.c0[2] + 1u) * 805459861u};
+    const uint32_t hy0 = c.c0[1] * 2654435761u, hy1 = hy0 + 2654435761u;
+    const uint32_t hz0 = c.c0[2] * 805459861u, hz1 = hz0 + 805459861u;
+    const uint32_t hyz[4] = {hy0 ^ hz0, hy1 ^ hz0, hy0 ^ hz1, hy1 ^ hz1};
 #pragma unroll
-    for (int k = 0; k < 8; ++k) idx[k] = (hx[k & 1] ^ hy[(k >> 1) & 1] ^ hz[(k >> 2) & 1]) & mask;
+    for (int k = 0; k < 8; ++k) idx[k] = (hx[k & 1] ^ hyz[k >> 1]) & mask;
   }
 }
 
@@ -174,6 +189,8 @@ __device__ __forceinline__ float3 env_lookup(const EnvP& e, float wx, float wy, 
 }
 
 // ---- a10: f_r (n.w_i)^+ / p per channel (Q21-Q23) ---------------------------
+__device__ __forceinline__ float sqrt_approx(float x) { float r; asm("sqrt.approx.f32 %0, %1;" : "=f"(r) : "f"(x)); return r; }
+
 __device__ __forceinline__ float3 brdf_cos_over_pdf(const ShadeP& sp, const float (&b)[7], float wix, float wiy, float wiz,
                                                     float wox, float woy, float woz, float pdf) {
   const float NoL = b[0] * wix + b[1] * wiy + b[2] * wiz;
@@ -182,19 +199,18 @@ __device__ __forceinline__ float3 brdf_cos_over_pdf(const ShadeP& sp, const floa
   if (sp.brdf_model == 1) {
     const float NoV = fmaxf(b[0] * wox + b[1] * woy + b[2] * woz, 1e-4f);
     float hx = wix + wox, hy = wiy + woy, hz = wiz + woz;
-    const float hn = 1.f / fmaxf(sqrtf(hx * hx + hy * hy + hz * hz), 1e-12f);
+    const float hn = rsqrtf(fmaxf(hx * hx + hy * hy + hz * hz, 1e-24f));
     hx *= hn; hy *= hn; hz *= hn;
     const float NoH = fmaxf(b[0] * hx + b[1] * hy + b[2] * hz, 0.f);
     const float VoH = fmaxf(wox * hx + woy * hy + woz * hz, 0.f);
     const float alpha = b[6] * b[6], k = alpha * alpha;
     const float dd = NoH * NoH * (k - 1.f) + 1.f;
-    const float D = k / (3.14159265358979f * dd * dd);
     const float m = 1.f - VoH, m2 = m * m;
     const float F = sp.f0 + (1.f - sp.f0) * (m2 * m2 * m);
-    const float Gv = 0.5f / (NoL * sqrtf(NoV * NoV * (1.f - k) + k) + NoV * sqrtf(NoL * NoL * (1.f - k) + k));
-    spec = D * F * Gv;
+    const float den = NoL * sqrt_approx(NoV * NoV * (1.f - k) + k) + NoV * sqrt_approx(NoL * NoL * (1.f - k) + k);
+    spec = __fdividef(0.5f * k * F, 3.14159265358979f * dd * dd * den);        // D F G_v
   }
-  const float sc = NoL / pdf;
+  const float sc = __fdividef(NoL, pdf);
   const float ipi = 0.3183098861837907f;
   return make_float3((b[3] * ipi + spec) * sc, (b[4] * ipi + spec) * sc, (b[5] * ipi + spec) * sc);
 }

@@ -207,7 +207,7 @@ template <> struct LevelTaps<false> { float2 v[8]; float w[3]; };
 template <bool F16>
 __device__ __forceinline__ void gather_level(const GridP& g, int l, float x, float y, float z, LevelTaps<F16>& t) {
   const uint32_t N = g.res[l];
-  const Cell cl = cell_of(N, x, y, z);
+  const Cell cl = cell_of_clamped(N, x, y, z);                 // callers pass x' = sec_hit(...), already in [0,1]^3
   uint32_t idx[8];
   corner_indices(cl, N, (g.dense_mask >> l) & 1u, g.log2_T, idx);
   if constexpr (F16) {
@@ -345,6 +345,48 @@ __device__ __forceinline__ void brdf_from_A(Ctx& c, const TcConst& cw, const Sha
   brdf_maps(sp, o, b);
 }
 
+// Primary point only (once per pixel): B in split precision.  n = o/||o|| amplifies an absolute error of o by 1/||o||
+// and every sample of the pixel sees the same n, so fp16-grade activations here would be a COHERENT pixel error; the
+// hi/lo split of f (already in A0[0..31]) and of the hidden layer keeps B's inputs to ~2^-22, layer 3 runs in fp32.
+__device__ __forceinline__ void brdf_precise_from_A(Ctx& c, const TcConst& cw, const ShadeP& sp, float (&b)[7]) {
+  issue_layer(c, 0, kColA, 1, 2, 1, 2, true);
+  wait_layer(c, 0);
+  const uint32_t tD = colD(c, 0), tA = colA(c, 0);
+#pragma unroll
+  for (int h = 0; h < 2; ++h) {
+    uint32_t r[32];
+    tmem_ld32(tD + 32 * h, r);
+    wait_ld();
+    uint32_t p[16], q[16];
+#pragma unroll
+    for (int k = 0; k < 16; ++k) {
+      const float a0 = fmaxf(__uint_as_float(r[2 * k]), 0.f), a1 = fmaxf(__uint_as_float(r[2 * k + 1]), 0.f);
+      p[k] = pack_rn(a0, a1);
+      q[k] = pack_lo(p[k], a0, a1);
+    }
+    tmem_st16(tA + 16 * h, p);
+    tmem_st16(tA + 32 + 16 * h, q);
+  }
+  issue_layer(c, 0, kColA, 3, 4, 1, 3, true);
+  wait_layer(c, 0);
+  float o[8];
+#pragma unroll
+  for (int q = 0; q < 8; ++q) o[q] = cw.Bb3[q];
+#pragma unroll
+  for (int h = 0; h < 2; ++h) {
+    uint32_t r[32];
+    tmem_ld32(tD + 32 * h, r);
+    wait_ld();
+#pragma unroll
+    for (int k = 0; k < 32; ++k) {
+      const float a = fmaxf(__uint_as_float(r[k]), 0.f);
+#pragma unroll
+      for (int q = 0; q < 7; ++q) o[q] = fmaf(a, cw.BW3[q][32 * h + k], o[q]);
+    }
+  }
+  brdf_maps(sp, o, b);
+}
+
 // h1 = relu(P + W1w . w) -> A[buf] columns 0..31 (P in registers)
 __device__ __forceinline__ void h1_from_regs(const Ctx& c, const TcConst& cw, int buf, const float (&P)[kH], float wx, float wy, float wz) {
   const uint32_t tA = colA(c, buf);
@@ -398,6 +440,37 @@ __device__ __forceinline__ void h1_from_regs_shared(const Ctx& c, int buf, const
       p[2 * k + 1] = pack_relu(P[j + 2] + q.z, P[j + 3] + q.w);
     }
     tmem_st16(tA + 16 * h, p);
+  }
+}
+
+// shared direction set, all-fp16x2 form: P and Q both pre-rounded to fp16 pairs, h1 = fma.relu(P, 1, Q): one
+// instruction per pair (the sum is rounded once more: 1.5 ulp of fp16 instead of 0.5 -- tertiary visibility only)
+__device__ __forceinline__ void h1_from_h2_shared(const Ctx& c, int buf, const uint32_t (&Ph)[kH / 2], const uint32_t* __restrict__ Qh) {
+  const uint32_t tA = colA(c, buf);
+#pragma unroll
+  for (int h = 0; h < 2; ++h) {
+    uint32_t p[16];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+      const uint4 q = reinterpret_cast<const uint4*>(Qh)[4 * h + k];
+      const uint32_t qq[4] = {q.x, q.y, q.z, q.w};
+#pragma unroll
+      for (int e = 0; e < 4; ++e)
+        asm("fma.rn.relu.f16x2 %0, %1, %2, %3;" : "=r"(p[4 * k + e]) : "r"(Ph[16 * h + 4 * k + e]), "r"(0x3C003C00u), "r"(qq[e]));
+    }
+    tmem_st16(tA + 16 * h, p);
+  }
+}
+// D0 -> fp16 pairs (32 registers)
+__device__ __forceinline__ void load_D_h2(const Ctx& c, uint32_t (&Ph)[kH / 2]) {
+  const uint32_t tD = colD(c, 0);
+#pragma unroll
+  for (int h = 0; h < 2; ++h) {
+    uint32_t r[32];
+    tmem_ld32(tD + 32 * h, r);
+    wait_ld();
+#pragma unroll
+    for (int k = 0; k < 16; ++k) Ph[16 * h + k] = pack_rn(__uint_as_float(r[2 * k]), __uint_as_float(r[2 * k + 1]));
   }
 }
 
@@ -476,8 +549,9 @@ __device__ __forceinline__ void teardown(const Ctx& c) {
 // ---------------------------------------------------------------------------------------------------- kernels
 struct SecRay { float v, wx, wy, wz, pdf, x, y, z; };   // one secondary direction of a pixel: visibility, direction, pdf, hit x'
 
-// render_frame (a1-a11), tensor-core path.
-template <bool F16>
+// render_frame (a1-a11), tensor-core path.  TSHARED: the tertiary set is one shared set (point_stride == 0).
+// LPI: levels of the next secondary point's gathers carried per tertiary iteration (0 = none; 2 needs S_2 == 8).
+template <bool F16, bool TSHARED, int LPI>
 __global__ void __launch_bounds__(kThreads, kCtasPerSm) k_render_tc(const __grid_constant__ GridP g, EnvP env, ShadeP sp,
                                                                     const __grid_constant__ TcConst cw, const uint8_t* __restrict__ wtiles,
                                                                     FrameP fr, float* __restrict__ rgb) {
@@ -486,12 +560,13 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) k_render_tc(const __grid
   Ctx c;
   setup(s, wtiles, c);
   const bool indirect = (fr.flags & 4u) && fr.s.S && fr.t.S;
-  const bool tshared = fr.t.stride == 0;
+  constexpr bool tshared = TSHARED;
   if (indirect && tshared) {                    // shared tertiary set: Q_k = W1w . w'_k; per k: radiance, pdf, direction
     for (int e = threadIdx.x; e < (int)fr.t.S * kH; e += kThreads) {
       const int k = e / kH, q = e % kH;
       const float* dp = fr.t.dir + 3 * k;
-      s.Qt[e] = cw.w1w[0][q] * __ldg(dp) + cw.w1w[1][q] * __ldg(dp + 1) + cw.w1w[2][q] * __ldg(dp + 2);
+      const float qv = cw.w1w[0][q] * __ldg(dp) + cw.w1w[1][q] * __ldg(dp + 1) + cw.w1w[2][q] * __ldg(dp + 2);
+      reinterpret_cast<__half*>(s.Qt)[e] = __float2half_rn(qv);    // Qh[k][q], fp16
     }
     for (int k = threadIdx.x; k < (int)fr.t.S; k += kThreads) {
       const float* dp = fr.t.dir + 3 * k;
@@ -508,7 +583,7 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) k_render_tc(const __grid
   const unsigned long long ntiles = (fr.N + kThreads - 1) / kThreads;
   const int jend = indirect ? (int)fr.s.S : 0;
   // levels of the NEXT secondary point gathered per tertiary iteration (0 = the tertiary loop cannot carry them)
-  const int lpi = (indirect && fr.t.S >= 4 && fr.t.S <= 16 && (16 % fr.t.S) == 0) ? 16 / (int)fr.t.S : 0;
+  constexpr int lpi = LPI;
 
   for (unsigned long long tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
     const unsigned long long i_raw = tile * kThreads + threadIdx.x;
@@ -531,7 +606,7 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) k_render_tc(const __grid
 #pragma unroll
         for (int k = 0; k < 7; ++k) b[k] = __ldg(fr.brdf + i * 7 + k);
       } else {
-        brdf_from_A(c, cw, sp, kColA, b);                           // A0[0..15] still holds f (hi)
+        brdf_precise_from_A(c, cw, sp, b);                          // A0[0..31] still holds f (hi | lo)
       }
       if (jend > 0) {
 #pragma unroll
@@ -553,13 +628,13 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) k_render_tc(const __grid
           dp = dir_of(fr.d, i, s2);
           const float d2x = __ldg(dp), d2y = __ldg(dp + 1), d2z = __ldg(dp + 2), d2p = pdf_of(fr.d, i, s2);
           float vd = 1.f;
+          if (shadow && k + 1 < S) { h1_from_regs(c, cw, bf ^ 1, P, d1x, d1y, d1z); issue_layer(c, bf ^ 1, kColA + kBufStride * (bf ^ 1), 2, 4, 0, 3); }
+          const float3 gg = brdf_cos_over_pdf(sp, b, d0x, d0y, d0z, ox, oy, oz, d0p);
+          const float3 L = incoming(env, fr.d, i, k, d0x, d0y, d0z);
           if (shadow) {
-            if (k + 1 < S) { h1_from_regs(c, cw, bf ^ 1, P, d1x, d1y, d1z); issue_layer(c, bf ^ 1, kColA + kBufStride * (bf ^ 1), 2, 4, 0, 3); }
             wait_layer(c, bf);
             vd = vis_of(sp, irt_epilogue_fast(c, cw, bf));
           }
-          const float3 gg = brdf_cos_over_pdf(sp, b, d0x, d0y, d0z, ox, oy, oz, d0p);
-          const float3 L = incoming(env, fr.d, i, k, d0x, d0y, d0z);
           ar = fmaf(vd * L.x, gg.x, ar); ag = fmaf(vd * L.y, gg.y, ag); ab = fmaf(vd * L.z, gg.z, ab);
           d0x = d1x; d0y = d1y; d0z = d1z; d0p = d1p;
           d1x = d2x; d1y = d2y; d1z = d2z; d1p = d2p;
@@ -594,8 +669,9 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) k_render_tc(const __grid
         // a1-a5 at x'_j: its features wait in the staging columns
         issue_layer(c, 0, kColNext, 0, 2, 0, 2);
         wait_layer(c, 0);
-        float P2[kH];
-        load_D(c, P2);
+        float P2[TSHARED ? 1 : kH];
+        uint32_t P2h[TSHARED ? kH / 2 : 1];
+        if constexpr (TSHARED) load_D_h2(c, P2h); else load_D(c, P2);
         float bb[7];
         brdf_from_A(c, cw, sp, kColNext, bb);
         const bool have_next = j + 1 < jend;
@@ -606,7 +682,7 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) k_render_tc(const __grid
         const unsigned long long trow = tshared ? 0ull : i * fr.s.S + j;
         float lr = 0.f, lg = 0.f, lb = 0.f;
         auto h1t = [&](uint32_t k, int bf) {
-          if (tshared) h1_from_regs_shared(c, bf, P2, s.Qt + k * kH);
+          if constexpr (TSHARED) h1_from_h2_shared(c, bf, P2h, reinterpret_cast<const uint32_t*>(s.Qt) + k * (kH / 2));
           else { const float* tp = dir_of(fr.t, trow, k); h1_from_regs(c, cw, bf, P2, __ldg(tp), __ldg(tp + 1), __ldg(tp + 2)); }
         };
         h1t(0, 0);
@@ -614,19 +690,17 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) k_render_tc(const __grid
         const uint32_t tN = colNext(c);
         for (uint32_t k = 0; k < S2; ++k) {
           const int bf = k & 1;
-          LevelTaps<F16> taps[4];
-          const bool carry = have_next && lpi > 0;
+          LevelTaps<F16> taps[LPI > 0 ? LPI : 1];
+          const bool carry = have_next && LPI > 0;
           if (carry) {
 #pragma unroll
-            for (int q = 0; q < 4; ++q) {
-              const int l = (int)k * lpi + q;
-              if (q < lpi && l < (int)g.L) gather_level<F16>(g, l, nxt.x, nxt.y, nxt.z, taps[q]);
+            for (int q = 0; q < LPI; ++q) {
+              const int l = (int)k * LPI + q;
+              if (l < (int)g.L) gather_level<F16>(g, l, nxt.x, nxt.y, nxt.z, taps[q]);
             }
           }
           if (k + 1 < S2) { h1t(k + 1, bf ^ 1); issue_layer(c, bf ^ 1, kColA + kBufStride * (bf ^ 1), 2, 4, 0, 3); }
-          wait_layer(c, bf);
-          const float v2 = vis_of(sp, irt_epilogue_fast(c, cw, bf));
-          float tx, ty, tz, tpdf;
+          float tx, ty, tz, tpdf;                                   // shading factors first: they do not need the MMA
           float3 L;
           if (tshared) {
             const float4 a = reinterpret_cast<const float4*>(s.Lt)[2 * k], d = reinterpret_cast<const float4*>(s.Lt)[2 * k + 1];
@@ -637,16 +711,18 @@ __global__ void __launch_bounds__(kThreads, kCtasPerSm) k_render_tc(const __grid
             L = incoming(env, fr.t, trow, k, tx, ty, tz);
           }
           const float3 gg = brdf_cos_over_pdf(sp, bb, tx, ty, tz, -cur.wx, -cur.wy, -cur.wz, tpdf);
+          wait_layer(c, bf);
+          const float v2 = vis_of(sp, irt_epilogue_fast(c, cw, bf));
           lr = fmaf(v2 * L.x, gg.x, lr); lg = fmaf(v2 * L.y, gg.y, lg); lb = fmaf(v2 * L.z, gg.z, lb);
           if (carry) {
 #pragma unroll
-            for (int q = 0; q < 4; ++q) {
-              const int l = (int)k * lpi + q;
-              if (q < lpi) tmem_st1(tN + l, l < (int)g.L ? lerp_level(taps[q]) : 0u);
+            for (int q = 0; q < LPI; ++q) {
+              const int l = (int)k * LPI + q;
+              tmem_st1(tN + l, l < (int)g.L ? lerp_level(taps[q]) : 0u);
             }
           }
         }
-        if (have_next && lpi == 0) encode_next_plain<F16>(g, c, nxt.x, nxt.y, nxt.z);
+        if (have_next && LPI == 0) encode_next_plain<F16>(g, c, nxt.x, nxt.y, nxt.z);
         const float3 gg = brdf_cos_over_pdf(sp, b, cur.wx, cur.wy, cur.wz, ox, oy, oz, cur.pdf);
         const float m = (1.f - cur.v) / (float)S2;
         ir = fmaf(m * lr, gg.x, ir); ig = fmaf(m * lg, gg.y, ig); ib = fmaf(m * lb, gg.z, ib);
@@ -745,8 +821,11 @@ inline void prepare_weights(const hr_config& cfg, const float* bw, const float* 
 
 inline cudaError_t set_attributes() {
   cudaError_t e;
-  if ((e = cudaFuncSetAttribute(k_render_tc<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes))) return e;
-  if ((e = cudaFuncSetAttribute(k_render_tc<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes))) return e;
+#define HR_TC_ATTR(K) if ((e = cudaFuncSetAttribute(K, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes))) return e
+  HR_TC_ATTR((k_render_tc<true, true, 2>)); HR_TC_ATTR((k_render_tc<true, true, 0>));
+  HR_TC_ATTR((k_render_tc<true, false, 2>)); HR_TC_ATTR((k_render_tc<true, false, 0>));
+  HR_TC_ATTR((k_render_tc<false, true, 0>)); HR_TC_ATTR((k_render_tc<false, false, 0>));
+#undef HR_TC_ATTR
   if ((e = cudaFuncSetAttribute(k_trace_tc<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes))) return e;
   if ((e = cudaFuncSetAttribute(k_trace_tc<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes))) return e;
   return cudaSuccess;
@@ -764,8 +843,16 @@ inline int grid_size(unsigned long long N, int num_sms) {
 inline cudaError_t launch_render(const GridP& g, const EnvP& env, const ShadeP& sp, const TcConst& cw, const uint8_t* d_tiles,
                                  const FrameP& fr, float* rgb, int num_sms, cudaStream_t st) {
   const int grid = grid_size(fr.N, num_sms);
-  if (g.f16) k_render_tc<true><<<grid, kThreads, kSmemBytes, st>>>(g, env, sp, cw, d_tiles, fr, rgb);
-  else k_render_tc<false><<<grid, kThreads, kSmemBytes, st>>>(g, env, sp, cw, d_tiles, fr, rgb);
+  const bool tsh = fr.t.stride == 0;
+  const bool carry = (fr.flags & 4u) && fr.t.S == 8;          // 16 levels / 8 tertiary iterations = 2 levels each
+#define HR_TC_LAUNCH(K) K<<<grid, kThreads, kSmemBytes, st>>>(g, env, sp, cw, d_tiles, fr, rgb)
+  if (g.f16) {
+    if (tsh) { if (carry) HR_TC_LAUNCH((k_render_tc<true, true, 2>)); else HR_TC_LAUNCH((k_render_tc<true, true, 0>)); }
+    else { if (carry) HR_TC_LAUNCH((k_render_tc<true, false, 2>)); else HR_TC_LAUNCH((k_render_tc<true, false, 0>)); }
+  } else {
+    if (tsh) HR_TC_LAUNCH((k_render_tc<false, true, 0>)); else HR_TC_LAUNCH((k_render_tc<false, false, 0>));
+  }
+#undef HR_TC_LAUNCH
   return cudaGetLastError();
 }
 
