@@ -259,10 +259,10 @@ def main():
         if e2e_steps:
             pin = lambda a: torch.from_numpy(a).pin_memory().numpy()
             hx, hwo = pin(fr["x"]), pin(fr["wo"])
-            hd = DirSet(pin(fr["dir_d"]), pin(fr["pdf_d"]))
+            hdir = DirSet(pin(fr["dir_d"]), pin(fr["pdf_d"]))
             hs = DirSet(pin(fr["dir_s"]), pin(fr["pdf_s"])) if indirect else None
             ht = DirSet(pin(fr["dir_t"]), pin(fr["pdf_t"])) if indirect else None
-            hframe = r.make_frame(hx, hwo, hd, hs, ht, flags=cfg.flags)
+            hframe = r.make_frame(hx, hwo, hdir, hs, ht, flags=cfg.flags)
             hrgb = torch.empty((cfg.N, 3), dtype=torch.float32).pin_memory().numpy()
             upb, downb = r.render_frame_host(hframe, hrgb, stream)      # warm-up (allocates staging)
             torch.cuda.synchronize()
