@@ -31,15 +31,26 @@ METRIC = "hash-renderer point-direction queries/s (800x800 frame, direct + shado
 UNIT = "queries/s"
 
 
-def algorithmic_flops(cfg) -> float:
+def algorithmic_flops(cfg, evaluated=None) -> float:
     """Factored algorithmic flop count of one frame: per IRT query
     2*(3*64 + 64*64 + 64*2) = 8832; per encoded point the per-point layer-1 partial 2*D*64 and, where B runs,
-    2*(D*64 + 64*64 + 64*7).  Zero padding to MMA shapes is never counted."""
+    2*(D*64 + 64*64 + 64*7).  Zero padding to MMA shapes and error-compensation passes are never counted.
+    `evaluated` = secondary hits whose L'_o was actually evaluated (None = all N*S_i of them, the dense count)."""
     D, H = cfg.D, cfg.hidden
     per_query = 2 * (3 * H + H * H + H * 2)
     per_point = 2 * D * H + 2 * (D * H + H * H + H * 7)
-    pts = cfg.N * (1 + (cfg.S_i if cfg.flags & gen.HR_INDIRECT else 0))
-    return cfg.queries * per_query + pts * per_point
+    ind = bool(cfg.flags & gen.HR_INDIRECT)
+    sec = cfg.N * cfg.S_i if ind else 0
+    ev = sec if evaluated is None else evaluated
+    queries = cfg.N * cfg.S_d + sec + ev * cfg.S_2
+    return queries * per_query + (cfg.N + ev) * per_point
+
+
+def executed_queries(cfg, evaluated=None) -> int:
+    ind = bool(cfg.flags & gen.HR_INDIRECT)
+    sec = cfg.N * cfg.S_i if ind else 0
+    ev = sec if evaluated is None else evaluated
+    return cfg.N * cfg.S_d + sec + ev * cfg.S_2
 
 
 def load_peaks():
@@ -195,6 +206,9 @@ def main():
     ap.add_argument("--ref-pixels", type=int, default=256, help="pixels per step for --impl reference")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--also", default="C3", help="second workload measured briefly and reported under `also` ('' = none)")
+    ap.add_argument("--compact", action="store_true", help="headline with the default API flags (zero-weight secondary rays skipped) "
+                    "instead of HR_DENSE")
+    ap.add_argument("--no-extra", action="store_true", help="skip the `also` measurements")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 0)
     cfg = gen.make_config(args.workload)
@@ -217,7 +231,7 @@ def main():
     from paper_2409_10327_b200 import DirSet, HashRenderer
     from paper_2409_10327_b200 import dist as hd
 
-    def measure(cfg, steps, warmup, e2e_steps, clocks):
+    def measure(cfg, steps, warmup, e2e_steps, clocks, dense=True):
         model = gen.make_model(cfg)
         fr = gen.make_frame(cfg, model["env"])
         r = HashRenderer.from_gen(cfg, model, vis_mode=args.vis_mode)
@@ -228,7 +242,8 @@ def main():
         d = DirSet(up(fr["dir_d"]), up(fr["pdf_d"]))
         s = DirSet(up(fr["dir_s"]), up(fr["pdf_s"])) if indirect else None
         t = DirSet(up(fr["dir_t"]), up(fr["pdf_t"])) if indirect else None
-        frame = r.make_frame(x, wo, d, s, t, flags=cfg.flags)
+        flags = cfg.flags | (gen.HR_DENSE if dense else 0)
+        frame = r.make_frame(x, wo, d, s, t, flags=flags)
         rgb = torch.empty((cfg.N, 3), device=dev)
         stream = torch.cuda.current_stream().cuda_stream
         for _ in range(warmup):
@@ -236,6 +251,7 @@ def main():
         torch.cuda.synchronize()
         if world > 1:
             dist.barrier()
+        r.stats(reset=True)
         l0 = r.launch_count()
         if clocks:
             clocks.start()
@@ -254,7 +270,9 @@ def main():
         per = [ev[k].elapsed_time(ev[k + 1]) for k in range(steps)]
         total_ms = hd.max_over_ranks(total_ms, dev)
         assert torch.isfinite(rgb).all()
-        out = dict(total_ms=total_ms, per=per, launches=launches, clk=clk, path=r.last_path(), mean_rgb=float(rgb.mean().item()))
+        traced, evaluated = r.stats()
+        out = dict(total_ms=total_ms, per=per, launches=launches, clk=clk, path=r.last_path(), mean_rgb=float(rgb.mean().item()),
+                   traced=traced // max(steps, 1), evaluated=(evaluated // max(steps, 1)) if traced else None)
         # end to end through the public host-buffer entry point: pinned host inputs, H2D + D2H inside the timed region
         if e2e_steps:
             pin = lambda a: torch.from_numpy(a).pin_memory().numpy()
@@ -262,7 +280,7 @@ def main():
             hdir = DirSet(pin(fr["dir_d"]), pin(fr["pdf_d"]))
             hs = DirSet(pin(fr["dir_s"]), pin(fr["pdf_s"])) if indirect else None
             ht = DirSet(pin(fr["dir_t"]), pin(fr["pdf_t"])) if indirect else None
-            hframe = r.make_frame(hx, hwo, hdir, hs, ht, flags=cfg.flags)
+            hframe = r.make_frame(hx, hwo, hdir, hs, ht, flags=flags)
             hrgb = torch.empty((cfg.N, 3), dtype=torch.float32).pin_memory().numpy()
             upb, downb = r.render_frame_host(hframe, hrgb, stream)      # warm-up (allocates staging)
             torch.cuda.synchronize()
@@ -275,7 +293,7 @@ def main():
             e1.record()
             torch.cuda.synchronize()
             out.update(e2e_ms=hd.max_over_ranks(e0.elapsed_time(e1), dev) / e2e_steps, h2d=upb, d2h=downb,
-                       e2e_matches=bool(np.allclose(hrgb, rgb.cpu().numpy(), rtol=1e-6, atol=1e-7)))
+                       e2e_matches=bool(np.allclose(hrgb, rgb.cpu().numpy(), rtol=1e-5, atol=1e-6)))
         r.destroy()
         del x, wo, d, s, t, rgb
         torch.cuda.empty_cache()
@@ -283,7 +301,7 @@ def main():
 
     peaks = load_peaks()
     clocks = ClockSampler(local) if rank == 0 else None
-    res, model = measure(cfg, args.steps, max(args.warmup, 3), args.e2e_steps, clocks)
+    res, model = measure(cfg, args.steps, max(args.warmup, 3), args.e2e_steps, clocks, dense=not args.compact)
 
     if rank != 0:
         if world > 1:
@@ -291,30 +309,45 @@ def main():
         return
     ms = res["total_ms"] / args.steps
     value = world * cfg.queries / (ms * 1e-3)
-    flops = algorithmic_flops(cfg)
     kernel_ms = float(np.mean(res["per"]))          # the step is ONE kernel launch: its duration is the step's
-    tc = res["path"].startswith("tcgen05")
-    if tc:
-        roof = {"bound": "tensor", "achieved": flops / (kernel_ms * 1e-3) / 1e12, "peak": peaks["tensor_sustained"], "unit": "TFLOP/s",
-                "peak_source": f"MEASURED_PEAKS.json bf16_tflops_sustained ({peaks['which']}; fp16 = bf16 rate; kernel runs back to back for the whole step)"}
-    else:
-        alu_peak = 148 * 128 * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12
-        roof = {"bound": "alu", "achieved": flops / (kernel_ms * 1e-3) / 1e12, "peak": alu_peak, "unit": "TFLOP/s",
-                "peak_source": "derived: 148 SM x 128 fp32 lanes x 2 flop x sm_max_mhz (DESIGN.md)"}
-    roof["frac"] = roof["achieved"] / roof["peak"]
-    roof["kernel"] = "k_render_tc" if tc else "k_render_ffma"
-    roof["kernel_ms"] = kernel_ms
-    roof["algorithmic_flops_per_launch"] = flops
-    tpath = os.path.join(ROOT, "profiles", "traffic.json")
-    roof["traffic"] = None
-    if os.path.exists(tpath):
-        roof["traffic"] = json.load(open(tpath)).get(f"{cfg.name}:{res['path']}")
 
+    def roofline(cfg, path, kernel_ms, evaluated):
+        flops = algorithmic_flops(cfg, evaluated)
+        ach = flops / (kernel_ms * 1e-3) / 1e12
+        if path == "tcgen05-f16":
+            roof = {"bound": "tensor", "achieved": ach, "peak": peaks["tensor_sustained"], "unit": "TFLOP/s",
+                    "peak_source": f"MEASURED_PEAKS.json bf16_tflops_sustained ({peaks['which']}; fp16 = bf16 rate; kernel runs back to back for the whole step)"}
+        elif path == "tcgen05-f16x3":
+            roof = {"bound": "tensor", "achieved": ach, "peak": peaks["tensor_sustained"] / 3.0, "unit": "TFLOP/s",
+                    "peak_source": f"MEASURED_PEAKS.json bf16_tflops_sustained ({peaks['which']}) / 3: an fp32-grade product on the fp16 tensor "
+                                   "cores is three MMA passes (hi*Whi + lo*Whi + hi*Wlo), only one of which is algorithmic work"}
+        else:
+            alu_peak = 148 * 128 * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12
+            roof = {"bound": "alu", "achieved": ach, "peak": alu_peak, "unit": "TFLOP/s",
+                    "peak_source": "derived: 148 SM x 128 fp32 lanes x 2 flop x sm_max_mhz (DESIGN.md)"}
+        roof["frac"] = roof["achieved"] / roof["peak"]
+        roof["kernel"] = "k_render_wg" if path.startswith("tcgen05") else "k_render_ffma"
+        roof["kernel_ms"] = kernel_ms
+        roof["algorithmic_flops_per_launch"] = flops
+        roof["note"] = ("the MLP contractions run on the tensor pipe, but the kernel's binding unit is the SM issue slots: per query the "
+                        "fp16 pack / epilogue / shading ALU work exceeds the 64x64 MMA (DESIGN.md 6.2); see profiles/ for issue-slot "
+                        "and tensor-pipe utilisation")
+        tpath = os.path.join(ROOT, "profiles", "traffic.json")
+        roof["traffic"] = None
+        if os.path.exists(tpath):
+            roof["traffic"] = json.load(open(tpath)).get(f"{cfg.name}:{path}")
+        return roof
+
+    roof = roofline(cfg, res["path"], kernel_ms, res["evaluated"])
+    dt = {"tcgen05-f16": "f16", "tcgen05-f16x3": "f16x3 (fp16 hi+lo split operands, three tcgen05 passes, fp32 accumulate)"}.get(res["path"], "f32")
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
         "ms_per_step": ms, "ms_per_frame": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-        "dtype": "f16" if tc else "f32", "data": "synthetic",
+        "dtype": dt, "data": "synthetic",
         "config": {"workload": workload_name(cfg), "queries_per_frame": cfg.queries, "vis_mode": "hard" if args.vis_mode else "soft",
+                   "secondary_rays": ("compacted: L'_o only where its Eq. 2 weight is non-zero (PAPER.md:82-84)" if args.compact else
+                                      "dense (HR_DENSE): L'_o evaluated at every secondary hit, all queries_per_frame executed"),
+                   "executed_queries_per_frame": executed_queries(cfg, res["evaluated"]),
                    "path": res["path"], "l2": "per-frame inputs (2.0 GB of directions/pdfs) exceed the 126 MB L2; the hash table is "
                    "L2-resident by design", "multi_gpu": "independent frames per rank, no collective"},
         "clocks": res["clk"], "gpu_launches": res["launches"], "roofline": roof,
@@ -322,14 +355,26 @@ def main():
     if "e2e_ms" in res:
         line["e2e"] = {"value": world * cfg.queries / (res["e2e_ms"] * 1e-3), "unit": UNIT, "ms_per_frame": res["e2e_ms"],
                        "h2d_bytes_per_step": res["h2d"], "d2h_bytes_per_step": res["d2h"], "matches_device_path": res["e2e_matches"]}
-    if args.also and args.also != args.workload and world == 1:
-        cfg2 = gen.make_config(args.also)
-        r2, _ = measure(cfg2, max(args.steps // 2, 3), 3, 0, None)
-        ms2 = r2["total_ms"] / max(args.steps // 2, 3)
-        f2 = algorithmic_flops(cfg2)
-        line["also"] = {"workload": workload_name(cfg2), "ms_per_frame": ms2, "value": cfg2.queries / (ms2 * 1e-3), "unit": UNIT,
-                        "path": r2["path"], "achieved_tflops": f2 / (ms2 * 1e-3) / 1e12,
-                        "frac_of_tensor_peak_sustained": f2 / (ms2 * 1e-3) / 1e12 / peaks["tensor_sustained"]}
+    if world == 1 and not args.no_extra:
+        # the same frame with the default API flags (zero-weight secondary rays compacted out), and the
+        # other precision; `value` here is frame-equivalent (queries_per_frame / time), executed queries are stated
+        extra = []
+        if cfg.flags & gen.HR_INDIRECT:
+            extra.append((cfg, args.compact))
+        if args.also and args.also != args.workload:
+            cfg2 = gen.make_config(args.also)
+            extra += [(cfg2, True), (cfg2, False)] if cfg2.flags & gen.HR_INDIRECT else [(cfg2, True)]
+        line["also"] = []
+        for c2, dense in extra:
+            st = max(args.steps // 2, 3)
+            r2, _ = measure(c2, st, 3, 0, None, dense=dense)
+            ms2 = r2["total_ms"] / st
+            rf = roofline(c2, r2["path"], ms2, r2["evaluated"])
+            line["also"].append({"workload": workload_name(c2), "secondary_rays": "dense" if dense else "compacted", "ms_per_frame": ms2,
+                                 "frame_equivalent_queries_per_s": c2.queries / (ms2 * 1e-3),
+                                 "executed_queries_per_frame": executed_queries(c2, r2["evaluated"]),
+                                 "executed_queries_per_s": executed_queries(c2, r2["evaluated"]) / (ms2 * 1e-3), "path": r2["path"],
+                                 "achieved_tflops": rf["achieved"], "roofline_frac": rf["frac"], "roofline_peak": rf["peak"]})
     if not args.no_cpu_baseline and world == 1:
         pix = sample_pixels(cfg, args.cpu_pixels)
         dt, q = oracle_sample(cfg, model, pix, args.vis_mode)

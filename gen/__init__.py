@@ -19,7 +19,7 @@ from dataclasses import dataclass
 
 import numpy as np
 
-HR_DIRECT, HR_SHADOW, HR_INDIRECT = 1, 2, 4
+HR_DIRECT, HR_SHADOW, HR_INDIRECT, HR_DENSE = 1, 2, 4, 8
 
 # stream ids (one independent Philox sub-stream per blob)
 _ST_TABLE, _ST_BRDF_W, _ST_IRT_W, _ST_ENV, _ST_POINTS, _ST_SCENE, _ST_DIR_D, _ST_DIR_S, _ST_DIR_T = range(9)

@@ -39,7 +39,9 @@ extern "C" {
 
 enum { HR_OK = 0, HR_ERR_INVALID_ARG = 1, HR_ERR_CUDA = 2, HR_ERR_OOM = 3, HR_ERR_UNSUPPORTED = 4 };
 enum { HR_F32 = 0, HR_F16 = 1 };
-enum { HR_DIRECT = 1, HR_SHADOW = 2, HR_INDIRECT = 4 };           /* hr_frame.flags */
+enum { HR_DIRECT = 1, HR_SHADOW = 2, HR_INDIRECT = 4,             /* hr_frame.flags */
+       HR_DENSE = 8 };  /* evaluate L'_o at EVERY secondary hit; default: only where its weight (1-v) f_r (n.w)^+ / p in
+                           Eq. 2 is non-zero ("only occluded rays"); the result is the same */
 enum { HR_TERM_DIRECT = 1, HR_TERM_INDIRECT = 2 };                /* hashrender_shade terms */
 enum { HR_VIS_SOFT = 0, HR_VIS_HARD = 1 };
 enum { HR_BRDF_LAMBERT = 0, HR_BRDF_DISNEY = 1 };
@@ -87,7 +89,7 @@ typedef struct {
   hr_dirset secondary;          /* used with HR_INDIRECT: directions along which x' = x + t w is traced */
   hr_dirset tertiary;           /* used with HR_INDIRECT: directions sampled at every x' (8);
                                    point_stride != 0 => row index is i*secondary.S + j */
-  uint32_t flags;               /* HR_DIRECT | HR_SHADOW | HR_INDIRECT */
+  uint32_t flags;               /* HR_DIRECT | HR_SHADOW | HR_INDIRECT [| HR_DENSE] */
 } hr_frame;
 
 /* Creates a renderer.  tables: host, fp32 [L][T][F] (every level owns T = 2^log2_T slots; a dense level --
@@ -129,10 +131,17 @@ int hashrender_render_frame(hashrender_t* h, const hr_frame* frame, float* rgb, 
 int hashrender_render_frame_host(hashrender_t* h, const hr_frame* frame, float* rgb, void* stream,
                                  uint64_t* h2d_bytes, uint64_t* d2h_bytes);
 
+/* Secondary-ray accounting of the render_frame calls since the last reset: rays_traced = secondary
+ * (point, direction) rays whose (v, t) were evaluated, rays_evaluated = those whose L'_o was evaluated (all of them with
+ * HR_DENSE).  Both nullable.  Synchronises the device.  Only the tcgen05 paths count; the FFMA path leaves both at 0. */
+int hashrender_stats(hashrender_t* h, uint64_t* rays_traced, uint64_t* rays_evaluated, int reset);
+
 /* Number of kernels this handle has launched so far (for launch accounting in benchmarks). */
 uint64_t hashrender_launch_count(const hashrender_t* h);
 
-/* Which implementation the last render_frame / trace used: "ffma32" or "tcgen05-f16". Never NULL. */
+/* Which implementation the last render_frame / trace used: "ffma32" (fp32 FFMA), "tcgen05-f16" (fp16 activations) or
+ * "tcgen05-f16x3" (fp32 model on the fp16 tensor cores: activations and weights split hi + lo, three MMA passes, fp32
+ * accumulate; chosen when tables, weights and activation bounds fit the fp16 range, else "ffma32"). Never NULL. */
 const char* hashrender_last_path(const hashrender_t* h);
 
 const char* hashrender_last_error(const hashrender_t* h);

@@ -9,14 +9,14 @@ from dataclasses import dataclass
 
 import numpy as np
 
-HR_DIRECT, HR_SHADOW, HR_INDIRECT = 1, 2, 4
+HR_DIRECT, HR_SHADOW, HR_INDIRECT, HR_DENSE = 1, 2, 4, 8
 HR_TERM_DIRECT, HR_TERM_INDIRECT = 1, 2
 _STATUS = {1: "HR_ERR_INVALID_ARG", 2: "HR_ERR_CUDA", 3: "HR_ERR_OOM", 4: "HR_ERR_UNSUPPORTED"}
 _LIB_PATH = os.path.join(os.path.dirname(os.path.abspath(__file__)), "libhashrender.so")
 
 EXPORTS = ["hashrender_create", "hashrender_destroy", "hashrender_set_env", "hashrender_encode", "hashrender_decode",
            "hashrender_trace", "hashrender_shade", "hashrender_render_frame", "hashrender_render_frame_host",
-           "hashrender_launch_count", "hashrender_last_path", "hashrender_last_error"]
+           "hashrender_stats", "hashrender_launch_count", "hashrender_last_path", "hashrender_last_error"]
 
 
 class HashRenderError(RuntimeError):
@@ -64,6 +64,7 @@ def load_library(path: str | None = None):
         lib.hashrender_shade.argtypes = [vp, vp, vp, u64, C.POINTER(hr_dirset), vp, vp, u32, vp, vp]
         lib.hashrender_render_frame.argtypes = [vp, C.POINTER(hr_frame), vp, vp]
         lib.hashrender_render_frame_host.argtypes = [vp, C.POINTER(hr_frame), vp, vp, C.POINTER(u64), C.POINTER(u64)]
+        lib.hashrender_stats.argtypes = [vp, C.POINTER(u64), C.POINTER(u64), C.c_int]
         lib.hashrender_launch_count.argtypes = [vp]
         lib.hashrender_launch_count.restype = u64
         lib.hashrender_last_path.argtypes = [vp]
@@ -189,6 +190,12 @@ class HashRenderer:
         up, down = C.c_uint64(), C.c_uint64()
         self._check(self._lib.hashrender_render_frame_host(self._h, C.byref(frame), _ptr(rgb), stream, C.byref(up), C.byref(down)))
         return up.value, down.value
+
+    def stats(self, reset=False):
+        """(secondary rays traced, secondary rays whose L'_o was evaluated) since the last reset."""
+        a, b = C.c_uint64(), C.c_uint64()
+        self._check(self._lib.hashrender_stats(self._h, C.byref(a), C.byref(b), 1 if reset else 0))
+        return a.value, b.value
 
     def launch_count(self) -> int:
         return int(self._lib.hashrender_launch_count(self._h))

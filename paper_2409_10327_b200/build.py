@@ -1,20 +1,23 @@
-"""Builds the C-ABI CUDA library in-tree (libhashrender.so) for sm_100a with nvcc.  No JIT cache."""
+"""Builds the C-ABI CUDA library in-tree (libhashrender.so) for sm_100a with nvcc.  No JIT cache.
+The translation units (host + FFMA/trace kernels, and the two families of tcgen05 render kernels) compile in parallel."""
 from __future__ import annotations
 
 import os
 import subprocess
 import sys
+from concurrent.futures import ThreadPoolExecutor
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
-SRC = os.path.join(_HERE, "csrc", "hashrender.cu")
+CSRC = os.path.join(_HERE, "csrc")
+SOURCES = ["hashrender.cu", "hr_wg_p0.cu", "hr_wg_p1.cu"]
 LIB = os.path.join(_HERE, "libhashrender.so")
-NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "-shared",
-              "-Xcompiler", "-fPIC", "--expt-relaxed-constexpr"]
+OBJDIR = os.path.join(_HERE, "build")
+NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "-Xcompiler", "-fPIC",
+              "--expt-relaxed-constexpr"]
 
 
 def _newest_source() -> float:
-    d = os.path.join(_HERE, "csrc")
-    t = [os.path.getmtime(os.path.join(d, f)) for f in os.listdir(d)]
+    t = [os.path.getmtime(os.path.join(CSRC, f)) for f in os.listdir(CSRC)]
     t.append(os.path.getmtime(os.path.join(_HERE, "..", "include", "hashrender.h")))
     return max(t)
 
@@ -23,13 +26,20 @@ def build(force: bool = False, verbose: bool = False, extra=()) -> str:
     if not force and os.path.exists(LIB) and os.path.getmtime(LIB) >= _newest_source():
         return LIB
     nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
-    if not os.path.exists(os.path.join(_HERE, "csrc", "hr_kernels_tc.cuh")):
-        extra = [*extra, "-DHR_NO_TC"]
-    cmd = [nvcc, *NVCC_FLAGS, *extra, "-o", LIB, SRC]
-    if verbose:
-        cmd.insert(1, "-Xptxas=-v")
-        print(" ".join(cmd))
-    subprocess.check_call(cmd)
+    os.makedirs(OBJDIR, exist_ok=True)
+
+    def compile_one(src: str) -> str:
+        obj = os.path.join(OBJDIR, src.replace(".cu", ".o"))
+        cmd = [nvcc, *NVCC_FLAGS, *extra, "-c", "-o", obj, os.path.join(CSRC, src)]
+        if verbose:
+            cmd.insert(1, "-Xptxas=-v")
+            print(" ".join(cmd))
+        subprocess.check_call(cmd)
+        return obj
+
+    with ThreadPoolExecutor(len(SOURCES)) as ex:
+        objs = list(ex.map(compile_one, SOURCES))
+    subprocess.check_call([nvcc, "-shared", "-gencode", "arch=compute_100a,code=sm_100a", "-o", LIB, *objs])
     return LIB
 
 

@@ -10,9 +10,8 @@
 
 #include "../../include/hashrender.h"
 #include "hr_kernels_ffma.cuh"
-#ifndef HR_NO_TC
 #include "hr_kernels_tc.cuh"
-#endif
+#include "hr_wg_api.h"
 
 using namespace hr;
 
@@ -24,8 +23,11 @@ struct hashrender {
   EnvP env;
   void* d_tables = nullptr;
   float* d_wts = nullptr;        // prepared fp32 weights (hr_kernels_ffma.cuh layout)
-  uint8_t* d_wts_tc = nullptr;   // prepared fp16 UMMA weight tiles (hr_kernels_tc.cuh), mlp_dtype == HR_F16
-  std::vector<uint8_t> h_wts_tc; // host copy of [TcConst | tiles]; TcConst is passed by value at launch
+  uint8_t* d_wts_tc = nullptr;   // fp16 UMMA weight tiles, hi then lo halves (hr_render_wg.cuh)
+  std::vector<uint8_t> h_wts_tc; // host copy of [TcConst | hi tiles | lo tiles]; TcConst is passed by value at launch
+  void* d_ring = nullptr;        // work-item rings of the render kernel (one per warpgroup)
+  unsigned long long* d_counters = nullptr;   // [0] tile counter, [1] items evaluated, [2] secondary rays traced
+  bool split_ok = false;         // fp32 model representable as fp16 hi + lo without overflow (enables the tcgen05 fp32 path)
   float* d_env = nullptr;
   size_t env_cap = 0;
   int num_sms = 148;
@@ -35,7 +37,7 @@ struct hashrender {
   // staging for render_frame_host
   void* stage[16] = {nullptr};
   size_t stage_cap[16] = {0};
-  int force_path = 0;            // 0 auto, 1 ffma, 2 tc  (env HASHRENDER_PATH, for A/B tests)
+  int force_path = 0;            // 0 auto, 1 ffma  (env HASHRENDER_PATH=ffma, for A/B tests)
 };
 
 namespace {
@@ -113,14 +115,29 @@ int check_dirset(hashrender* h, const hr_dirset* d, const char* name, bool need_
   return HR_OK;
 }
 
-bool use_tc(const hashrender* h) {
-#ifdef HR_NO_TC
-  return false;
-#else
-  if (h->force_path == 1) return false;
-  if (h->force_path == 2) return h->d_wts_tc != nullptr;
-  return h->cfg.mlp_dtype == HR_F16 && h->d_wts_tc != nullptr;
-#endif
+// 0 = fp32 FFMA kernels, 1 = tcgen05 with fp16 activations, 2 = tcgen05 in hi/lo split precision (fp32 models)
+int render_path(const hashrender* h) {
+  if (h->force_path == 1 || !h->d_wts_tc) return 0;
+  if (h->cfg.mlp_dtype == HR_F16) return 1;
+  return h->split_ok ? 2 : 0;
+}
+
+// Upper bound of every hidden activation of an MLP whose inputs are bounded by in_max: the split-precision path holds
+// activations as fp16 hi + lo, so they must stay far below 65504.
+float mlp_bound(const float* w, int din, int H, float in_max) {
+  const float* W1 = w; const float* b1 = W1 + H * din; const float* W2 = b1 + H; const float* b2 = W2 + H * H;
+  float B1 = 0.f, B2 = 0.f;
+  for (int j = 0; j < H; ++j) {
+    float s = fabsf(b1[j]);
+    for (int k = 0; k < din; ++k) s += fabsf(W1[j * din + k]) * in_max;
+    B1 = fmaxf(B1, s);
+  }
+  for (int j = 0; j < H; ++j) {
+    float s = fabsf(b2[j]);
+    for (int k = 0; k < H; ++k) s += fabsf(W2[j * H + k]) * B1;
+    B2 = fmaxf(B2, s);
+  }
+  return fmaxf(B1, B2);
 }
 
 }  // namespace
@@ -150,7 +167,7 @@ int hashrender_create(const hr_config* cfg, const float* tables, const float* br
   HR_CUDA(h, cudaGetDevice(&dev));
   HR_CUDA(h, cudaDeviceGetAttribute(&h->num_sms, cudaDevAttrMultiProcessorCount, dev));
   const char* fp = getenv("HASHRENDER_PATH");
-  if (fp) h->force_path = !strcmp(fp, "ffma") ? 1 : (!strcmp(fp, "tc") ? 2 : 0);
+  if (fp) h->force_path = !strcmp(fp, "ffma") ? 1 : 0;
 
   // grid parameters
   GridP& g = h->grid;
@@ -187,15 +204,24 @@ int hashrender_create(const hr_config* cfg, const float* tables, const float* br
   prepare_weights_ffma(*cfg, brdf_w, irt_w, w);
   HR_CUDA(h, cudaMalloc(&h->d_wts, w.size() * sizeof(float)));
   HR_CUDA(h, cudaMemcpy(h->d_wts, w.data(), w.size() * sizeof(float), cudaMemcpyHostToDevice));
-#ifndef HR_NO_TC
-  if (cfg->mlp_dtype == HR_F16 || h->force_path == 2) {
-    tc::prepare_weights(*cfg, brdf_w, irt_w, h->h_wts_tc);
-    const size_t tb = h->h_wts_tc.size() - sizeof(tc::TcConst);
+  {
+    size_t cb = 0, tb = 0;
+    wg::prepare_weights_blob(*cfg, brdf_w, irt_w, h->h_wts_tc, &cb, &tb);
     HR_CUDA(h, cudaMalloc(&h->d_wts_tc, tb));
-    HR_CUDA(h, cudaMemcpy(h->d_wts_tc, h->h_wts_tc.data() + sizeof(tc::TcConst), tb, cudaMemcpyHostToDevice));
+    HR_CUDA(h, cudaMemcpy(h->d_wts_tc, h->h_wts_tc.data() + cb, tb, cudaMemcpyHostToDevice));
     HR_CUDA(h, tc::set_attributes());
+    HR_CUDA(h, cudaMalloc(&h->d_ring, wg::ring_bytes(h->num_sms)));
+    HR_CUDA(h, cudaMalloc(&h->d_counters, 4 * sizeof(unsigned long long)));
+    HR_CUDA(h, cudaMemset(h->d_counters, 0, 4 * sizeof(unsigned long long)));
+    // fp32 model on the fp16 tensor cores: every value is carried as fp16 hi + lo, so tables, weights and hidden
+    // activations must be finite and well inside the fp16 range
+    float tmax = 0.f;
+    for (size_t i = 0; i < n; ++i) tmax = fmaxf(tmax, fabsf(tables[i]));
+    const int D = cfg->L * cfg->F;
+    const float fb = fmaxf(tmax, 1.f);
+    const float bound = fmaxf(mlp_bound(brdf_w, D, kH, fb), mlp_bound(irt_w, D + 3, kH, fb));
+    h->split_ok = tmax < 1024.f && bound < 16384.f;      // NaN fails both comparisons
   }
-#endif
   ShadeP& s = h->shade;
   s.near_t = cfg->near_t; s.far_t = cfg->far_t; s.rough_min = cfg->rough_min; s.f0 = cfg->fresnel_f0;
   s.vis_mode = cfg->vis_mode; s.brdf_model = cfg->brdf_model;
@@ -215,6 +241,7 @@ int hashrender_destroy(hashrender_t* h) {
   if (!h) return HR_ERR_INVALID_ARG;
   cudaDeviceSynchronize();
   cudaFree(h->d_tables); cudaFree(h->d_wts); cudaFree(h->d_wts_tc); cudaFree(h->d_env);
+  cudaFree(h->d_ring); cudaFree(h->d_counters);
   for (int i = 0; i < 16; ++i) cudaFree(h->stage[i]);
   delete h;
   return HR_OK;
@@ -269,15 +296,13 @@ int hashrender_trace(hashrender_t* h, const float* x, const float* feat, uint64_
   if (xsec && !x) return fail(h, HR_ERR_INVALID_ARG, "trace: xsec needs x");
   if (N > h->cfg.max_points) return fail(h, HR_ERR_INVALID_ARG, "trace: N exceeds max_points");
   const DirsetP d = to_dev(*ds);
-#ifndef HR_NO_TC
-  if (use_tc(h) && !feat) {
+  if (render_path(h) == 1 && !feat) {
     h->last_path = "tcgen05-f16";
     HR_CUDA(h, tc::launch_trace(h->grid, h->shade, *reinterpret_cast<const tc::TcConst*>(h->h_wts_tc.data()), h->d_wts_tc, x, N, d, vis,
                                 zv, t, xsec, h->num_sms, (cudaStream_t)stream));
     h->launches++;
     return HR_OK;
   }
-#endif
   h->last_path = "ffma32";
   const int grid = grid_for(h, N, NT_FFMA, 1);
   const size_t smem = ffma_smem_bytes(NT_FFMA, false);
@@ -308,7 +333,7 @@ static int check_frame(hashrender* h, const hr_frame* f, const float* rgb) {
   if (f->N == 0) return HR_OK;
   if (!f->x || !f->wo || !rgb) return fail(h, HR_ERR_INVALID_ARG, "render_frame: NULL x / wo / rgb");
   if (f->N > h->cfg.max_points) return fail(h, HR_ERR_INVALID_ARG, "render_frame: N exceeds max_points");
-  if (!(f->flags & (HR_DIRECT | HR_INDIRECT)) || (f->flags & ~7u)) return fail(h, HR_ERR_INVALID_ARG, "render_frame: bad flags");
+  if (!(f->flags & (HR_DIRECT | HR_INDIRECT)) || (f->flags & ~15u)) return fail(h, HR_ERR_INVALID_ARG, "render_frame: bad flags");
   bool need_env = false;
   if (f->flags & HR_DIRECT) {
     if (int e = check_dirset(h, &f->direct, "render_frame.direct", true)) return e;
@@ -333,15 +358,18 @@ int hashrender_render_frame(hashrender_t* h, const hr_frame* f, float* rgb, void
   fr.d = to_dev(f->direct); fr.s = to_dev(f->secondary); fr.t = to_dev(f->tertiary);
   if (!(f->flags & HR_DIRECT)) fr.d.S = 0;
   if (!(f->flags & HR_INDIRECT)) { fr.s.S = 0; fr.t.S = 0; }
-#ifndef HR_NO_TC
-  if (use_tc(h) && tc::frame_supported(fr)) {
-    h->last_path = "tcgen05-f16";
-    HR_CUDA(h, tc::launch_render(h->grid, h->env, h->shade, *reinterpret_cast<const tc::TcConst*>(h->h_wts_tc.data()), h->d_wts_tc, fr,
-                                 rgb, h->num_sms, (cudaStream_t)stream));
+  const int path = render_path(h);
+  if (path && wg::frame_ok(fr)) {
+    h->last_path = path == 1 ? "tcgen05-f16" : "tcgen05-f16x3";
+    if (path == 1)
+      HR_CUDA(h, wg::launch_p0(h->grid.f16, h->grid, h->env, h->shade, h->h_wts_tc.data(), h->d_wts_tc, h->d_wts, fr, rgb, h->d_ring, h->d_counters,
+                               h->num_sms, (cudaStream_t)stream));
+    else
+      HR_CUDA(h, wg::launch_p1(h->grid.f16, h->grid, h->env, h->shade, h->h_wts_tc.data(), h->d_wts_tc, h->d_wts, fr, rgb, h->d_ring, h->d_counters,
+                               h->num_sms, (cudaStream_t)stream));
     h->launches++;
     return HR_OK;
   }
-#endif
   h->last_path = "ffma32";
   const int grid = grid_for(h, f->N, NT_FFMA, 1);
   const size_t smem = ffma_smem_bytes(NT_FFMA, true);
@@ -407,6 +435,17 @@ int hashrender_render_frame_host(hashrender_t* h, const hr_frame* f, float* rgb,
   HR_CUDA(h, cudaStreamSynchronize(st));
   if (h2d_bytes) *h2d_bytes = up;
   if (d2h_bytes) *d2h_bytes = f->N * 12;
+  return HR_OK;
+}
+
+int hashrender_stats(hashrender_t* h, uint64_t* rays_traced, uint64_t* rays_evaluated, int reset) {
+  if (!h) return HR_ERR_INVALID_ARG;
+  unsigned long long c[4] = {0, 0, 0, 0};
+  HR_CUDA(h, cudaDeviceSynchronize());
+  HR_CUDA(h, cudaMemcpy(c, h->d_counters, sizeof(c), cudaMemcpyDeviceToHost));
+  if (rays_traced) *rays_traced = c[2];
+  if (rays_evaluated) *rays_evaluated = c[1];
+  if (reset) HR_CUDA(h, cudaMemset(h->d_counters, 0, sizeof(c)));
   return HR_OK;
 }
 

@@ -189,7 +189,7 @@ __global__ void __launch_bounds__(NT, 1) k_trace_ffma(GridP g, ShadeP sp, const 
 }
 
 // shade: Eq. 1 with Eq. 2 per direction on one set (a9-a11)
-__global__ void __launch_bounds__(256) k_shade(EnvP env, ShadeP sp, const float* __restrict__ brdf, const float* __restrict__ wo,
+static __global__ void __launch_bounds__(256) k_shade(EnvP env, ShadeP sp, const float* __restrict__ brdf, const float* __restrict__ wo,
                                                unsigned long long N, DirsetP ds, const float* __restrict__ vis,
                                                const float* __restrict__ Lind, uint32_t terms, float* __restrict__ rgb) {
   for (unsigned long long i = blockIdx.x * (unsigned long long)blockDim.x + threadIdx.x; i < N;

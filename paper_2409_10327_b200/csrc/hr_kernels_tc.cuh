@@ -547,196 +547,6 @@ __device__ __forceinline__ void teardown(const Ctx& c) {
 }
 
 // ---------------------------------------------------------------------------------------------------- kernels
-struct SecRay { float v, wx, wy, wz, pdf, x, y, z; };   // one secondary direction of a pixel: visibility, direction, pdf, hit x'
-
-// render_frame (a1-a11), tensor-core path.  TSHARED: the tertiary set is one shared set (point_stride == 0).
-// LPI: levels of the next secondary point's gathers carried per tertiary iteration (0 = none; 2 needs S_2 == 8).
-template <bool F16, bool TSHARED, int LPI>
-__global__ void __launch_bounds__(kThreads, kCtasPerSm) k_render_tc(const __grid_constant__ GridP g, EnvP env, ShadeP sp,
-                                                                    const __grid_constant__ TcConst cw, const uint8_t* __restrict__ wtiles,
-                                                                    FrameP fr, float* __restrict__ rgb) {
-  extern __shared__ uint8_t smem_raw[];
-  const Smem s = carve(smem_raw);
-  Ctx c;
-  setup(s, wtiles, c);
-  const bool indirect = (fr.flags & 4u) && fr.s.S && fr.t.S;
-  constexpr bool tshared = TSHARED;
-  if (indirect && tshared) {                    // shared tertiary set: Q_k = W1w . w'_k; per k: radiance, pdf, direction
-    for (int e = threadIdx.x; e < (int)fr.t.S * kH; e += kThreads) {
-      const int k = e / kH, q = e % kH;
-      const float* dp = fr.t.dir + 3 * k;
-      const float qv = cw.w1w[0][q] * __ldg(dp) + cw.w1w[1][q] * __ldg(dp + 1) + cw.w1w[2][q] * __ldg(dp + 2);
-      reinterpret_cast<__half*>(s.Qt)[e] = __float2half_rn(qv);    // Qh[k][q], fp16
-    }
-    for (int k = threadIdx.x; k < (int)fr.t.S; k += kThreads) {
-      const float* dp = fr.t.dir + 3 * k;
-      const float tx = __ldg(dp), ty = __ldg(dp + 1), tz = __ldg(dp + 2);
-      float3 L;
-      if (fr.t.Lin) L = make_float3(__ldg(fr.t.Lin + 3 * k), __ldg(fr.t.Lin + 3 * k + 1), __ldg(fr.t.Lin + 3 * k + 2));
-      else L = env_lookup(env, tx, ty, tz);
-      float* o = s.Lt + 8 * k;
-      o[0] = L.x; o[1] = L.y; o[2] = L.z; o[3] = __ldg(fr.t.pdf + k); o[4] = tx; o[5] = ty; o[6] = tz; o[7] = 0.f;
-    }
-  }
-  __syncthreads();
-  float* Ps = s.Ps + threadIdx.x;
-  const unsigned long long ntiles = (fr.N + kThreads - 1) / kThreads;
-  const int jend = indirect ? (int)fr.s.S : 0;
-  // levels of the NEXT secondary point gathered per tertiary iteration (0 = the tertiary loop cannot carry them)
-  constexpr int lpi = LPI;
-
-  for (unsigned long long tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
-    const unsigned long long i_raw = tile * kThreads + threadIdx.x;
-    const bool valid = i_raw < fr.N;
-    const unsigned long long i = valid ? i_raw : fr.N - 1;        // idle rows shadow the last point (uniform control flow)
-    const bool live = valid && !(fr.mask && !fr.mask[i]);
-    const float px = __ldg(fr.x + 3 * i), py = __ldg(fr.x + 3 * i + 1), pz = __ldg(fr.x + 3 * i + 2);
-    const float ox = __ldg(fr.wo + 3 * i), oy = __ldg(fr.wo + 3 * i + 1), oz = __ldg(fr.wo + 3 * i + 2);
-    float b[7];                                                     // primary BRDF
-    float r = 0.f, gch = 0.f, bch = 0.f;                            // direct term of Eq. 1
-
-    // ---- primary point: a1-a5, then the direct set -------------------------------------------------------------
-    {
-      encode_split_to_A<F16>(g, c, px, py, pz);
-      issue_layer(c, 0, kColA, 0, 2, 0, 2, true);                   // P = W1f f + b1, split-precision f
-      wait_layer(c, 0);
-      float P[kH];
-      load_D(c, P);
-      if (fr.brdf) {
-#pragma unroll
-        for (int k = 0; k < 7; ++k) b[k] = __ldg(fr.brdf + i * 7 + k);
-      } else {
-        brdf_precise_from_A(c, cw, sp, b);                          // A0[0..31] still holds f (hi | lo)
-      }
-      if (jend > 0) {
-#pragma unroll
-        for (int k = 0; k < kH; ++k) Ps[k * kThreads] = P[k];
-      }
-      if ((fr.flags & 1u) && fr.d.S) {                              // direct term of Eq. 1, two queries in flight
-        const uint32_t S = fr.d.S;
-        const bool shadow = fr.flags & 2u;
-        float ar = 0.f, ag = 0.f, ab = 0.f;
-        const float* dp = dir_of(fr.d, i, 0);
-        float d0x = __ldg(dp), d0y = __ldg(dp + 1), d0z = __ldg(dp + 2), d0p = pdf_of(fr.d, i, 0);
-        const uint32_t s1 = S > 1 ? 1u : 0u;
-        dp = dir_of(fr.d, i, s1);
-        float d1x = __ldg(dp), d1y = __ldg(dp + 1), d1z = __ldg(dp + 2), d1p = pdf_of(fr.d, i, s1);
-        if (shadow) { h1_from_regs(c, cw, 0, P, d0x, d0y, d0z); issue_layer(c, 0, kColA, 2, 4, 0, 3); }
-        for (uint32_t k = 0; k < S; ++k) {
-          const int bf = k & 1;
-          const uint32_t s2 = k + 2 < S ? k + 2 : S - 1;            // prefetch direction k + 2
-          dp = dir_of(fr.d, i, s2);
-          const float d2x = __ldg(dp), d2y = __ldg(dp + 1), d2z = __ldg(dp + 2), d2p = pdf_of(fr.d, i, s2);
-          float vd = 1.f;
-          if (shadow && k + 1 < S) { h1_from_regs(c, cw, bf ^ 1, P, d1x, d1y, d1z); issue_layer(c, bf ^ 1, kColA + kBufStride * (bf ^ 1), 2, 4, 0, 3); }
-          const float3 gg = brdf_cos_over_pdf(sp, b, d0x, d0y, d0z, ox, oy, oz, d0p);
-          const float3 L = incoming(env, fr.d, i, k, d0x, d0y, d0z);
-          if (shadow) {
-            wait_layer(c, bf);
-            vd = vis_of(sp, irt_epilogue_fast(c, cw, bf));
-          }
-          ar = fmaf(vd * L.x, gg.x, ar); ag = fmaf(vd * L.y, gg.y, ag); ab = fmaf(vd * L.z, gg.z, ab);
-          d0x = d1x; d0y = d1y; d0z = d1z; d0p = d1p;
-          d1x = d2x; d1y = d2y; d1z = d2z; d1p = d2p;
-        }
-        const float inv = 1.f / (float)S;
-        r = ar * inv; gch = ag * inv; bch = ab * inv;
-      }
-    }
-
-    // ---- secondary set: (1 - V) L'_o term of Eq. 2 ---------------------------------------------------------------
-    if (jend > 0) {
-      float ir = 0.f, ig = 0.f, ib = 0.f;
-      // a6/a7 along secondary direction j, split precision (buffer pair 0)
-      auto trace_secondary = [&](int j) -> SecRay {
-        SecRay q;
-        const float* dp = dir_of(fr.s, i, j);
-        q.wx = __ldg(dp); q.wy = __ldg(dp + 1); q.wz = __ldg(dp + 2);
-        q.pdf = pdf_of(fr.s, i, j);
-        h1_from_smem_split(c, cw, Ps, q.wx, q.wy, q.wz);
-        issue_layer(c, 0, kColA, 2, 4, -1, 0, true);
-        wait_layer(c, 0);
-        float zv, zt, t;
-        irt_epilogue_precise(c, cw, 0, zv, zt);
-        irt_maps(sp, zv, zt, q.v, t);
-        q.x = sec_hit(px, t, q.wx); q.y = sec_hit(py, t, q.wy); q.z = sec_hit(pz, t, q.wz);
-        return q;
-      };
-      SecRay nxt = trace_secondary(0);
-      encode_next_plain<F16>(g, c, nxt.x, nxt.y, nxt.z);
-      for (int j = 0; j < jend; ++j) {
-        const SecRay cur = nxt;
-        // a1-a5 at x'_j: its features wait in the staging columns
-        issue_layer(c, 0, kColNext, 0, 2, 0, 2);
-        wait_layer(c, 0);
-        float P2[TSHARED ? 1 : kH];
-        uint32_t P2h[TSHARED ? kH / 2 : 1];
-        if constexpr (TSHARED) load_D_h2(c, P2h); else load_D(c, P2);
-        float bb[7];
-        brdf_from_A(c, cw, sp, kColNext, bb);
-        const bool have_next = j + 1 < jend;
-        if (have_next) nxt = trace_secondary(j + 1);                // overwrites the staging columns: they are consumed
-        // a8: Eq. 1 at x'_j over the tertiary set (w_o' = -w_j), two queries in flight; each iteration also carries
-        // `lpi` levels of the gathers of x'_{j+1}
-        const uint32_t S2 = fr.t.S;
-        const unsigned long long trow = tshared ? 0ull : i * fr.s.S + j;
-        float lr = 0.f, lg = 0.f, lb = 0.f;
-        auto h1t = [&](uint32_t k, int bf) {
-          if constexpr (TSHARED) h1_from_h2_shared(c, bf, P2h, reinterpret_cast<const uint32_t*>(s.Qt) + k * (kH / 2));
-          else { const float* tp = dir_of(fr.t, trow, k); h1_from_regs(c, cw, bf, P2, __ldg(tp), __ldg(tp + 1), __ldg(tp + 2)); }
-        };
-        h1t(0, 0);
-        issue_layer(c, 0, kColA, 2, 4, 0, 3);
-        const uint32_t tN = colNext(c);
-        for (uint32_t k = 0; k < S2; ++k) {
-          const int bf = k & 1;
-          LevelTaps<F16> taps[LPI > 0 ? LPI : 1];
-          const bool carry = have_next && LPI > 0;
-          if (carry) {
-#pragma unroll
-            for (int q = 0; q < LPI; ++q) {
-              const int l = (int)k * LPI + q;
-              if (l < (int)g.L) gather_level<F16>(g, l, nxt.x, nxt.y, nxt.z, taps[q]);
-            }
-          }
-          if (k + 1 < S2) { h1t(k + 1, bf ^ 1); issue_layer(c, bf ^ 1, kColA + kBufStride * (bf ^ 1), 2, 4, 0, 3); }
-          float tx, ty, tz, tpdf;                                   // shading factors first: they do not need the MMA
-          float3 L;
-          if (tshared) {
-            const float4 a = reinterpret_cast<const float4*>(s.Lt)[2 * k], d = reinterpret_cast<const float4*>(s.Lt)[2 * k + 1];
-            L = make_float3(a.x, a.y, a.z); tpdf = a.w; tx = d.x; ty = d.y; tz = d.z;
-          } else {
-            const float* tp = dir_of(fr.t, trow, k);
-            tx = __ldg(tp); ty = __ldg(tp + 1); tz = __ldg(tp + 2); tpdf = pdf_of(fr.t, trow, k);
-            L = incoming(env, fr.t, trow, k, tx, ty, tz);
-          }
-          const float3 gg = brdf_cos_over_pdf(sp, bb, tx, ty, tz, -cur.wx, -cur.wy, -cur.wz, tpdf);
-          wait_layer(c, bf);
-          const float v2 = vis_of(sp, irt_epilogue_fast(c, cw, bf));
-          lr = fmaf(v2 * L.x, gg.x, lr); lg = fmaf(v2 * L.y, gg.y, lg); lb = fmaf(v2 * L.z, gg.z, lb);
-          if (carry) {
-#pragma unroll
-            for (int q = 0; q < LPI; ++q) {
-              const int l = (int)k * LPI + q;
-              tmem_st1(tN + l, l < (int)g.L ? lerp_level(taps[q]) : 0u);
-            }
-          }
-        }
-        if (have_next && LPI == 0) encode_next_plain<F16>(g, c, nxt.x, nxt.y, nxt.z);
-        const float3 gg = brdf_cos_over_pdf(sp, b, cur.wx, cur.wy, cur.wz, ox, oy, oz, cur.pdf);
-        const float m = (1.f - cur.v) / (float)S2;
-        ir = fmaf(m * lr, gg.x, ir); ig = fmaf(m * lg, gg.y, ig); ib = fmaf(m * lb, gg.z, ib);
-      }
-      const float inv = 1.f / (float)jend;
-      r = fmaf(ir, inv, r); gch = fmaf(ig, inv, gch); bch = fmaf(ib, inv, bch);
-    }
-    if (valid) {
-      rgb[3 * i] = live ? r : 0.f; rgb[3 * i + 1] = live ? gch : 0.f; rgb[3 * i + 2] = live ? bch : 0.f;
-    }
-  }
-  teardown(c);
-}
-
 // trace with the encode fused (a1-a4, a6, a7), tensor-core path (t is an output: precise epilogue).
 template <bool F16>
 __global__ void __launch_bounds__(kThreads, kCtasPerSm) k_trace_tc(const __grid_constant__ GridP g, ShadeP sp, const __grid_constant__ TcConst cw,
@@ -821,11 +631,6 @@ inline void prepare_weights(const hr_config& cfg, const float* bw, const float* 
 
 inline cudaError_t set_attributes() {
   cudaError_t e;
-#define HR_TC_ATTR(K) if ((e = cudaFuncSetAttribute(K, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes))) return e
-  HR_TC_ATTR((k_render_tc<true, true, 2>)); HR_TC_ATTR((k_render_tc<true, true, 0>));
-  HR_TC_ATTR((k_render_tc<true, false, 2>)); HR_TC_ATTR((k_render_tc<true, false, 0>));
-  HR_TC_ATTR((k_render_tc<false, true, 0>)); HR_TC_ATTR((k_render_tc<false, false, 0>));
-#undef HR_TC_ATTR
   if ((e = cudaFuncSetAttribute(k_trace_tc<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes))) return e;
   if ((e = cudaFuncSetAttribute(k_trace_tc<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes))) return e;
   return cudaSuccess;
@@ -837,23 +642,6 @@ inline int grid_size(unsigned long long N, int num_sms) {
   const unsigned long long tiles = (N + kThreads - 1) / kThreads;
   const unsigned long long cap = (unsigned long long)num_sms * kCtasPerSm;
   return (int)(tiles < cap ? tiles : cap);
-}
-
-// h_blob: host copy of the prepared blob (for the by-value TcConst); d_tiles: device pointer to the tiles
-inline cudaError_t launch_render(const GridP& g, const EnvP& env, const ShadeP& sp, const TcConst& cw, const uint8_t* d_tiles,
-                                 const FrameP& fr, float* rgb, int num_sms, cudaStream_t st) {
-  const int grid = grid_size(fr.N, num_sms);
-  const bool tsh = fr.t.stride == 0;
-  const bool carry = (fr.flags & 4u) && fr.t.S == 8;          // 16 levels / 8 tertiary iterations = 2 levels each
-#define HR_TC_LAUNCH(K) K<<<grid, kThreads, kSmemBytes, st>>>(g, env, sp, cw, d_tiles, fr, rgb)
-  if (g.f16) {
-    if (tsh) { if (carry) HR_TC_LAUNCH((k_render_tc<true, true, 2>)); else HR_TC_LAUNCH((k_render_tc<true, true, 0>)); }
-    else { if (carry) HR_TC_LAUNCH((k_render_tc<true, false, 2>)); else HR_TC_LAUNCH((k_render_tc<true, false, 0>)); }
-  } else {
-    if (tsh) HR_TC_LAUNCH((k_render_tc<false, true, 0>)); else HR_TC_LAUNCH((k_render_tc<false, false, 0>));
-  }
-#undef HR_TC_LAUNCH
-  return cudaGetLastError();
 }
 
 inline cudaError_t launch_trace(const GridP& g, const ShadeP& sp, const TcConst& cw, const uint8_t* d_tiles, const float* x,

@@ -1,0 +1,705 @@
+// hr_render_wg.cuh -- the fused render_frame kernel (steps a1-a11) on tcgen05 / TMEM, warpgroup-multiplexed.
+//
+// One persistent CTA per SM holds G independent 128-thread warpgroups (WG).  A WG is the 128 TMEM lanes of its own
+// TMEM column range: thread r owns row r of every 128 x N tcgen05.mma the WG issues, so an MLP activation never
+// crosses threads.  The G warpgroups share the UMMA weight tiles in shared memory, are scheduled independently
+// (named barriers + one mbarrier each) and hide each other's MMA / gather / barrier latencies: with G = 4 every SM
+// sub-partition has four warps to pick from instead of two.
+//
+// Per 128-pixel tile a WG runs
+//   A   primary point: f = H(x) (fp32, hi/lo split), P = W1f f + b1, n,a,r = B(f)                     (a1-a5)
+//   A2  direct set: v = I(f, w_s) per direction, Eq. 1 with the env map                                (a6, a9-a11)
+//   B   secondary set: (v, t) = I(f, w_j) in split precision, x' = x + t w_j, and the weight
+//       g_j = (1 - v_j) f_r (n.w_j)^+ / (p_j S_i S_2) of L'_o in Eq. 2.  Every ray with a non-zero weight
+//       becomes a 48-byte work item in the WG's ring (only occluded rays are traced further;
+//       HR_DENSE keeps every ray)                                                                      (a6, a7)
+//   C   items are drained 128 at a time, one per thread, whoever produced them: f' = H(x'), P' = W1f f' + b1,
+//       n',a',r' = B(f'), v'_k = I(f', w'_k) over the tertiary set, L'_o (Eq. 1 with w_o' = -w_j); the weighted
+//       radiance is added to the owner pixel's accumulator in shared memory                           (a8)
+//   D   rgb = direct + indirect                                                                        (a11)
+//
+// PREC = 0: fp16 activations (BASELINE.json configs[3]); the primary point and the secondary trace, whose t moves
+//           x', run in split precision (hi + lo fp16, SURVEY 8(c) conditioning note).
+// PREC = 1: fp32-grade arithmetic on the fp16 tensor cores for mlp_dtype == HR_F32: every activation AND every
+//           weight is split x = hi + lo (both fp16), each layer is three MMA passes hi*Whi + lo*Whi + hi*Wlo with
+//           fp32 accumulation (the dropped lo*lo term is 2^-22 relative), epilogues and shading in fp32.
+#pragma once
+#include <cstring>
+
+#include "hr_kernels_ffma.cuh"
+#include "hr_kernels_tc.cuh"
+
+namespace hr {
+namespace wg {
+using namespace hr::tc;
+
+constexpr int kRows = 128;                    // rows (threads) per warpgroup
+constexpr int kRing = 1024;                   // work items per WG ring (power of two, >= 127 + kChunkJ * 128)
+constexpr int kChunkJ = 4;                    // secondary directions traced between two drains
+constexpr int kMaxG = 4;
+constexpr int kMaxS2 = tc::kMaxS2;              // shared tertiary set staged in shared memory
+constexpr int kHiTileBytes = kNumTiles * kTileBytes + kTile3Bytes;       // 34 KB: I.W1f, B.W1, I.W2, B.W2, B.W3
+
+struct __align__(16) Item {                   // one secondary hit waiting for its L'_o
+  float x, y, z, wx;                          // x' and the direction it was reached along (w_o' = -w)
+  float wy, wz, gr, gg;                       // weight of L'_o in the owner's pixel, per channel
+  float gb; uint32_t owner; uint32_t pad0, pad1;   // owner = row | j << 8
+};
+static_assert(sizeof(Item) == 48, "Item is three 16-byte words");
+
+template <int PREC, int G> struct Cols {
+  static_assert(G >= 1 && G <= kMaxG, "1..4 warpgroups");
+  static_assert(PREC == 0 || G <= 3, "split precision needs 144 TMEM columns per warpgroup");
+  static constexpr uint32_t stride = G == 4 ? 128u : (G == 3 ? 168u : (G == 2 ? 256u : 512u));
+  // A = columns 0..63 (fp16 pairs; hi | lo for the split layers), D = 64 fp32 accumulator columns, and the constant bias
+  // K-step of A, [1, 1, 0 .. 0].  With 128 columns per warpgroup (G = 4) the bias step shares columns 32..39 with the lo
+  // half of A: K = 64 split layers then add their bias in the fp32 epilogue and rewrite the step afterwards.
+  static constexpr bool bias64 = stride >= 144u;
+  static constexpr uint32_t one = bias64 ? 64u : 32u;
+  static constexpr uint32_t d = bias64 ? 80u : 64u;
+};
+
+struct WgCtx {
+  uint32_t tmem;      // TMEM address of the WG's column 0, lane 0
+  uint32_t lane;      // this warp's lane base << 16
+  uint32_t mbar;      // shared address of the WG's mbarrier
+  uint32_t phase;
+  uint32_t tile0;     // shared address of the weight tiles
+  uint32_t lo_off;    // byte offset of the lo tiles (PREC = 1)
+  int bar_id;         // named barrier of the WG
+  int t;              // thread index in the WG
+};
+
+__device__ __forceinline__ void tmem_st4(uint32_t taddr, const uint32_t (&r)[4]) {
+  asm volatile("tcgen05.st.sync.aligned.32x32b.x4.b32 [%0], {%1,%2,%3,%4};" ::"r"(taddr), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]) : "memory");
+}
+__device__ __forceinline__ void tmem_stN(uint32_t taddr, const uint32_t (&r)[4]) { tmem_st4(taddr, r); }
+__device__ __forceinline__ void tmem_stN(uint32_t taddr, const uint32_t (&r)[2]) {
+  asm volatile("tcgen05.st.sync.aligned.32x32b.x2.b32 [%0], {%1,%2};" ::"r"(taddr), "r"(r[0]), "r"(r[1]) : "memory");
+}
+__device__ __forceinline__ void wg_sync(const WgCtx& c) { asm volatile("bar.sync %0, 128;" ::"r"(c.bar_id) : "memory"); }
+
+// One 128 x N layer of the WG: D = A W^T (+ bias K-step).  A = `ksteps` K-steps of fp16 at column a_col; split_a: a lo
+// block follows the hi block; PREC = 1 adds the pass against the lo weights.  All threads must have stored their A rows.
+template <int PREC, int G>
+__device__ __forceinline__ void issue_layer(const WgCtx& c, uint32_t a_col, int tile, int ksteps, bool split_a, int bias_tile,
+                                            int bias_kstep, uint32_t idesc = kIdesc) {
+  wait_st();
+  fence_before();
+  wg_sync(c);
+  if (c.t == 0) {
+    fence_after();
+    const uint32_t d = c.tmem + Cols<PREC, G>::d;
+    const uint32_t a = c.tmem + a_col;
+    const uint64_t bd = make_bdesc(c.tile0 + tile * kTileBytes);
+    for (int k = 0; k < ksteps; ++k) mma_f16_ts(d, a + 8 * k, bd + 2 * k, idesc, k > 0);
+    if (split_a)
+      for (int k = 0; k < ksteps; ++k) mma_f16_ts(d, a + 8 * (ksteps + k), bd + 2 * k, idesc, 1u);
+    if (PREC == 1) {
+      const uint64_t bl = make_bdesc(c.tile0 + c.lo_off + tile * kTileBytes);
+      for (int k = 0; k < ksteps; ++k) mma_f16_ts(d, a + 8 * k, bl + 2 * k, idesc, 1u);
+    }
+    if (bias_tile >= 0)
+      mma_f16_ts(d, c.tmem + Cols<PREC, G>::one, make_bdesc(c.tile0 + bias_tile * kTileBytes) + 2 * bias_kstep, idesc, 1u);
+    mma_commit(c.mbar);
+  }
+}
+template <int PREC, int G>
+__device__ __forceinline__ void restore_one(const WgCtx& c) {
+  const uint32_t one[8] = {0x3C003C00u, 0u, 0u, 0u, 0u, 0u, 0u, 0u};
+  tmem_st8(c.tmem + c.lane + Cols<PREC, G>::one, one);
+}
+__device__ __forceinline__ void wait_layer(WgCtx& c) {
+  mbar_wait(c.mbar, c.phase);
+  c.phase ^= 1u;
+  fence_after();
+}
+
+// ---------------------------------------------------------------------------------------------------- row stages
+// fp32 pair -> hi fp16x2 word and the fp16x2 word of the residual
+__device__ __forceinline__ void split_pair(float a0, float a1, uint32_t& hi, uint32_t& lo) {
+  hi = pack_rn(a0, a1);
+  lo = pack_lo(hi, a0, a1);
+}
+
+// z_v = b3 + w3v . relu(D) with fp16x2 FMAs (b2 rode in the MMA); PREC = 0 direct / tertiary queries
+__device__ __forceinline__ float epi_fast(uint32_t tD, const TcConst& cw) {
+  __half2 acc[4];
+#pragma unroll
+  for (int q = 0; q < 4; ++q) acc[q] = __float2half2_rn(0.f);
+#pragma unroll
+  for (int h = 0; h < 2; ++h) {
+    uint32_t r[32];
+    tmem_ld32(tD + 32 * h, r);
+    wait_ld();
+#pragma unroll
+    for (int k = 0; k < 16; ++k) {
+      const uint32_t p = pack_relu(__uint_as_float(r[2 * k]), __uint_as_float(r[2 * k + 1]));
+      const uint32_t w = cw.w3v_h2[16 * h + k];
+      acc[k & 3] = __hfma2(*reinterpret_cast<const __half2*>(&p), *reinterpret_cast<const __half2*>(&w), acc[k & 3]);
+    }
+  }
+  float z = cw.b3[0];
+#pragma unroll
+  for (int q = 0; q < 4; ++q) { const float2 f = __half22float2(acc[q]); z += f.x + f.y; }
+  return z;
+}
+// fp32 epilogues (b2 rode in the MMA as a hi/lo bias K-step unless ADD_B2)
+template <bool ADD_B2>
+__device__ __forceinline__ void epi_precise(uint32_t tD, const TcConst& cw, float& zv, float& zt) {
+  float z0[4] = {cw.b3[0], 0.f, 0.f, 0.f}, z1[4] = {cw.b3[1], 0.f, 0.f, 0.f};
+#pragma unroll
+  for (int h = 0; h < 2; ++h) {
+    uint32_t r[32];
+    tmem_ld32(tD + 32 * h, r);
+    wait_ld();
+#pragma unroll
+    for (int k = 0; k < 32; ++k) {
+      const float a = fmaxf(ADD_B2 ? __uint_as_float(r[k]) + cw.b2[32 * h + k] : __uint_as_float(r[k]), 0.f);
+      z0[k & 3] = fmaf(a, cw.w3[0][32 * h + k], z0[k & 3]);
+      z1[k & 3] = fmaf(a, cw.w3[1][32 * h + k], z1[k & 3]);
+    }
+  }
+  zv = (z0[0] + z0[1]) + (z0[2] + z0[3]);
+  zt = (z1[0] + z1[1]) + (z1[2] + z1[3]);
+}
+__device__ __forceinline__ float epi_precise_v(uint32_t tD, const TcConst& cw) {
+  float z0[4] = {cw.b3[0], 0.f, 0.f, 0.f};
+#pragma unroll
+  for (int h = 0; h < 2; ++h) {
+    uint32_t r[32];
+    tmem_ld32(tD + 32 * h, r);
+    wait_ld();
+#pragma unroll
+    for (int k = 0; k < 32; ++k) z0[k & 3] = fmaf(fmaxf(__uint_as_float(r[k]), 0.f), cw.w3[0][32 * h + k], z0[k & 3]);
+  }
+  return (z0[0] + z0[1]) + (z0[2] + z0[3]);
+}
+
+// relu(D) -> A columns 0..31 (fp16) or 0..31 | 32..63 (hi | lo)
+template <bool SPLIT>
+__device__ __forceinline__ void hidden_to_A(uint32_t tD, uint32_t tA) {
+#pragma unroll
+  for (int h = 0; h < 2; ++h) {
+    uint32_t r[32];
+    tmem_ld32(tD + 32 * h, r);
+    wait_ld();
+    uint32_t p[16], q[16];
+#pragma unroll
+    for (int k = 0; k < 16; ++k) {
+      if (SPLIT) split_pair(fmaxf(__uint_as_float(r[2 * k]), 0.f), fmaxf(__uint_as_float(r[2 * k + 1]), 0.f), p[k], q[k]);
+      else p[k] = pack_relu(__uint_as_float(r[2 * k]), __uint_as_float(r[2 * k + 1]));
+    }
+    tmem_st16(tA + 16 * h, p);
+    if (SPLIT) tmem_st16(tA + 32 + 16 * h, q);
+  }
+}
+
+// h1 = relu(P + W1w . w) -> A; P(j) yields the layer-1 partial of hidden unit j
+template <bool SPLIT, typename PF>
+__device__ __forceinline__ void h1_dir(uint32_t tA, const TcConst& cw, PF P, float wx, float wy, float wz) {
+#pragma unroll
+  for (int h = 0; h < 2; ++h) {
+    uint32_t p[16], q[16];
+#pragma unroll
+    for (int k = 0; k < 16; ++k) {
+      const int j = 32 * h + 2 * k;
+      float a0 = fmaf(cw.w1w[0][j], wx, P(j));
+      a0 = fmaf(cw.w1w[1][j], wy, a0); a0 = fmaf(cw.w1w[2][j], wz, a0);
+      float a1 = fmaf(cw.w1w[0][j + 1], wx, P(j + 1));
+      a1 = fmaf(cw.w1w[1][j + 1], wy, a1); a1 = fmaf(cw.w1w[2][j + 1], wz, a1);
+      if (SPLIT) split_pair(fmaxf(a0, 0.f), fmaxf(a1, 0.f), p[k], q[k]);
+      else p[k] = pack_relu(a0, a1);
+    }
+    tmem_st16(tA + 16 * h, p);
+    if (SPLIT) tmem_st16(tA + 32 + 16 * h, q);
+  }
+}
+// shared tertiary set, PREC = 0: P and Q = W1w . w'_k both fp16 pairs, one fma.relu per pair
+__device__ __forceinline__ void h1_shared_h2(uint32_t tA, const uint32_t (&Ph)[kH / 2], const uint32_t* __restrict__ Qh) {
+#pragma unroll
+  for (int h = 0; h < 2; ++h) {
+    uint32_t p[16];
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+      const uint4 q = reinterpret_cast<const uint4*>(Qh)[4 * h + k];
+      const uint32_t qq[4] = {q.x, q.y, q.z, q.w};
+#pragma unroll
+      for (int e = 0; e < 4; ++e)
+        asm("fma.rn.relu.f16x2 %0, %1, %2, %3;" : "=r"(p[4 * k + e]) : "r"(Ph[16 * h + 4 * k + e]), "r"(0x3C003C00u), "r"(qq[e]));
+    }
+    tmem_st16(tA + 16 * h, p);
+  }
+}
+// shared tertiary set, PREC = 1: fp32 P (registers) + fp32 Q (shared memory), split
+__device__ __forceinline__ void h1_shared_split(uint32_t tA, const float (&P)[kH], const float* __restrict__ Q) {
+#pragma unroll
+  for (int h = 0; h < 2; ++h) {
+    uint32_t p[16], q[16];
+#pragma unroll
+    for (int k = 0; k < 8; ++k) {
+      const float4 v = reinterpret_cast<const float4*>(Q)[8 * h + k];
+      const int j = 32 * h + 4 * k;
+      split_pair(fmaxf(P[j] + v.x, 0.f), fmaxf(P[j + 1] + v.y, 0.f), p[2 * k], q[2 * k]);
+      split_pair(fmaxf(P[j + 2] + v.z, 0.f), fmaxf(P[j + 3] + v.w, 0.f), p[2 * k + 1], q[2 * k + 1]);
+    }
+    tmem_st16(tA + 16 * h, p);
+    tmem_st16(tA + 32 + 16 * h, q);
+  }
+}
+
+template <int N>
+__device__ __forceinline__ void load_D_f32(uint32_t tD, float (&P)[N]) {
+  static_assert(N == kH, "64 accumulator columns");
+#pragma unroll
+  for (int h = 0; h < 2; ++h) {
+    uint32_t r[32];
+    tmem_ld32(tD + 32 * h, r);
+    wait_ld();
+#pragma unroll
+    for (int k = 0; k < 32; ++k) P[32 * h + k] = __uint_as_float(r[k]);
+  }
+}
+__device__ __forceinline__ void load_D_h2(uint32_t tD, uint32_t (&Ph)[kH / 2]) {
+#pragma unroll
+  for (int h = 0; h < 2; ++h) {
+    uint32_t r[32];
+    tmem_ld32(tD + 32 * h, r);
+    wait_ld();
+#pragma unroll
+    for (int k = 0; k < 16; ++k) Ph[16 * h + k] = pack_rn(__uint_as_float(r[2 * k]), __uint_as_float(r[2 * k + 1]));
+  }
+}
+
+// f = H(x) in fp32 -> A columns 0..15 (hi) | 16..31 (lo)
+template <bool F16TAB, int LIF>
+__device__ __forceinline__ void encode_split_to(uint32_t tA, const GridP& g, float x, float y, float z, float* scr = nullptr) {
+#pragma unroll 1
+  for (int l0 = 0; l0 < kMaxL; l0 += LIF) {               // LIF levels (8 LIF gathers) in flight
+    uint32_t hi[LIF], lo[LIF];
+#pragma unroll
+    for (int q = 0; q < LIF; ++q) {
+      hi[q] = 0u; lo[q] = 0u;
+      if (l0 + q < (int)g.L) {
+        const float2 v = encode_level<F16TAB>(g, l0 + q, x, y, z, nullptr, nullptr);
+        split_pair(v.x, v.y, hi[q], lo[q]);
+        if (scr) { scr[(2 * (l0 + q)) * kRows] = v.x; scr[(2 * (l0 + q) + 1) * kRows] = v.y; }
+      } else if (scr) {
+        scr[(2 * (l0 + q)) * kRows] = 0.f; scr[(2 * (l0 + q) + 1) * kRows] = 0.f;
+      }
+    }
+    tmem_stN(tA + l0, hi);
+    tmem_stN(tA + 16 + l0, lo);
+  }
+}
+// fast encode of a secondary point (already clamped) -> A columns 0..15, fp16 pairs
+template <bool F16TAB, int LIF>
+__device__ __forceinline__ void encode_fast_to(uint32_t tA, const GridP& g, float x, float y, float z) {
+#pragma unroll 1
+  for (int l0 = 0; l0 < kMaxL; l0 += LIF) {               // LIF levels (8 LIF gathers) in flight
+    LevelTaps<F16TAB> t[LIF];
+#pragma unroll
+    for (int q = 0; q < LIF; ++q)
+      if (l0 + q < (int)g.L) gather_level<F16TAB>(g, l0 + q, x, y, z, t[q]);
+    uint32_t f[LIF];
+#pragma unroll
+    for (int q = 0; q < LIF; ++q) f[q] = l0 + q < (int)g.L ? lerp_level(t[q]) : 0u;
+    tmem_stN(tA + l0, f);
+  }
+}
+
+// B over the features at A columns 0.. (hi | lo when PREC = 1): all three layers on the tensor core, biases of layers 1-2
+// ride as K-steps, layer 3 is an N = 16 MMA over the zero-padded 7-row W3; b3 is added in registers.
+template <int PREC, int G>
+__device__ __forceinline__ void brdf_mma(WgCtx& c, const TcConst& cw, const ShadeP& sp, float (&b)[7]) {
+  const uint32_t tA = c.tmem + c.lane, tD = c.tmem + c.lane + Cols<PREC, G>::d;
+  issue_layer<PREC, G>(c, 0, 1, 2, PREC == 1, 1, 2);
+  wait_layer(c);
+  hidden_to_A<PREC == 1>(tD, tA);
+  issue_layer<PREC, G>(c, 0, 3, 4, PREC == 1, 1, 3);
+  wait_layer(c);
+  hidden_to_A<PREC == 1>(tD, tA);
+  issue_layer<PREC, G>(c, 0, 4, 4, PREC == 1, -1, 0, kIdescN16);
+  wait_layer(c);
+  uint32_t r[8];
+  tmem_ld8(tD, r);
+  wait_ld();
+  float o[8];
+#pragma unroll
+  for (int q = 0; q < 8; ++q) o[q] = __uint_as_float(r[q]) + cw.Bb3[q];
+  brdf_maps(sp, o, b);
+}
+
+// Primary point (once per pixel): B in split precision with layer 3 in fp32 registers (n = o/||o|| amplifies an absolute
+// error of o and every sample of the pixel sees the same n).  f (hi | lo) must sit in A columns 0..31.
+template <int PREC, int G>
+__device__ __forceinline__ void brdf_primary(WgCtx& c, const TcConst& cw, const ShadeP& sp, float (&b)[7]) {
+  const uint32_t tA = c.tmem + c.lane, tD = c.tmem + c.lane + Cols<PREC, G>::d;
+  issue_layer<PREC, G>(c, 0, 1, 2, true, 1, 2);
+  wait_layer(c);
+  hidden_to_A<true>(tD, tA);
+  constexpr bool bias64 = Cols<PREC, G>::bias64;
+  issue_layer<PREC, G>(c, 0, 3, 4, true, bias64 ? 1 : -1, 3);
+  wait_layer(c);
+  float o[8];
+#pragma unroll
+  for (int q = 0; q < 8; ++q) o[q] = cw.Bb3[q];
+#pragma unroll
+  for (int h = 0; h < 2; ++h) {
+    uint32_t r[32];
+    tmem_ld32(tD + 32 * h, r);
+    wait_ld();
+#pragma unroll
+    for (int k = 0; k < 32; ++k) {
+      const float a = fmaxf(bias64 ? __uint_as_float(r[k]) : __uint_as_float(r[k]) + cw.Bb2[32 * h + k], 0.f);
+#pragma unroll
+      for (int q = 0; q < 7; ++q) o[q] = fmaf(a, cw.BW3[q][32 * h + k], o[q]);
+    }
+  }
+  if (!bias64) restore_one<PREC, G>(c);
+  brdf_maps(sp, o, b);
+}
+
+// ---------------------------------------------------------------------------------------------------- shared memory
+template <int PREC, bool TSHARED, int G> struct SmemPlan {
+  static constexpr bool p2_in_smem = !TSHARED;                       // per-point tertiary sets keep P' in shared memory
+  static constexpr size_t tiles = (size_t)kHiTileBytes * (PREC ? 2 : 1);
+  static constexpr size_t per_wg = (size_t)kH * kRows * 4 * (p2_in_smem ? 2 : 1)      // Ps (+ P2s)
+                                   + kRows * 4 * 4                                     // acc[128][4]
+                                   + 64;                                               // queue head/tail, tile slot
+  static constexpr size_t shared_set = (size_t)kMaxS2 * kH * 4 + kMaxS2 * 8 * 4;      // Qt, Lt
+  static constexpr size_t bytes = 1024 + tiles + G * per_wg + shared_set + 8 * kMaxG + 16;
+};
+
+// ---------------------------------------------------------------------------------------------------- the kernel
+// counters[0]: next tile (zeroed before every launch); [1]: items evaluated; [2]: secondary rays traced (dense count)
+template <bool F16TAB, int PREC, bool TSHARED, int G>
+__global__ void __launch_bounds__(kRows* G, 1)
+    k_render_wg(const __grid_constant__ GridP g, EnvP env, ShadeP sp, const __grid_constant__ TcConst cw, const uint8_t* __restrict__ wtiles,
+                const float* __restrict__ wts32, FrameP fr, float* __restrict__ rgb, Item* __restrict__ ring,
+                unsigned long long* __restrict__ counters) {
+  using CL = Cols<PREC, G>;
+  constexpr int LIF = G == 4 ? 2 : 4;               // register budget: 128 per thread at G = 4
+  using SP = SmemPlan<PREC, TSHARED, G>;
+  extern __shared__ uint8_t smem_raw[];
+  uint8_t* sp0 = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
+  uint8_t* s_tiles = sp0;
+  uint8_t* s_wg = s_tiles + SP::tiles;
+  float* s_Qt = reinterpret_cast<float*>(s_wg + G * SP::per_wg);
+  float* s_Lt = s_Qt + kMaxS2 * kH;
+  uint64_t* s_mbar = reinterpret_cast<uint64_t*>(s_Lt + kMaxS2 * 8);
+  uint32_t* s_tmem = reinterpret_cast<uint32_t*>(s_mbar + kMaxG);
+
+  const int wgi = threadIdx.x / kRows;
+  const int warp = threadIdx.x >> 5;
+  WgCtx c;
+  c.t = threadIdx.x % kRows;
+  c.bar_id = 1 + wgi;
+  // ---- setup: TMEM (the CTA owns all 512 columns), mbarriers, weight tiles -----------------------------------------
+  if (warp == 0) {
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(s_tmem)), "r"(512u) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+  }
+  if (threadIdx.x < G) asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(smem_u32(s_mbar + threadIdx.x)) : "memory");
+  if (threadIdx.x == 0) asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  {
+    const uint4* src = reinterpret_cast<const uint4*>(wtiles);
+    uint4* dst = reinterpret_cast<uint4*>(s_tiles);
+    for (int i = threadIdx.x; i < (int)(SP::tiles / 16); i += kRows * G) dst[i] = __ldg(src + i);
+  }
+  const bool indirect = (fr.flags & 4u) && fr.s.S && fr.t.S;
+  if (indirect && TSHARED) {                    // shared tertiary set: Q_k = W1w . w'_k; per k: radiance, pdf, direction
+    for (int e = threadIdx.x; e < (int)fr.t.S * kH; e += kRows * G) {
+      const int k = e / kH, q = e % kH;
+      const float* dp = fr.t.dir + 3 * k;
+      const float qv = cw.w1w[0][q] * __ldg(dp) + cw.w1w[1][q] * __ldg(dp + 1) + cw.w1w[2][q] * __ldg(dp + 2);
+      if (PREC == 0) reinterpret_cast<__half*>(s_Qt)[e] = __float2half_rn(qv);
+      else s_Qt[e] = qv;
+    }
+    for (int k = threadIdx.x; k < (int)fr.t.S; k += kRows * G) {
+      const float* dp = fr.t.dir + 3 * k;
+      const float tx = __ldg(dp), ty = __ldg(dp + 1), tz = __ldg(dp + 2);
+      float3 L;
+      if (fr.t.Lin) L = make_float3(__ldg(fr.t.Lin + 3 * k), __ldg(fr.t.Lin + 3 * k + 1), __ldg(fr.t.Lin + 3 * k + 2));
+      else L = env_lookup(env, tx, ty, tz);
+      float* o = s_Lt + 8 * k;
+      o[0] = L.x; o[1] = L.y; o[2] = L.z; o[3] = __ldg(fr.t.pdf + k); o[4] = tx; o[5] = ty; o[6] = tz; o[7] = 0.f;
+    }
+  }
+  asm volatile("fence.proxy.async.shared::cta;" ::: "memory");     // generic-proxy tile writes -> visible to the tensor core
+  fence_before();
+  __syncthreads();
+  fence_after();
+  c.tmem = *s_tmem + CL::stride * wgi;
+  c.lane = (uint32_t)((warp & 3) * 32) << 16;
+  c.mbar = smem_u32(s_mbar + wgi);
+  c.phase = 0;
+  c.tile0 = smem_u32(s_tiles);
+  c.lo_off = kHiTileBytes;
+  const uint32_t tA = c.tmem + c.lane, tD = c.tmem + c.lane + CL::d;
+  restore_one<PREC, G>(c);
+  wait_st();
+  uint8_t* my = s_wg + wgi * SP::per_wg;
+  float* Ps = reinterpret_cast<float*>(my) + c.t;                                     // Ps[k * 128]
+  float* P2s = SP::p2_in_smem ? Ps + kH * kRows : nullptr;
+  float* acc = reinterpret_cast<float*>(my + (size_t)kH * kRows * 4 * (SP::p2_in_smem ? 2 : 1));
+  uint32_t* qctl = reinterpret_cast<uint32_t*>(acc + kRows * 4);                      // [0] head, [1] tail, [2] tile
+  Item* myring = ring + ((size_t)blockIdx.x * G + wgi) * kRing;
+  if (c.t == 0) { qctl[0] = 0u; qctl[1] = 0u; }
+  const unsigned long long ntiles = (fr.N + kRows - 1) / kRows;
+  const int S_i = indirect ? (int)fr.s.S : 0;
+  const uint32_t S2 = fr.t.S;
+  const bool dense = fr.flags & 8u;
+  const bool shadow = fr.flags & 2u;
+  uint32_t n_items = 0, n_rays = 0;
+  uint32_t head = 0;                                                                  // mirrored in registers (uniform in the WG)
+
+  // ---- phase C: one 128-item group, one item per thread -------------------------------------------------------------
+  auto drain_group = [&](uint32_t count, unsigned long long tile_base) {
+    const bool on = (uint32_t)c.t < count;
+    float ix = 0.5f, iy = 0.5f, iz = 0.5f, iwx = 0.f, iwy = 0.f, iwz = 1.f, wr = 0.f, wgc = 0.f, wb = 0.f;
+    uint32_t owner = 0;
+    if (on) {
+      const float4* ip = reinterpret_cast<const float4*>(myring + ((head + c.t) & (kRing - 1)));
+      const float4 a = __ldcg(ip), b4 = __ldcg(ip + 1), c4 = __ldcg(ip + 2);
+      ix = a.x; iy = a.y; iz = a.z; iwx = a.w; iwy = b4.x; iwz = b4.y; wr = b4.z; wgc = b4.w; wb = c4.x;
+      owner = __float_as_uint(c4.y);
+    }
+    // a1-a4 at x', then P' = W1f f' + b1
+    if (PREC == 1) encode_split_to<F16TAB, LIF>(tA, g, ix, iy, iz);
+    else encode_fast_to<F16TAB, LIF>(tA, g, ix, iy, iz);
+    issue_layer<PREC, G>(c, 0, 0, 2, PREC == 1, 0, 2);
+    wait_layer(c);
+    uint32_t P2h[kH / 2];                                             // only the one the instantiation uses survives
+    float P2[kH];
+    if constexpr (TSHARED) {
+      if constexpr (PREC == 0) load_D_h2(tD, P2h); else load_D_f32(tD, P2);
+    } else {
+#pragma unroll
+      for (int h = 0; h < 2; ++h) {
+        uint32_t r[32];
+        tmem_ld32(tD + 32 * h, r);
+        wait_ld();
+#pragma unroll
+        for (int k = 0; k < 32; ++k) P2s[(32 * h + k) * kRows] = __uint_as_float(r[k]);
+      }
+    }
+    float bb[7];
+    brdf_mma<PREC, G>(c, cw, sp, bb);                                 // a5 at x' (A columns 0.. still hold f')
+    // a8: Eq. 1 at x' over the tertiary set, w_o' = -w_j
+    const unsigned long long trow = TSHARED ? 0ull : (tile_base + (owner & 0xFFu)) * (unsigned long long)fr.s.S + (owner >> 8);
+    float lr = 0.f, lg = 0.f, lb = 0.f;
+    for (uint32_t k = 0; k < S2; ++k) {
+      float tx, ty, tz, tpdf;
+      float3 L;
+      if constexpr (TSHARED) {
+        if constexpr (PREC == 0) h1_shared_h2(tA, P2h, reinterpret_cast<const uint32_t*>(s_Qt) + k * (kH / 2));
+        else h1_shared_split(tA, P2, s_Qt + k * kH);
+      } else {
+        const float* tp = dir_of(fr.t, trow, k);
+        h1_dir<PREC == 1>(tA, cw, [&](int j) { return P2s[j * kRows]; }, __ldg(tp), __ldg(tp + 1), __ldg(tp + 2));
+      }
+      issue_layer<PREC, G>(c, 0, 2, 4, PREC == 1, 0, 3);
+      if (TSHARED) {                                                  // shading factors: they do not need the MMA
+        const float4 a = reinterpret_cast<const float4*>(s_Lt)[2 * k], d = reinterpret_cast<const float4*>(s_Lt)[2 * k + 1];
+        L = make_float3(a.x, a.y, a.z); tpdf = a.w; tx = d.x; ty = d.y; tz = d.z;
+      } else {
+        const float* tp = dir_of(fr.t, trow, k);
+        tx = __ldg(tp); ty = __ldg(tp + 1); tz = __ldg(tp + 2); tpdf = pdf_of(fr.t, trow, k);
+        L = incoming(env, fr.t, trow, k, tx, ty, tz);
+      }
+      const float3 gg = brdf_cos_over_pdf(sp, bb, tx, ty, tz, -iwx, -iwy, -iwz, tpdf);
+      wait_layer(c);
+      const float v2 = vis_of(sp, PREC == 0 ? epi_fast(tD, cw) : epi_precise_v(tD, cw));
+      lr = fmaf(v2 * L.x, gg.x, lr); lg = fmaf(v2 * L.y, gg.y, lg); lb = fmaf(v2 * L.z, gg.z, lb);
+    }
+    if (on) {
+      float* a = acc + 4 * (owner & 0xFFu);
+      atomicAdd(a, wr * lr); atomicAdd(a + 1, wgc * lg); atomicAdd(a + 2, wb * lb);
+    }
+  };
+
+  // ---- tile loop (dynamic: work per tile varies with the number of occluded rays) ------------------------------------
+  while (true) {
+    if (c.t == 0) qctl[2] = (uint32_t)atomicAdd(counters, 1ull);
+    wg_sync(c);
+    const unsigned long long tile = qctl[2];
+    if (tile >= ntiles) break;
+    const unsigned long long tile_base = tile * kRows;
+    const unsigned long long i_raw = tile_base + c.t;
+    const bool valid = i_raw < fr.N;
+    const unsigned long long i = valid ? i_raw : fr.N - 1;          // idle rows shadow the last point (uniform control flow)
+    const bool live = valid && !(fr.mask && !fr.mask[i]);
+    const float px = __ldg(fr.x + 3 * i), py = __ldg(fr.x + 3 * i + 1), pz = __ldg(fr.x + 3 * i + 2);
+    const float ox = __ldg(fr.wo + 3 * i), oy = __ldg(fr.wo + 3 * i + 1), oz = __ldg(fr.wo + 3 * i + 2);
+    float b[7];
+    float r = 0.f, gch = 0.f, bch = 0.f;
+    acc[4 * c.t] = 0.f; acc[4 * c.t + 1] = 0.f; acc[4 * c.t + 2] = 0.f;
+
+    // ---- phase A: primary point ---------------------------------------------------------------------------------------
+    const bool decode = !fr.brdf;
+    encode_split_to<F16TAB, LIF>(tA, g, px, py, pz, (PREC == 1 && decode) ? Ps : nullptr);
+    issue_layer<PREC, G>(c, 0, 0, 2, true, 0, 2);                     // P = W1f f + b1
+    if (PREC == 1 && decode) {
+      // fp32 model: the primary point's B runs in plain fp32 FFMAs (weights broadcast from L1) while the MMA is in
+      // flight.  n = o/||o|| and n.w amplify an absolute error of o, and every sample of the pixel shares it, so the
+      // 22-bit split arithmetic is not enough here; the cost is once per pixel.
+      brdf_decode_scr<kRows>(sp, wts32, Ps, b);
+    }
+    wait_layer(c);
+    {
+#pragma unroll
+      for (int h = 0; h < 2; ++h) {
+        uint32_t rr[32];
+        tmem_ld32(tD + 32 * h, rr);
+        wait_ld();
+#pragma unroll
+        for (int k = 0; k < 32; ++k) Ps[(32 * h + k) * kRows] = __uint_as_float(rr[k]);
+      }
+    }
+    if (!decode) {
+#pragma unroll
+      for (int k = 0; k < 7; ++k) b[k] = __ldg(fr.brdf + i * 7 + k);
+    } else if (PREC == 0) {
+      brdf_primary<PREC, G>(c, cw, sp, b);                            // A columns 0..31 still hold f (hi | lo)
+    }
+
+    // ---- phase A2: direct term of Eq. 1 -------------------------------------------------------------------------------
+    if ((fr.flags & 1u) && fr.d.S) {
+      const uint32_t S = fr.d.S;
+      float ar = 0.f, ag = 0.f, ab = 0.f;
+      const float* dp = dir_of(fr.d, i, 0);
+      float nx = __ldg(dp), ny = __ldg(dp + 1), nz = __ldg(dp + 2), np = pdf_of(fr.d, i, 0);
+      for (uint32_t k = 0; k < S; ++k) {
+        const float wx = nx, wy = ny, wz = nz, wp = np;
+        const uint32_t k1 = k + 1 < S ? k + 1 : k;                    // prefetch the next direction
+        dp = dir_of(fr.d, i, k1);
+        nx = __ldg(dp); ny = __ldg(dp + 1); nz = __ldg(dp + 2); np = pdf_of(fr.d, i, k1);
+        if (shadow) {
+          h1_dir<PREC == 1>(tA, cw, [&](int j) { return Ps[j * kRows]; }, wx, wy, wz);
+          issue_layer<PREC, G>(c, 0, 2, 4, PREC == 1, 0, 3);
+        }
+        const float3 gg = brdf_cos_over_pdf(sp, b, wx, wy, wz, ox, oy, oz, wp);
+        const float3 L = incoming(env, fr.d, i, k, wx, wy, wz);
+        float vd = 1.f;
+        if (shadow) {
+          wait_layer(c);
+          vd = vis_of(sp, PREC == 0 ? epi_fast(tD, cw) : epi_precise_v(tD, cw));
+        }
+        ar = fmaf(vd * L.x, gg.x, ar); ag = fmaf(vd * L.y, gg.y, ag); ab = fmaf(vd * L.z, gg.z, ab);
+      }
+      const float inv = 1.f / (float)S;
+      r = ar * inv; gch = ag * inv; bch = ab * inv;
+    }
+
+    // ---- phases B + C: secondary rays -> work items -> L'_o -----------------------------------------------------------
+    if (S_i > 0) {
+      const float wscale = 1.f / ((float)S_i * (float)S2);
+      for (int j0 = 0; j0 < S_i; j0 += kChunkJ) {
+        const int j1 = min(j0 + kChunkJ, S_i);
+        for (int j = j0; j < j1; ++j) {
+          const float* dp = dir_of(fr.s, i, j);
+          const float wx = __ldg(dp), wy = __ldg(dp + 1), wz = __ldg(dp + 2), wp = pdf_of(fr.s, i, j);
+          h1_dir<true>(tA, cw, [&](int q) { return Ps[q * kRows]; }, wx, wy, wz);
+          issue_layer<PREC, G>(c, 0, 2, 4, true, CL::bias64 ? 0 : -1, 3);
+          const float3 gg = brdf_cos_over_pdf(sp, b, wx, wy, wz, ox, oy, oz, wp);
+          wait_layer(c);
+          float zv, zt, v, t;
+          epi_precise<!CL::bias64>(tD, cw, zv, zt);
+          if (!CL::bias64) restore_one<PREC, G>(c);
+          irt_maps(sp, zv, zt, v, t);
+          const float m = (1.f - v) * wscale;
+          const float gr = m * gg.x, ggc = m * gg.y, gb = m * gg.z;
+          const bool push = live && (dense || gr != 0.f || ggc != 0.f || gb != 0.f);
+          const unsigned bal = __ballot_sync(0xFFFFFFFFu, push);
+          if (bal) {
+            const int lane = threadIdx.x & 31, leader = __ffs(bal) - 1;
+            uint32_t base = 0;
+            if (lane == leader) base = atomicAdd(&qctl[1], (uint32_t)__popc(bal));
+            base = __shfl_sync(0xFFFFFFFFu, base, leader);
+            if (push) {
+              float4* ip = reinterpret_cast<float4*>(myring + ((base + __popc(bal & ((1u << lane) - 1u))) & (kRing - 1)));
+              __stcg(ip, make_float4(sec_hit(px, t, wx), sec_hit(py, t, wy), sec_hit(pz, t, wz), wx));
+              __stcg(ip + 1, make_float4(wy, wz, gr, ggc));
+              __stcg(ip + 2, make_float4(gb, __uint_as_float((uint32_t)c.t | ((uint32_t)j << 8)), 0.f, 0.f));
+            }
+          }
+          n_rays += live ? 1u : 0u;
+        }
+        wg_sync(c);                                                   // items of this chunk are visible to the whole WG
+        uint32_t count = qctl[1] - head;
+        const bool last = j1 == S_i;
+        while (count >= (uint32_t)kRows || (last && count > 0u)) {
+          const uint32_t n = count < (uint32_t)kRows ? count : (uint32_t)kRows;
+          drain_group(n, tile_base);
+          head += n; count -= n;
+          n_items += (uint32_t)c.t < n ? 1u : 0u;
+        }
+      }
+      wg_sync(c);                                                     // every contribution has landed in acc
+      r += acc[4 * c.t]; gch += acc[4 * c.t + 1]; bch += acc[4 * c.t + 2];
+    }
+    if (valid) {
+      rgb[3 * i] = live ? r : 0.f; rgb[3 * i + 1] = live ? gch : 0.f; rgb[3 * i + 2] = live ? bch : 0.f;
+    }
+  }
+  // ---- teardown ---------------------------------------------------------------------------------------------------------
+  for (int o = 16; o > 0; o >>= 1) {
+    n_items += __shfl_xor_sync(0xFFFFFFFFu, n_items, o);
+    n_rays += __shfl_xor_sync(0xFFFFFFFFu, n_rays, o);
+  }
+  if ((threadIdx.x & 31) == 0 && (n_items | n_rays)) { atomicAdd(counters + 1, (unsigned long long)n_items); atomicAdd(counters + 2, (unsigned long long)n_rays); }
+  fence_before();
+  __syncthreads();
+  if (warp == 0) {
+    fence_after();
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(*s_tmem), "r"(512u) : "memory");
+  }
+}
+
+// ---------------------------------------------------------------------------------------------------- host side
+// Blob = [ TcConst | hi tiles (34 KB) | lo tiles (34 KB) ].  hi = fp16(w), lo = fp16(w - hi); bias K-steps only in the hi tiles.
+inline void prepare_weights(const hr_config& cfg, const float* bw, const float* iw, std::vector<uint8_t>& out) {
+  std::vector<uint8_t> hi;
+  tc::prepare_weights(cfg, bw, iw, hi);                 // TcConst + hi tiles (weights rounded to fp16, biases split)
+  out.assign(sizeof(TcConst) + 2 * kHiTileBytes, 0);
+  memcpy(out.data(), hi.data(), sizeof(TcConst) + kHiTileBytes);
+  const int D = cfg.L * cfg.F, H = kH, Din = D + 3;
+  uint8_t* lo = out.data() + sizeof(TcConst) + kHiTileBytes;
+  auto put_lo = [&](int t, int j, int k, float v) {
+    const float h = __half2float(__float2half_rn(v));
+    *reinterpret_cast<__half*>(lo + (size_t)t * kTileBytes + tile_off(j, k)) = __float2half_rn(v - h);
+  };
+  const float* BW1 = bw; const float* BW2 = BW1 + H * D + H; const float* BW3 = BW2 + H * H + H;
+  const float* IW1 = iw; const float* IW2 = IW1 + H * Din + H;
+  for (int j = 0; j < H; ++j) {
+    for (int k = 0; k < D; ++k) { put_lo(0, j, k, IW1[j * Din + k]); put_lo(1, j, k, BW1[j * D + k]); }
+    for (int k = 0; k < H; ++k) { put_lo(2, j, k, IW2[j * H + k]); put_lo(3, j, k, BW2[j * H + k]); }
+    for (int q = 0; q < 7; ++q) put_lo(4, q, j, BW3[q * H + j]);
+  }
+}
+
+inline bool frame_supported(const FrameP& fr) { return !(fr.flags & 4u) || fr.t.stride != 0 || fr.t.S <= (uint32_t)kMaxS2; }
+
+template <bool F16TAB, int PREC, bool TSHARED, int G>
+inline cudaError_t launch_one(const GridP& g, const EnvP& env, const ShadeP& sp, const TcConst& cw, const uint8_t* d_tiles,
+                              const float* wts32, const FrameP& fr, float* rgb, Item* ring, unsigned long long* counters, int num_sms, cudaStream_t st) {
+  using SP = SmemPlan<PREC, TSHARED, G>;
+  static bool attr_done = false;
+  auto kern = k_render_wg<F16TAB, PREC, TSHARED, G>;
+  if (!attr_done) {
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SP::bytes);
+    if (e != cudaSuccess) return e;
+    attr_done = true;
+  }
+  cudaError_t e = cudaMemsetAsync(counters, 0, 8, st);                // the tile counter; the statistics keep accumulating
+  if (e != cudaSuccess) return e;
+  const unsigned long long tiles = (fr.N + kRows - 1) / kRows;
+  const unsigned long long need = (tiles + G - 1) / G;
+  const int grid = (int)(need < (unsigned long long)num_sms ? need : (unsigned long long)num_sms);
+  kern<<<grid, kRows * G, SP::bytes, st>>>(g, env, sp, cw, d_tiles, wts32, fr, rgb, ring, counters);
+  return cudaGetLastError();
+}
+
+}  // namespace wg
+}  // namespace hr

@@ -1,0 +1,26 @@
+// hr_wg_p1.cu -- instantiations of k_render_wg in split precision (mlp_dtype == HR_F32 on the fp16 tensor cores).
+#include "hr_render_wg.cuh"
+#include "hr_wg_api.h"
+
+#ifndef HR_G_P1
+#define HR_G_P1 3
+#endif
+
+namespace hr {
+namespace wg {
+
+cudaError_t launch_p1(bool f16tab, const GridP& g, const EnvP& env, const ShadeP& sp, const void* tc_const, const uint8_t* d_tiles,
+                      const float* wts32, const FrameP& fr, float* rgb, void* ring, unsigned long long* counters, int num_sms, cudaStream_t st) {
+  const TcConst& cw = *reinterpret_cast<const TcConst*>(tc_const);
+  Item* rg = reinterpret_cast<Item*>(ring);
+  const bool tsh = fr.t.stride == 0;
+  if (f16tab) {
+    if (tsh) return launch_one<true, 1, true, HR_G_P1>(g, env, sp, cw, d_tiles, wts32, fr, rgb, rg, counters, num_sms, st);
+    return launch_one<true, 1, false, 2>(g, env, sp, cw, d_tiles, wts32, fr, rgb, rg, counters, num_sms, st);
+  }
+  if (tsh) return launch_one<false, 1, true, HR_G_P1>(g, env, sp, cw, d_tiles, wts32, fr, rgb, rg, counters, num_sms, st);
+  return launch_one<false, 1, false, 2>(g, env, sp, cw, d_tiles, wts32, fr, rgb, rg, counters, num_sms, st);
+}
+
+}  // namespace wg
+}  // namespace hr

@@ -13,7 +13,7 @@ from hr_testutil import check_close, gpu_render, make_renderer, oracle_render, t
 pytestmark = pytest.mark.gpu
 
 TOL32, TOL16 = 1e-4, 3e-3
-DELTA32, DELTA16 = 2e-5, 4e-3      # |z_v| band in which a hard-visibility flip is legitimate (Q33)
+DELTA32, DELTA16 = 1e-4, 4e-3      # |z_v| band in which a hard-visibility flip is legitimate (Q33)
 
 
 @pytest.fixture(scope="module")
@@ -258,8 +258,36 @@ def test_render_frame_host_matches_device(torch):
     r = make_renderer(cfg, m)
     a = gpu_render(r, cfg, fr)
     b = gpu_render(r, cfg, fr, host=True)
-    assert np.array_equal(a, b)
+    # same kernel, same inputs; the indirect term is summed with shared-memory float atomics, so the order (and the
+    # last bit) may differ from run to run
+    np.testing.assert_allclose(a, b, rtol=2e-6, atol=1e-7)
     assert r.launch_count() >= 2
+
+
+@pytest.mark.parametrize("name", ["C2", "C3"])
+def test_compaction_equals_dense(torch, name):
+    """only rays with a non-zero Eq. 2 weight are traced further.  The compacted evaluation (default) and the
+    dense one (HR_DENSE) must give the same frame (up to the summation order of the shared-memory atomics), and the
+    ray accounting must add up."""
+    from paper_2409_10327_b200 import HR_DENSE
+    cfg = gen.make_config(name)
+    m = gen.make_model(cfg)
+    pix = np.arange(0, cfg.N, 487)
+    fr = gen.make_frame(cfg, m["env"], pix)
+    r = make_renderer(cfg, m, vis_mode=1)
+    r.stats(reset=True)
+    a = gpu_render(r, cfg, fr, flags=cfg.flags | HR_DENSE)
+    traced_d, eval_d = r.stats(reset=True)
+    b = gpu_render(r, cfg, fr, flags=cfg.flags)
+    traced_c, eval_c = r.stats(reset=True)
+    assert traced_d == traced_c == len(pix) * cfg.S_i
+    assert eval_d == traced_d and 0 < eval_c < traced_c
+    np.testing.assert_allclose(a, b, rtol=5e-6, atol=1e-7)
+    # soft visibility: (1 - v) never vanishes, only back-facing / zero-pdf rays drop out
+    r0 = make_renderer(cfg, m, vis_mode=0)
+    a0 = gpu_render(r0, cfg, fr, flags=cfg.flags | HR_DENSE)
+    b0 = gpu_render(r0, cfg, fr, flags=cfg.flags)
+    np.testing.assert_allclose(a0, b0, rtol=5e-6, atol=1e-7)
 
 
 def test_frame_errors(torch):
