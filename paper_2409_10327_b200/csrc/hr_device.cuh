@@ -89,15 +89,25 @@ __device__ __forceinline__ void corner_indices(const Cell& c, uint32_t N, bool d
   }
 }
 
+// Gather of one table row: address = level base + idx * row bytes in ONE integer multiply-add (mad.wide.u32), read-only path.
+__device__ __forceinline__ __half2 gather_h2(const void* level_base, uint32_t idx) {
+  uint32_t v;
+  asm("{\n\t.reg .u64 a;\n\tmad.wide.u32 a, %1, 4, %2;\n\tld.global.nc.b32 %0, [a];\n\t}" : "=r"(v) : "r"(idx), "l"(level_base));
+  return *reinterpret_cast<__half2*>(&v);
+}
+__device__ __forceinline__ float2 gather_f2(const void* level_base, uint32_t idx) {
+  float2 v;
+  asm("{\n\t.reg .u64 a;\n\tmad.wide.u32 a, %2, 8, %3;\n\tld.global.nc.v2.f32 {%0, %1}, [a];\n\t}" : "=f"(v.x), "=f"(v.y) : "r"(idx), "l"(level_base));
+  return v;
+}
 template <bool F16>
-__device__ __forceinline__ float2 table_load(const void* tables, uint32_t log2_T, int l, uint32_t idx) {
-  const size_t off = ((size_t)l << log2_T) + idx;
-  if (F16) {
-    const __half2 v = __ldg(reinterpret_cast<const __half2*>(tables) + off);
-    return __half22float2(v);
-  } else {
-    return __ldg(reinterpret_cast<const float2*>(tables) + off);
-  }
+__device__ __forceinline__ const void* level_base(const void* tables, uint32_t log2_T, int l) {
+  return reinterpret_cast<const char*>(tables) + (((size_t)l << log2_T) << (F16 ? 2 : 3));
+}
+template <bool F16>
+__device__ __forceinline__ float2 table_load(const void* lbase, uint32_t idx) {
+  if (F16) return __half22float2(gather_h2(lbase, idx));
+  return gather_f2(lbase, idx);
 }
 
 // a3/a4: gather 8 corners of one level and interpolate.  Corner number b0 + 2 b1 + 4 b2 (Q9).
@@ -109,8 +119,9 @@ __device__ __forceinline__ float2 encode_level(const GridP& g, int l, float x, f
   uint32_t idx[8];
   corner_indices(c, N, (g.dense_mask >> l) & 1u, g.log2_T, idx);
   float2 v[8];
+  const void* lb = level_base<F16>(g.tables, g.log2_T, l);
 #pragma unroll
-  for (int k = 0; k < 8; ++k) v[k] = table_load<F16>(g.tables, g.log2_T, l, idx[k]);
+  for (int k = 0; k < 8; ++k) v[k] = table_load<F16>(lb, idx[k]);
   if (idx_out) {
 #pragma unroll
     for (int k = 0; k < 8; ++k) idx_out[k] = idx[k];

@@ -67,7 +67,7 @@ __device__ __forceinline__ void mbar_wait(uint32_t mbar, uint32_t parity) {
   do {
     asm volatile("{\n\t.reg .pred P1;\n\tmbarrier.try_wait.parity.shared::cta.b64 P1, [%1], %2;\n\tselp.b32 %0, 1, 0, P1;\n\t}\n"
                  : "=r"(done) : "r"(mbar), "r"(parity) : "memory");
-  } while (!done);
+  } while (!__all_sync(0xFFFFFFFFu, done));                 // warp-uniform exit keeps the code after the wait convergent
 }
 
 #define HR_R16(r, o) "=r"(r[o+0]), "=r"(r[o+1]), "=r"(r[o+2]), "=r"(r[o+3]), "=r"(r[o+4]), "=r"(r[o+5]), "=r"(r[o+6]), "=r"(r[o+7]), \
@@ -210,16 +210,15 @@ __device__ __forceinline__ void gather_level(const GridP& g, int l, float x, flo
   const Cell cl = cell_of_clamped(N, x, y, z);                 // callers pass x' = sec_hit(...), already in [0,1]^3
   uint32_t idx[8];
   corner_indices(cl, N, (g.dense_mask >> l) & 1u, g.log2_T, idx);
+  const void* lb = level_base<F16>(g.tables, g.log2_T, l);
   if constexpr (F16) {
-    const __half2* tb = reinterpret_cast<const __half2*>(g.tables) + ((size_t)l << g.log2_T);
 #pragma unroll
-    for (int k = 0; k < 8; ++k) t.v[k] = __ldg(tb + idx[k]);
+    for (int k = 0; k < 8; ++k) t.v[k] = gather_h2(lb, idx[k]);
 #pragma unroll
     for (int d = 0; d < 3; ++d) t.w[d] = __float2half2_rn(cl.w[d]);
   } else {
-    const float2* tb = reinterpret_cast<const float2*>(g.tables) + ((size_t)l << g.log2_T);
 #pragma unroll
-    for (int k = 0; k < 8; ++k) t.v[k] = __ldg(tb + idx[k]);
+    for (int k = 0; k < 8; ++k) t.v[k] = gather_f2(lb, idx[k]);
 #pragma unroll
     for (int d = 0; d < 3; ++d) t.w[d] = cl.w[d];
   }

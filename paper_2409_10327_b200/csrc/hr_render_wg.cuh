@@ -139,10 +139,8 @@ __device__ __forceinline__ float epi_fast(uint32_t tD, const TcConst& cw) {
       acc[k & 3] = __hfma2(*reinterpret_cast<const __half2*>(&p), *reinterpret_cast<const __half2*>(&w), acc[k & 3]);
     }
   }
-  float z = cw.b3[0];
-#pragma unroll
-  for (int q = 0; q < 4; ++q) { const float2 f = __half22float2(acc[q]); z += f.x + f.y; }
-  return z;
+  const float2 f = __half22float2(__hadd2(__hadd2(acc[0], acc[1]), __hadd2(acc[2], acc[3])));
+  return cw.b3[0] + (f.x + f.y);
 }
 // fp32 epilogues (b2 rode in the MMA as a hi/lo bias K-step unless ADD_B2)
 template <bool ADD_B2>
@@ -195,24 +193,47 @@ __device__ __forceinline__ void hidden_to_A(uint32_t tD, uint32_t tA) {
   }
 }
 
-// h1 = relu(P + W1w . w) -> A; P(j) yields the layer-1 partial of hidden unit j
+// h1 = relu(P + W1w . w) -> A; P4(q) yields the layer-1 partials of hidden units 4q .. 4q+3 (one LDS.128)
 template <bool SPLIT, typename PF>
-__device__ __forceinline__ void h1_dir(uint32_t tA, const TcConst& cw, PF P, float wx, float wy, float wz) {
+__device__ __forceinline__ void h1_dir(uint32_t tA, const TcConst& cw, PF P4, float wx, float wy, float wz) {
 #pragma unroll
   for (int h = 0; h < 2; ++h) {
     uint32_t p[16], q[16];
 #pragma unroll
-    for (int k = 0; k < 16; ++k) {
-      const int j = 32 * h + 2 * k;
-      float a0 = fmaf(cw.w1w[0][j], wx, P(j));
-      a0 = fmaf(cw.w1w[1][j], wy, a0); a0 = fmaf(cw.w1w[2][j], wz, a0);
-      float a1 = fmaf(cw.w1w[0][j + 1], wx, P(j + 1));
-      a1 = fmaf(cw.w1w[1][j + 1], wy, a1); a1 = fmaf(cw.w1w[2][j + 1], wz, a1);
-      if (SPLIT) split_pair(fmaxf(a0, 0.f), fmaxf(a1, 0.f), p[k], q[k]);
-      else p[k] = pack_relu(a0, a1);
+    for (int k = 0; k < 8; ++k) {
+      const float4 pv = P4(8 * h + k);
+      const float pin[4] = {pv.x, pv.y, pv.z, pv.w};
+      float a[4];
+#pragma unroll
+      for (int e = 0; e < 4; ++e) {
+        const int j = 32 * h + 4 * k + e;
+        a[e] = fmaf(cw.w1w[0][j], wx, pin[e]);
+        a[e] = fmaf(cw.w1w[1][j], wy, a[e]);
+        a[e] = fmaf(cw.w1w[2][j], wz, a[e]);
+      }
+      if (SPLIT) {
+        split_pair(fmaxf(a[0], 0.f), fmaxf(a[1], 0.f), p[2 * k], q[2 * k]);
+        split_pair(fmaxf(a[2], 0.f), fmaxf(a[3], 0.f), p[2 * k + 1], q[2 * k + 1]);
+      } else {
+        p[2 * k] = pack_relu(a[0], a[1]);
+        p[2 * k + 1] = pack_relu(a[2], a[3]);
+      }
     }
     tmem_st16(tA + 16 * h, p);
     if (SPLIT) tmem_st16(tA + 32 + 16 * h, q);
+  }
+}
+// D (64 fp32 columns) -> this thread's column of a [16][128] float4 array in shared memory
+__device__ __forceinline__ void store_D_f4(uint32_t tD, float4* dst) {
+#pragma unroll
+  for (int h = 0; h < 2; ++h) {
+    uint32_t r[32];
+    tmem_ld32(tD + 32 * h, r);
+    wait_ld();
+#pragma unroll
+    for (int k = 0; k < 8; ++k)
+      dst[(8 * h + k) * kRows] = make_float4(__uint_as_float(r[4 * k]), __uint_as_float(r[4 * k + 1]), __uint_as_float(r[4 * k + 2]),
+                                             __uint_as_float(r[4 * k + 3]));
   }
 }
 // shared tertiary set, PREC = 0: P and Q = W1w . w'_k both fp16 pairs, one fma.relu per pair
@@ -441,7 +462,8 @@ __global__ void __launch_bounds__(kRows* G, 1)
   wait_st();
   uint8_t* my = s_wg + wgi * SP::per_wg;
   float* Ps = reinterpret_cast<float*>(my) + c.t;                                     // Ps[k * 128]
-  float* P2s = SP::p2_in_smem ? Ps + kH * kRows : nullptr;
+  float4* Ps4 = reinterpret_cast<float4*>(my) + c.t;                                  // the same memory as [16][128] float4
+  float4* P2s4 = SP::p2_in_smem ? Ps4 + (kH / 4) * kRows : nullptr;
   float* acc = reinterpret_cast<float*>(my + (size_t)kH * kRows * 4 * (SP::p2_in_smem ? 2 : 1));
   uint32_t* qctl = reinterpret_cast<uint32_t*>(acc + kRows * 4);                      // [0] head, [1] tail, [2] tile
   Item* myring = ring + ((size_t)blockIdx.x * G + wgi) * kRing;
@@ -475,14 +497,7 @@ __global__ void __launch_bounds__(kRows* G, 1)
     if constexpr (TSHARED) {
       if constexpr (PREC == 0) load_D_h2(tD, P2h); else load_D_f32(tD, P2);
     } else {
-#pragma unroll
-      for (int h = 0; h < 2; ++h) {
-        uint32_t r[32];
-        tmem_ld32(tD + 32 * h, r);
-        wait_ld();
-#pragma unroll
-        for (int k = 0; k < 32; ++k) P2s[(32 * h + k) * kRows] = __uint_as_float(r[k]);
-      }
+      store_D_f4(tD, P2s4);
     }
     float bb[7];
     brdf_mma<PREC, G>(c, cw, sp, bb);                                 // a5 at x' (A columns 0.. still hold f')
@@ -497,7 +512,7 @@ __global__ void __launch_bounds__(kRows* G, 1)
         else h1_shared_split(tA, P2, s_Qt + k * kH);
       } else {
         const float* tp = dir_of(fr.t, trow, k);
-        h1_dir<PREC == 1>(tA, cw, [&](int j) { return P2s[j * kRows]; }, __ldg(tp), __ldg(tp + 1), __ldg(tp + 2));
+        h1_dir<PREC == 1>(tA, cw, [&](int q) { return P2s4[q * kRows]; }, __ldg(tp), __ldg(tp + 1), __ldg(tp + 2));
       }
       issue_layer<PREC, G>(c, 0, 2, 4, PREC == 1, 0, 3);
       if (TSHARED) {                                                  // shading factors: they do not need the MMA
@@ -524,7 +539,7 @@ __global__ void __launch_bounds__(kRows* G, 1)
     if (c.t == 0) qctl[2] = (uint32_t)atomicAdd(counters, 1ull);
     wg_sync(c);
     const unsigned long long tile = qctl[2];
-    if (tile >= ntiles) break;
+    if (__any_sync(0xFFFFFFFFu, tile >= ntiles)) break;      // WG-uniform; the vote tells the compiler so
     const unsigned long long tile_base = tile * kRows;
     const unsigned long long i_raw = tile_base + c.t;
     const bool valid = i_raw < fr.N;
@@ -547,16 +562,7 @@ __global__ void __launch_bounds__(kRows* G, 1)
       brdf_decode_scr<kRows>(sp, wts32, Ps, b);
     }
     wait_layer(c);
-    {
-#pragma unroll
-      for (int h = 0; h < 2; ++h) {
-        uint32_t rr[32];
-        tmem_ld32(tD + 32 * h, rr);
-        wait_ld();
-#pragma unroll
-        for (int k = 0; k < 32; ++k) Ps[(32 * h + k) * kRows] = __uint_as_float(rr[k]);
-      }
-    }
+    store_D_f4(tD, Ps4);
     if (!decode) {
 #pragma unroll
       for (int k = 0; k < 7; ++k) b[k] = __ldg(fr.brdf + i * 7 + k);
@@ -576,7 +582,7 @@ __global__ void __launch_bounds__(kRows* G, 1)
         dp = dir_of(fr.d, i, k1);
         nx = __ldg(dp); ny = __ldg(dp + 1); nz = __ldg(dp + 2); np = pdf_of(fr.d, i, k1);
         if (shadow) {
-          h1_dir<PREC == 1>(tA, cw, [&](int j) { return Ps[j * kRows]; }, wx, wy, wz);
+          h1_dir<PREC == 1>(tA, cw, [&](int q) { return Ps4[q * kRows]; }, wx, wy, wz);
           issue_layer<PREC, G>(c, 0, 2, 4, PREC == 1, 0, 3);
         }
         const float3 gg = brdf_cos_over_pdf(sp, b, wx, wy, wz, ox, oy, oz, wp);
@@ -600,7 +606,7 @@ __global__ void __launch_bounds__(kRows* G, 1)
         for (int j = j0; j < j1; ++j) {
           const float* dp = dir_of(fr.s, i, j);
           const float wx = __ldg(dp), wy = __ldg(dp + 1), wz = __ldg(dp + 2), wp = pdf_of(fr.s, i, j);
-          h1_dir<true>(tA, cw, [&](int q) { return Ps[q * kRows]; }, wx, wy, wz);
+          h1_dir<true>(tA, cw, [&](int q) { return Ps4[q * kRows]; }, wx, wy, wz);
           issue_layer<PREC, G>(c, 0, 2, 4, true, CL::bias64 ? 0 : -1, 3);
           const float3 gg = brdf_cos_over_pdf(sp, b, wx, wy, wz, ox, oy, oz, wp);
           wait_layer(c);
@@ -629,7 +635,7 @@ __global__ void __launch_bounds__(kRows* G, 1)
         wg_sync(c);                                                   // items of this chunk are visible to the whole WG
         uint32_t count = qctl[1] - head;
         const bool last = j1 == S_i;
-        while (count >= (uint32_t)kRows || (last && count > 0u)) {
+        while (__any_sync(0xFFFFFFFFu, count >= (uint32_t)kRows || (last && count > 0u))) {
           const uint32_t n = count < (uint32_t)kRows ? count : (uint32_t)kRows;
           drain_group(n, tile_base);
           head += n; count -= n;
