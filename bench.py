@@ -151,7 +151,9 @@ def run_c4_sweep(args):
     peaks = load_peaks()
     rows = []
     Ns = [1 << 20, 1 << 22, 1 << 24] + ([1 << 26] if args.full_sweep else [])
-    for log2_T in (16, 19, 22, 24):
+    if args.c4_n:
+        Ns = [args.c4_n]
+    for log2_T in ((args.c4_log2t,) if args.c4_log2t else (16, 19, 22, 24)):
         cfg = gen.make_config("C4", log2_T=log2_T, N=max(Ns))
         model = gen.make_model(cfg)
         r = HashRenderer.from_gen(cfg, model, vis_mode=args.vis_mode, max_points=max(Ns))
@@ -199,6 +201,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--workload", default="C2", choices=["C1", "C2", "C3", "C3a", "C4"])
     ap.add_argument("--full-sweep", action="store_true", help="C4: include 2^26 points")
+    ap.add_argument("--c4-log2t", type=int, default=0, help="C4: only this table size (for profiling one point of the sweep)")
+    ap.add_argument("--c4-n", type=int, default=0, help="C4: only this many points")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--vis-mode", type=int, default=1, help="1 = hard visibility (paper-faithful), 0 = soft")
     ap.add_argument("--e2e-steps", type=int, default=3)

@@ -209,7 +209,6 @@ int hashrender_create(const hr_config* cfg, const float* tables, const float* br
     wg::prepare_weights_blob(*cfg, brdf_w, irt_w, h->h_wts_tc, &cb, &tb);
     HR_CUDA(h, cudaMalloc(&h->d_wts_tc, tb));
     HR_CUDA(h, cudaMemcpy(h->d_wts_tc, h->h_wts_tc.data() + cb, tb, cudaMemcpyHostToDevice));
-    HR_CUDA(h, tc::set_attributes());
     HR_CUDA(h, cudaMalloc(&h->d_ring, wg::ring_bytes(h->num_sms)));
     HR_CUDA(h, cudaMalloc(&h->d_counters, 4 * sizeof(unsigned long long)));
     HR_CUDA(h, cudaMemset(h->d_counters, 0, 4 * sizeof(unsigned long long)));
@@ -298,8 +297,8 @@ int hashrender_trace(hashrender_t* h, const float* x, const float* feat, uint64_
   const DirsetP d = to_dev(*ds);
   if (render_path(h) == 1 && !feat) {
     h->last_path = "tcgen05-f16";
-    HR_CUDA(h, tc::launch_trace(h->grid, h->shade, *reinterpret_cast<const tc::TcConst*>(h->h_wts_tc.data()), h->d_wts_tc, x, N, d, vis,
-                                zv, t, xsec, h->num_sms, (cudaStream_t)stream));
+    HR_CUDA(h, wg::launch_trace_p0(h->grid.f16, h->grid, h->shade, h->h_wts_tc.data(), h->d_wts_tc, x, N, d, vis, zv, t, xsec, h->num_sms,
+                                   (cudaStream_t)stream));
     h->launches++;
     return HR_OK;
   }

@@ -545,48 +545,6 @@ __device__ __forceinline__ void teardown(const Ctx& c) {
   }
 }
 
-// ---------------------------------------------------------------------------------------------------- kernels
-// trace with the encode fused (a1-a4, a6, a7), tensor-core path (t is an output: precise epilogue).
-template <bool F16>
-__global__ void __launch_bounds__(kThreads, kCtasPerSm) k_trace_tc(const __grid_constant__ GridP g, ShadeP sp, const __grid_constant__ TcConst cw,
-                                                                   const uint8_t* __restrict__ wtiles, const float* __restrict__ x,
-                                                                   unsigned long long N, DirsetP ds, float* __restrict__ vis,
-                                                                   float* __restrict__ zvo, float* __restrict__ to, float* __restrict__ xsec) {
-  extern __shared__ uint8_t smem_raw[];
-  const Smem s = carve(smem_raw);
-  Ctx c;
-  setup(s, wtiles, c);
-  const unsigned long long ntiles = (N + kThreads - 1) / kThreads;
-  for (unsigned long long tile = blockIdx.x; tile < ntiles; tile += gridDim.x) {
-    const unsigned long long i_raw = tile * kThreads + threadIdx.x;
-    const bool valid = i_raw < N;
-    const unsigned long long i = valid ? i_raw : N - 1;
-    const float px = __ldg(x + 3 * i), py = __ldg(x + 3 * i + 1), pz = __ldg(x + 3 * i + 2);
-    encode_split_to_A<F16>(g, c, px, py, pz);
-    issue_layer(c, 0, kColA, 0, 2, 0, 2, true);
-    wait_layer(c, 0);
-    float P[kH];
-    load_D(c, P);
-    for (uint32_t sidx = 0; sidx < ds.S; ++sidx) {
-      const float* dp = dir_of(ds, i, sidx);
-      const float wx = __ldg(dp), wy = __ldg(dp + 1), wz = __ldg(dp + 2);
-      h1_from_regs(c, cw, 0, P, wx, wy, wz);
-      issue_layer(c, 0, kColA, 2, 4, -1, 0);
-      wait_layer(c, 0);
-      float zv, zt, v, t;
-      irt_epilogue_precise(c, cw, 0, zv, zt);
-      irt_maps(sp, zv, zt, v, t);
-      if (valid) {
-        const unsigned long long o = i * ds.S + sidx;
-        vis[o] = v; to[o] = t;
-        if (zvo) zvo[o] = zv;
-        if (xsec) { xsec[o * 3] = sec_hit(px, t, wx); xsec[o * 3 + 1] = sec_hit(py, t, wy); xsec[o * 3 + 2] = sec_hit(pz, t, wz); }
-      }
-    }
-  }
-  teardown(c);
-}
-
 // ---------------------------------------------------------------------------------------------------- host side
 struct HostWeights { TcConst cw; };
 
@@ -628,29 +586,7 @@ inline void prepare_weights(const hr_config& cfg, const float* bw, const float* 
   for (int q = 0; q < 8; ++q) cw.Bb3[q] = q < 7 ? Bb3[q] : 0.f;
 }
 
-inline cudaError_t set_attributes() {
-  cudaError_t e;
-  if ((e = cudaFuncSetAttribute(k_trace_tc<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes))) return e;
-  if ((e = cudaFuncSetAttribute(k_trace_tc<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kSmemBytes))) return e;
-  return cudaSuccess;
-}
-
 inline bool frame_supported(const FrameP& fr) { return !(fr.flags & 4u) || fr.t.stride != 0 || fr.t.S <= (uint32_t)kMaxS2; }
-
-inline int grid_size(unsigned long long N, int num_sms) {
-  const unsigned long long tiles = (N + kThreads - 1) / kThreads;
-  const unsigned long long cap = (unsigned long long)num_sms * kCtasPerSm;
-  return (int)(tiles < cap ? tiles : cap);
-}
-
-inline cudaError_t launch_trace(const GridP& g, const ShadeP& sp, const TcConst& cw, const uint8_t* d_tiles, const float* x,
-                                unsigned long long N, const DirsetP& ds, float* vis, float* zv, float* t, float* xsec, int num_sms,
-                                cudaStream_t st) {
-  const int grid = grid_size(N, num_sms);
-  if (g.f16) k_trace_tc<true><<<grid, kThreads, kSmemBytes, st>>>(g, sp, cw, d_tiles, x, N, ds, vis, zv, t, xsec);
-  else k_trace_tc<false><<<grid, kThreads, kSmemBytes, st>>>(g, sp, cw, d_tiles, x, N, ds, vis, zv, t, xsec);
-  return cudaGetLastError();
-}
 
 }  // namespace tc
 }  // namespace hr

@@ -663,6 +663,107 @@ __global__ void __launch_bounds__(kRows* G, 1)
   }
 }
 
+// ---------------------------------------------------------------------------------------------------- trace kernel
+// hashrender_trace with the encode fused (a1-a4, a6, a7) for fp16 models -- the kernel of the encode + IRT sweep
+// (BASELINE.json configs[4]).  Same warpgroup scheme with G = 4 and four levels (32 gathers) in flight per thread: 16 warps
+// x 32 outstanding loads per SM keep the gather pipeline full when the table spills from L2 to HBM.  t is an output, so the
+// fp32 epilogue is used (features hi/lo split for P, fp16 h1).
+constexpr int kTraceG = 4;
+constexpr size_t kTraceSmem = 1024 + kHiTileBytes + (size_t)kTraceG * kH * kRows * 4 + 8 * kMaxG + 16;
+
+template <bool F16TAB>
+__global__ void __launch_bounds__(kRows* kTraceG, 1)
+    k_trace_wg(const __grid_constant__ GridP g, ShadeP sp, const __grid_constant__ TcConst cw, const uint8_t* __restrict__ wtiles,
+               const float* __restrict__ x, unsigned long long N, DirsetP ds, float* __restrict__ vis, float* __restrict__ zvo,
+               float* __restrict__ to, float* __restrict__ xsec) {
+  constexpr int G = kTraceG;
+  using CL = Cols<0, G>;
+  extern __shared__ uint8_t smem_raw[];
+  uint8_t* s_tiles = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
+  float4* s_P = reinterpret_cast<float4*>(s_tiles + kHiTileBytes);
+  uint64_t* s_mbar = reinterpret_cast<uint64_t*>(s_P + (size_t)G * (kH / 4) * kRows);
+  uint32_t* s_tmem = reinterpret_cast<uint32_t*>(s_mbar + kMaxG);
+  const int wgi = threadIdx.x / kRows, warp = threadIdx.x >> 5;
+  WgCtx c;
+  c.t = threadIdx.x % kRows;
+  c.bar_id = 1 + wgi;
+  if (warp == 0) {
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(s_tmem)), "r"(512u) : "memory");
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+  }
+  if (threadIdx.x < G) asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(smem_u32(s_mbar + threadIdx.x)) : "memory");
+  if (threadIdx.x == 0) asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+  {
+    const uint4* src = reinterpret_cast<const uint4*>(wtiles);
+    uint4* dst = reinterpret_cast<uint4*>(s_tiles);
+    for (int i = threadIdx.x; i < kHiTileBytes / 16; i += kRows * G) dst[i] = __ldg(src + i);
+  }
+  asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
+  fence_before();
+  __syncthreads();
+  fence_after();
+  c.tmem = *s_tmem + CL::stride * wgi;
+  c.lane = (uint32_t)((warp & 3) * 32) << 16;
+  c.mbar = smem_u32(s_mbar + wgi);
+  c.phase = 0;
+  c.tile0 = smem_u32(s_tiles);
+  c.lo_off = 0;
+  const uint32_t tA = c.tmem + c.lane, tD = c.tmem + c.lane + CL::d;
+  restore_one<0, G>(c);
+  wait_st();
+  float4* Ps4 = s_P + (size_t)wgi * (kH / 4) * kRows + c.t;
+  const unsigned long long ntiles = (N + kRows - 1) / kRows;
+  for (unsigned long long tile = (unsigned long long)blockIdx.x * G + wgi; tile < ntiles; tile += (unsigned long long)gridDim.x * G) {
+    const unsigned long long i_raw = tile * kRows + c.t;
+    const bool valid = i_raw < N;
+    const unsigned long long i = valid ? i_raw : N - 1;
+    const float px = __ldg(x + 3 * i), py = __ldg(x + 3 * i + 1), pz = __ldg(x + 3 * i + 2);
+    encode_split_to<F16TAB, 4>(tA, g, px, py, pz);
+    issue_layer<0, G>(c, 0, 0, 2, true, 0, 2);                        // P = W1f f + b1, split-precision f
+    wait_layer(c);
+    store_D_f4(tD, Ps4);
+    for (uint32_t sidx = 0; sidx < ds.S; ++sidx) {
+      const float* dp = dir_of(ds, i, sidx);
+      const float wx = __ldg(dp), wy = __ldg(dp + 1), wz = __ldg(dp + 2);
+      h1_dir<false>(tA, cw, [&](int q) { return Ps4[q * kRows]; }, wx, wy, wz);
+      issue_layer<0, G>(c, 0, 2, 4, false, 0, 3);
+      wait_layer(c);
+      float zv, zt, v, t;
+      epi_precise<false>(tD, cw, zv, zt);
+      irt_maps(sp, zv, zt, v, t);
+      if (valid) {
+        const unsigned long long o = i * ds.S + sidx;
+        vis[o] = v; to[o] = t;
+        if (zvo) zvo[o] = zv;
+        if (xsec) { xsec[o * 3] = sec_hit(px, t, wx); xsec[o * 3 + 1] = sec_hit(py, t, wy); xsec[o * 3 + 2] = sec_hit(pz, t, wz); }
+      }
+    }
+  }
+  fence_before();
+  __syncthreads();
+  if (warp == 0) {
+    fence_after();
+    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(*s_tmem), "r"(512u) : "memory");
+  }
+}
+
+template <bool F16TAB>
+inline cudaError_t launch_trace_one(const GridP& g, const ShadeP& sp, const TcConst& cw, const uint8_t* d_tiles, const float* x,
+                                    unsigned long long N, const DirsetP& ds, float* vis, float* zv, float* t, float* xsec, int num_sms,
+                                    cudaStream_t st) {
+  static bool attr_done = false;
+  auto kern = k_trace_wg<F16TAB>;
+  if (!attr_done) {
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kTraceSmem);
+    if (e != cudaSuccess) return e;
+    attr_done = true;
+  }
+  const unsigned long long need = ((N + kRows - 1) / kRows + kTraceG - 1) / kTraceG;
+  const int grid = (int)(need < (unsigned long long)num_sms ? need : (unsigned long long)num_sms);
+  kern<<<grid, kRows * kTraceG, kTraceSmem, st>>>(g, sp, cw, d_tiles, x, N, ds, vis, zv, t, xsec);
+  return cudaGetLastError();
+}
+
 // ---------------------------------------------------------------------------------------------------- host side
 // Blob = [ TcConst | hi tiles (34 KB) | lo tiles (34 KB) ].  hi = fp16(w), lo = fp16(w - hi); bias K-steps only in the hi tiles.
 inline void prepare_weights(const hr_config& cfg, const float* bw, const float* iw, std::vector<uint8_t>& out) {

@@ -26,5 +26,10 @@ cudaError_t launch_p0(bool f16tab, const GridP& g, const EnvP& env, const ShadeP
 cudaError_t launch_p1(bool f16tab, const GridP& g, const EnvP& env, const ShadeP& sp, const void* tc_const, const uint8_t* d_tiles,
                       const float* wts32, const FrameP& fr, float* rgb, void* ring, unsigned long long* counters, int num_sms, cudaStream_t st);
 
+// hashrender_trace with the encode fused, fp16 models (k_trace_wg)
+cudaError_t launch_trace_p0(bool f16tab, const GridP& g, const ShadeP& sp, const void* tc_const, const uint8_t* d_tiles, const float* x,
+                            unsigned long long N, const DirsetP& ds, float* vis, float* zv, float* t, float* xsec, int num_sms,
+                            cudaStream_t st);
+
 }  // namespace wg
 }  // namespace hr

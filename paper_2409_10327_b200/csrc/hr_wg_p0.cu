@@ -31,5 +31,13 @@ cudaError_t launch_p0(bool f16tab, const GridP& g, const EnvP& env, const ShadeP
   return launch_one<false, 0, false, 2>(g, env, sp, cw, d_tiles, wts32, fr, rgb, rg, counters, num_sms, st);
 }
 
+cudaError_t launch_trace_p0(bool f16tab, const GridP& g, const ShadeP& sp, const void* tc_const, const uint8_t* d_tiles, const float* x,
+                            unsigned long long N, const DirsetP& ds, float* vis, float* zv, float* t, float* xsec, int num_sms,
+                            cudaStream_t st) {
+  const TcConst& cw = *reinterpret_cast<const TcConst*>(tc_const);
+  if (f16tab) return launch_trace_one<true>(g, sp, cw, d_tiles, x, N, ds, vis, zv, t, xsec, num_sms, st);
+  return launch_trace_one<false>(g, sp, cw, d_tiles, x, N, ds, vis, zv, t, xsec, num_sms, st);
+}
+
 }  // namespace wg
 }  // namespace hr
