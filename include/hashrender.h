@@ -18,8 +18,8 @@
  *    synchronises except hashrender_create, hashrender_destroy and hashrender_render_frame_host.
  *  - Outputs are caller-allocated.  The library neither frees nor keeps caller memory after a call
  *    returns; hashrender_create COPIES (and re-lays-out / converts) tables and weights.
- *  - No allocation after create, except hashrender_render_frame_host's staging buffers (grown on demand,
- *    released by destroy).
+ *  - No allocation after create, except hashrender_render_frame_host's staging buffers, copy stream and events
+ *    (created / grown on demand, released by destroy).
  *  - Arrays are row-major, innermost index last; float = IEEE binary32.  Directions and w_o are assumed
  *    unit length (not re-normalised).  Positions outside [0,1]^3 are clamped per component (Q6).
  *  - N == 0 is a no-op returning HR_OK.  NULL handle / NULL required pointer / S == 0 where a set is
@@ -126,7 +126,8 @@ int hashrender_shade(hashrender_t* h, const float* brdf, const float* wo, uint64
 int hashrender_render_frame(hashrender_t* h, const hr_frame* frame, float* rgb, void* stream);
 
 /* Same as hashrender_render_frame but EVERY pointer in `frame` and `rgb` is a HOST pointer (pinned memory
- * recommended): copies inputs host->device, renders, copies rgb device->host, synchronises `stream`.
+ * recommended): copies inputs host->device, renders, copies rgb device->host, synchronises `stream`.  Large frames are
+ * cut into row chunks whose copies (on an internal stream) overlap the previous chunk's render.
  * h2d_bytes / d2h_bytes (nullable) receive the bytes moved. */
 int hashrender_render_frame_host(hashrender_t* h, const hr_frame* frame, float* rgb, void* stream,
                                  uint64_t* h2d_bytes, uint64_t* d2h_bytes);

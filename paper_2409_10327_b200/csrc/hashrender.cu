@@ -37,6 +37,8 @@ struct hashrender {
   // staging for render_frame_host
   void* stage[16] = {nullptr};
   size_t stage_cap[16] = {0};
+  cudaStream_t copy_stream = nullptr;   // render_frame_host: H2D copies of chunk c+1 overlap the render of chunk c
+  cudaEvent_t ev[9] = {nullptr};
   int force_path = 0;            // 0 auto, 1 ffma  (env HASHRENDER_PATH=ffma, for A/B tests)
 };
 
@@ -241,6 +243,10 @@ int hashrender_destroy(hashrender_t* h) {
   cudaDeviceSynchronize();
   cudaFree(h->d_tables); cudaFree(h->d_wts); cudaFree(h->d_wts_tc); cudaFree(h->d_env);
   cudaFree(h->d_ring); cudaFree(h->d_counters);
+  if (h->copy_stream) {
+    cudaStreamDestroy(h->copy_stream);
+    for (int i = 0; i < 9; ++i) cudaEventDestroy(h->ev[i]);
+  }
   for (int i = 0; i < 16; ++i) cudaFree(h->stage[i]);
   delete h;
   return HR_OK;
@@ -379,6 +385,8 @@ int hashrender_render_frame(hashrender_t* h, const hr_frame* f, float* rgb, void
   return HR_OK;
 }
 
+// Host-buffer variant.  The frame is cut into up to 8 row chunks: chunk c+1 is copied host->device on an internal copy stream
+// while chunk c renders on the caller's stream, so the end-to-end time is max(copy, render) instead of their sum.
 int hashrender_render_frame_host(hashrender_t* h, const hr_frame* f, float* rgb, void* stream, uint64_t* h2d_bytes, uint64_t* d2h_bytes) {
   if (!h) return HR_ERR_INVALID_ARG;
   if (h2d_bytes) *h2d_bytes = 0;
@@ -386,54 +394,107 @@ int hashrender_render_frame_host(hashrender_t* h, const hr_frame* f, float* rgb,
   if (int e = check_frame(h, f, rgb)) return e;
   if (f->N == 0) return HR_OK;
   cudaStream_t st = (cudaStream_t)stream;
+  if (!h->copy_stream) {
+    HR_CUDA(h, cudaStreamCreateWithFlags(&h->copy_stream, cudaStreamNonBlocking));
+    for (int i = 0; i < 9; ++i) HR_CUDA(h, cudaEventCreateWithFlags(&h->ev[i], cudaEventDisableTiming));
+  }
+  const uint64_t N = f->N;
+  const uint64_t wave = (uint64_t)h->num_sms * 4 * 128;              // pixels one pass of the render kernel's warpgroups covers
+  int nchunks = (int)(N / (2 * wave));
+  nchunks = nchunks < 1 ? 1 : (nchunks > 8 ? 8 : nchunks);
+  const uint64_t rows_per = ((N + nchunks - 1) / nchunks + 127) / 128 * 128;
+
+  // one entry per array that travels: `rows` rows of `row_elems` elements (the last row holds `last_elems`), elem bytes
+  struct Arr { const char* src; char* dst; uint64_t rows, row_bytes, last_bytes, per_point; };
+  Arr arr[16];
+  int na = 0, slot = 0;
   uint64_t up = 0;
-  int slot = 0;
-  int rc = HR_OK;
-  auto stage = [&](const void* src, size_t bytes) -> const void* {
-    if (!src || rc != HR_OK) return nullptr;
-    const int s = slot++;
+  auto ensure = [&](int s, size_t bytes) -> char* {
     if (bytes > h->stage_cap[s]) {
       cudaFree(h->stage[s]); h->stage[s] = nullptr; h->stage_cap[s] = 0;
-      cudaError_t e = cudaMalloc(&h->stage[s], bytes);
-      if (e != cudaSuccess) { rc = fail(h, HR_ERR_OOM, "render_frame_host: staging alloc of %zu bytes failed", bytes); return nullptr; }
+      if (cudaMalloc(&h->stage[s], bytes) != cudaSuccess) return nullptr;
       h->stage_cap[s] = bytes;
     }
-    cudaError_t e = cudaMemcpyAsync(h->stage[s], src, bytes, cudaMemcpyHostToDevice, st);
-    if (e != cudaSuccess) { rc = fail(h, HR_ERR_CUDA, "render_frame_host: H2D failed: %s", cudaGetErrorString(e)); return nullptr; }
-    up += bytes;
-    return h->stage[s];
+    return (char*)h->stage[s];
   };
-  auto stage_set = [&](const hr_dirset& d, uint64_t rows, bool used) -> hr_dirset {
+  bool oom = false;
+  // per_point = rows of this array per primary point (S_i for per-secondary-point tertiary sets, else 1; 0 = shared, copied once)
+  auto add = [&](const void* src, uint64_t rows, uint64_t row_bytes, uint64_t last_bytes, uint64_t per_point) -> const void* {
+    const int s = slot++;
+    if (!src) return nullptr;
+    const uint64_t total = (rows - 1) * row_bytes + last_bytes;
+    char* d = ensure(s, total);
+    if (!d) { oom = true; return nullptr; }
+    arr[na++] = Arr{(const char*)src, d, rows, row_bytes, last_bytes, per_point};
+    up += total;
+    return d;
+  };
+  auto add_set = [&](const hr_dirset& d, uint64_t rows, uint64_t per_point, bool used) -> hr_dirset {
     hr_dirset o = d;
     if (!used) { slot += 3; return o; }
-    const uint64_t R = d.point_stride ? rows : 1;
-    const uint64_t dir_elems = d.point_stride ? (R - 1) * d.point_stride + 3ull * d.S : 3ull * d.S;
-    const uint64_t pdf_elems = d.point_stride ? (R - 1) * (d.point_stride / 3) + d.S : d.S;
-    o.dir = (const float*)stage(d.dir, dir_elems * 4);
-    o.pdf = (const float*)stage(d.pdf, pdf_elems * 4);
-    if (d.Lin) o.Lin = (const float*)stage(d.Lin, dir_elems * 4); else slot++;
+    if (d.point_stride) {
+      o.dir = (const float*)add(d.dir, rows, d.point_stride * 4, 12ull * d.S, per_point);
+      o.pdf = (const float*)add(d.pdf, rows, d.point_stride / 3 * 4, 4ull * d.S, per_point);
+      o.Lin = (const float*)add(d.Lin, rows, d.point_stride * 4, 12ull * d.S, per_point);
+    } else {
+      o.dir = (const float*)add(d.dir, 1, 0, 12ull * d.S, 0);
+      o.pdf = (const float*)add(d.pdf, 1, 0, 4ull * d.S, 0);
+      o.Lin = (const float*)add(d.Lin, 1, 0, 12ull * d.S, 0);
+    }
     return o;
   };
   hr_frame df = *f;
-  df.x = (const float*)stage(f->x, f->N * 12);
-  if (f->brdf) df.brdf = (const float*)stage(f->brdf, f->N * 28); else slot++;
-  df.wo = (const float*)stage(f->wo, f->N * 12);
-  if (f->mask) df.mask = (const uint8_t*)stage(f->mask, f->N); else slot++;
-  df.direct = stage_set(f->direct, f->N, f->flags & HR_DIRECT);
-  df.secondary = stage_set(f->secondary, f->N, f->flags & HR_INDIRECT);
-  df.tertiary = stage_set(f->tertiary, f->N * (uint64_t)f->secondary.S, f->flags & HR_INDIRECT);
-  if (rc != HR_OK) return rc;
-  const int s_rgb = 15;
-  if (f->N * 12 > h->stage_cap[s_rgb]) {
-    cudaFree(h->stage[s_rgb]); h->stage[s_rgb] = nullptr; h->stage_cap[s_rgb] = 0;
-    HR_CUDA(h, cudaMalloc(&h->stage[s_rgb], f->N * 12));
-    h->stage_cap[s_rgb] = f->N * 12;
+  df.x = (const float*)add(f->x, N, 12, 12, 1);
+  df.brdf = (const float*)add(f->brdf, N, 28, 28, 1);
+  df.wo = (const float*)add(f->wo, N, 12, 12, 1);
+  df.mask = (const uint8_t*)add(f->mask, N, 1, 1, 1);
+  df.direct = add_set(f->direct, N, 1, f->flags & HR_DIRECT);
+  df.secondary = add_set(f->secondary, N, 1, f->flags & HR_INDIRECT);
+  df.tertiary = add_set(f->tertiary, N * (uint64_t)f->secondary.S, f->secondary.S, f->flags & HR_INDIRECT);
+  float* d_rgb = (float*)ensure(15, N * 12);
+  if (oom || !d_rgb) return fail(h, HR_ERR_OOM, "render_frame_host: staging allocation failed");
+
+  // the copy stream must not overwrite staging buffers an earlier call on `st` may still be reading
+  HR_CUDA(h, cudaEventRecord(h->ev[8], st));
+  HR_CUDA(h, cudaStreamWaitEvent(h->copy_stream, h->ev[8], 0));
+  for (int c = 0; c < nchunks; ++c) {
+    const uint64_t p0 = (uint64_t)c * rows_per, p1 = p0 + rows_per < N ? p0 + rows_per : N;
+    if (p0 >= N) { nchunks = c; break; }
+    for (int k = 0; k < na; ++k) {
+      const Arr& a = arr[k];
+      if (a.per_point == 0) {                                         // shared set: once, with the first chunk
+        if (c == 0) HR_CUDA(h, cudaMemcpyAsync(a.dst, a.src, a.last_bytes, cudaMemcpyHostToDevice, h->copy_stream));
+        continue;
+      }
+      const uint64_t r0 = p0 * a.per_point, r1 = p1 * a.per_point;
+      const uint64_t bytes = r1 == a.rows ? (r1 - 1 - r0) * a.row_bytes + a.last_bytes : (r1 - r0) * a.row_bytes;
+      HR_CUDA(h, cudaMemcpyAsync(a.dst + r0 * a.row_bytes, a.src + r0 * a.row_bytes, bytes, cudaMemcpyHostToDevice, h->copy_stream));
+    }
+    HR_CUDA(h, cudaEventRecord(h->ev[c], h->copy_stream));
   }
-  if (int e = hashrender_render_frame(h, &df, (float*)h->stage[s_rgb], stream)) return e;
-  HR_CUDA(h, cudaMemcpyAsync(rgb, h->stage[s_rgb], f->N * 12, cudaMemcpyDeviceToHost, st));
+  for (int c = 0; c < nchunks; ++c) {
+    const uint64_t p0 = (uint64_t)c * rows_per, p1 = p0 + rows_per < N ? p0 + rows_per : N;
+    hr_frame cf = df;
+    cf.N = p1 - p0;
+    cf.x = df.x + 3 * p0;
+    cf.wo = df.wo + 3 * p0;
+    if (df.brdf) cf.brdf = df.brdf + 7 * p0;
+    if (df.mask) cf.mask = df.mask + p0;
+    auto off = [&](hr_dirset& d, uint64_t r0) {
+      if (!d.point_stride) return;
+      if (d.dir) d.dir += r0 * d.point_stride;
+      if (d.pdf) d.pdf += r0 * (d.point_stride / 3);
+      if (d.Lin) d.Lin += r0 * d.point_stride;
+    };
+    if (f->flags & HR_DIRECT) off(cf.direct, p0);
+    if (f->flags & HR_INDIRECT) { off(cf.secondary, p0); off(cf.tertiary, p0 * (uint64_t)f->secondary.S); }
+    HR_CUDA(h, cudaStreamWaitEvent(st, h->ev[c], 0));
+    if (int e = hashrender_render_frame(h, &cf, d_rgb + 3 * p0, stream)) return e;
+  }
+  HR_CUDA(h, cudaMemcpyAsync(rgb, d_rgb, N * 12, cudaMemcpyDeviceToHost, st));
   HR_CUDA(h, cudaStreamSynchronize(st));
   if (h2d_bytes) *h2d_bytes = up;
-  if (d2h_bytes) *d2h_bytes = f->N * 12;
+  if (d2h_bytes) *d2h_bytes = N * 12;
   return HR_OK;
 }
 

@@ -290,6 +290,22 @@ def test_compaction_equals_dense(torch, name):
     np.testing.assert_allclose(a0, b0, rtol=5e-6, atol=1e-7)
 
 
+def test_render_frame_host_chunked_pipeline(torch):
+    """render_frame_host cuts a large frame into row chunks whose H2D copies overlap the previous chunk's render; the result
+    must equal the one-launch device path (per-point direct / secondary sets, shared tertiary set, mask)."""
+    cfg = gen.make_config("C2", S_d=3, S_i=2, S_2=2)
+    m = gen.make_model(cfg)
+    fr = gen.make_frame(cfg, m["env"])
+    mask = (np.arange(cfg.N) % 7 != 0).astype(np.uint8)
+    r = make_renderer(cfg, m)
+    a = gpu_render(r, cfg, fr, mask=mask)
+    b = gpu_render(r, cfg, fr, mask=mask, host=True)
+    assert r.launch_count() >= 1 + 4                                  # 640 000 pixels -> 4 chunks on a 148-SM part
+    np.testing.assert_allclose(a, b, rtol=2e-6, atol=1e-7)
+    b2 = gpu_render(r, cfg, fr, mask=mask, host=True)                 # staging buffers are reused safely
+    np.testing.assert_allclose(a, b2, rtol=2e-6, atol=1e-7)
+
+
 def test_frame_errors(torch):
     from paper_2409_10327_b200 import DirSet, HashRenderError
     cfg = gen.make_config("C0")
