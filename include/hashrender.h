@@ -132,6 +132,20 @@ int hashrender_render_frame(hashrender_t* h, const hr_frame* frame, float* rgb, 
 int hashrender_render_frame_host(hashrender_t* h, const hr_frame* frame, float* rgb, void* stream,
                                  uint64_t* h2d_bytes, uint64_t* d2h_bytes);
 
+/* On-device direction sampler (the step before the hot path; Q35-Q38).
+ * sample_mis: per point i and sample s < spp, slot 2s = a light-importance ray (env-map luminance * sin(theta), stratified CDF
+ * inversion, jittered in the texel), slot 2s+1 = a GGX visible-normal ray (alpha = roughness^2) about the normal of brdf[i]
+ * ([N,7] = n a r, post-activation) for the view direction wo[i]; every ray carries the balance-heuristic pdf
+ * (p_light + p_ggx) / 2, so the set plugs into hr_dirset with S = 2 spp.  dir [N, 2 spp, 3], pdf [N, 2 spp].  Needs set_env; the
+ * first call after set_env builds the light tables on the host (synchronises `stream` once).  A pure function of
+ * (env, brdf, wo, spp, seed): the generator is counter-based.
+ * sample_stratified: Sa x Sb jittered strata per row, slot a*Sb + b; normal [rows,3] != NULL: cosine-weighted hemisphere about
+ * normal[row] (pdf cos/pi); NULL: whole sphere (pdf 1/4pi).  dir [rows, Sa*Sb, 3], pdf [rows, Sa*Sb]. */
+int hashrender_sample_mis(hashrender_t* h, const float* brdf, const float* wo, uint64_t N, uint32_t spp, uint64_t seed, float* dir,
+                          float* pdf, void* stream);
+int hashrender_sample_stratified(hashrender_t* h, const float* normal, uint64_t rows, uint32_t Sa, uint32_t Sb, uint64_t seed,
+                                 float* dir, float* pdf, void* stream);
+
 /* Secondary-ray accounting of the render_frame calls since the last reset: rays_traced = secondary
  * (point, direction) rays whose (v, t) were evaluated, rays_evaluated = those whose L'_o was evaluated (all of them with
  * HR_DENSE).  Both nullable.  Synchronises the device.  Only the tcgen05 paths count; the FFMA path leaves both at 0. */

@@ -16,7 +16,7 @@ _LIB_PATH = os.path.join(os.path.dirname(os.path.abspath(__file__)), "libhashren
 
 EXPORTS = ["hashrender_create", "hashrender_destroy", "hashrender_set_env", "hashrender_encode", "hashrender_decode",
            "hashrender_trace", "hashrender_shade", "hashrender_render_frame", "hashrender_render_frame_host",
-           "hashrender_stats", "hashrender_launch_count", "hashrender_last_path", "hashrender_last_error"]
+           "hashrender_sample_mis", "hashrender_sample_stratified", "hashrender_stats", "hashrender_launch_count", "hashrender_last_path", "hashrender_last_error"]
 
 
 class HashRenderError(RuntimeError):
@@ -64,6 +64,8 @@ def load_library(path: str | None = None):
         lib.hashrender_shade.argtypes = [vp, vp, vp, u64, C.POINTER(hr_dirset), vp, vp, u32, vp, vp]
         lib.hashrender_render_frame.argtypes = [vp, C.POINTER(hr_frame), vp, vp]
         lib.hashrender_render_frame_host.argtypes = [vp, C.POINTER(hr_frame), vp, vp, C.POINTER(u64), C.POINTER(u64)]
+        lib.hashrender_sample_mis.argtypes = [vp, vp, vp, u64, u32, u64, vp, vp, vp]
+        lib.hashrender_sample_stratified.argtypes = [vp, vp, u64, u32, u32, u64, vp, vp, vp]
         lib.hashrender_stats.argtypes = [vp, C.POINTER(u64), C.POINTER(u64), C.c_int]
         lib.hashrender_launch_count.argtypes = [vp]
         lib.hashrender_launch_count.restype = u64
@@ -190,6 +192,12 @@ class HashRenderer:
         up, down = C.c_uint64(), C.c_uint64()
         self._check(self._lib.hashrender_render_frame_host(self._h, C.byref(frame), _ptr(rgb), stream, C.byref(up), C.byref(down)))
         return up.value, down.value
+
+    def sample_mis(self, brdf, wo, spp, seed, dir, pdf, stream=None):
+        self._check(self._lib.hashrender_sample_mis(self._h, _ptr(brdf), _ptr(wo), brdf.shape[0], spp, seed, _ptr(dir), _ptr(pdf), stream))
+
+    def sample_stratified(self, normal, rows, Sa, Sb, seed, dir, pdf, stream=None):
+        self._check(self._lib.hashrender_sample_stratified(self._h, _ptr(normal), rows, Sa, Sb, seed, _ptr(dir), _ptr(pdf), stream))
 
     def stats(self, reset=False):
         """(secondary rays traced, secondary rays whose L'_o was evaluated) since the last reset."""

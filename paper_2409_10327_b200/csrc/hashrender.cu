@@ -4,6 +4,7 @@
 
 #include <cstdarg>
 #include <cstdio>
+#include <cmath>
 #include <cstring>
 #include <new>
 #include <vector>
@@ -11,6 +12,7 @@
 #include "../../include/hashrender.h"
 #include "hr_kernels_ffma.cuh"
 #include "hr_kernels_tc.cuh"
+#include "hr_sampler.cuh"
 #include "hr_wg_api.h"
 
 using namespace hr;
@@ -37,6 +39,9 @@ struct hashrender {
   // staging for render_frame_host
   void* stage[16] = {nullptr};
   size_t stage_cap[16] = {0};
+  float* d_light = nullptr;      // sampler tables: pmf [He*We] then cdf [He*We] (built lazily from the env map)
+  size_t light_cap = 0;
+  bool light_valid = false;
   cudaStream_t copy_stream = nullptr;   // render_frame_host: H2D copies of chunk c+1 overlap the render of chunk c
   cudaEvent_t ev[9] = {nullptr};
   int force_path = 0;            // 0 auto, 1 ffma  (env HASHRENDER_PATH=ffma, for A/B tests)
@@ -242,7 +247,7 @@ int hashrender_destroy(hashrender_t* h) {
   if (!h) return HR_ERR_INVALID_ARG;
   cudaDeviceSynchronize();
   cudaFree(h->d_tables); cudaFree(h->d_wts); cudaFree(h->d_wts_tc); cudaFree(h->d_env);
-  cudaFree(h->d_ring); cudaFree(h->d_counters);
+  cudaFree(h->d_ring); cudaFree(h->d_counters); cudaFree(h->d_light);
   if (h->copy_stream) {
     cudaStreamDestroy(h->copy_stream);
     for (int i = 0; i < 9; ++i) cudaEventDestroy(h->ev[i]);
@@ -263,6 +268,7 @@ int hashrender_set_env(hashrender_t* h, const float* env, uint32_t He, uint32_t 
   }
   HR_CUDA(h, cudaMemcpyAsync(h->d_env, env, bytes, cudaMemcpyDeviceToDevice, (cudaStream_t)stream));
   h->env.env = h->d_env; h->env.He = He; h->env.We = We;
+  h->light_valid = false;
   return HR_OK;
 }
 
@@ -495,6 +501,75 @@ int hashrender_render_frame_host(hashrender_t* h, const hr_frame* f, float* rgb,
   HR_CUDA(h, cudaStreamSynchronize(st));
   if (h2d_bytes) *h2d_bytes = up;
   if (d2h_bytes) *d2h_bytes = N * 12;
+  return HR_OK;
+}
+
+// Light-importance tables of the current env map (Q37): pmf over texels ~ luminance * sin(theta of the row centre), and
+// its running sum rounded to fp32.  Built on the host in double (the map is a few KB), once per set_env.  Synchronises.
+static int build_light_tables(hashrender* h, cudaStream_t st) {
+  if (h->light_valid) return HR_OK;
+  if (!h->env.env) return fail(h, HR_ERR_INVALID_ARG, "sample_mis: no env map set");
+  const uint32_t He = h->env.He, We = h->env.We;
+  const size_t n = (size_t)He * We;
+  std::vector<float> env(n * 3), tab(2 * n);
+  HR_CUDA(h, cudaStreamSynchronize(st));
+  HR_CUDA(h, cudaMemcpy(env.data(), h->d_env, n * 12, cudaMemcpyDeviceToHost));
+  std::vector<double> w(n);
+  double tot = 0.0;
+  for (uint32_t r = 0; r < He; ++r) {
+    const double st_ = sin(3.14159265358979323846 * (r + 0.5) / He);
+    for (uint32_t c = 0; c < We; ++c) {
+      const float* p = &env[((size_t)r * We + c) * 3];
+      const double Y = 0.2126 * (double)p[0] + 0.7152 * (double)p[1] + 0.0722 * (double)p[2];
+      w[(size_t)r * We + c] = (Y > 0.0 ? Y : 0.0) * st_;
+      tot += w[(size_t)r * We + c];
+    }
+  }
+  if (!(tot > 0.0)) {
+    tot = 0.0;
+    for (uint32_t r = 0; r < He; ++r)
+      for (uint32_t c = 0; c < We; ++c) { w[(size_t)r * We + c] = sin(3.14159265358979323846 * (r + 0.5) / He); tot += w[(size_t)r * We + c]; }
+  }
+  double run = 0.0;
+  for (size_t k = 0; k < n; ++k) { const double q = w[k] / tot; run += q; tab[k] = (float)q; tab[n + k] = (float)run; }
+  tab[2 * n - 1] = 1.0f;
+  if (2 * n * 4 > h->light_cap) {
+    cudaFree(h->d_light); h->d_light = nullptr; h->light_cap = 0;
+    HR_CUDA(h, cudaMalloc(&h->d_light, 2 * n * 4));
+    h->light_cap = 2 * n * 4;
+  }
+  HR_CUDA(h, cudaMemcpy(h->d_light, tab.data(), 2 * n * 4, cudaMemcpyHostToDevice));
+  h->light_valid = true;
+  return HR_OK;
+}
+
+int hashrender_sample_mis(hashrender_t* h, const float* brdf, const float* wo, uint64_t N, uint32_t spp, uint64_t seed, float* dir, float* pdf,
+                          void* stream) {
+  if (!h) return HR_ERR_INVALID_ARG;
+  if (N == 0) return HR_OK;
+  if (!brdf || !wo || !dir || !pdf || spp == 0) return fail(h, HR_ERR_INVALID_ARG, "sample_mis: NULL brdf / wo / dir / pdf or spp == 0");
+  if (N > h->cfg.max_points) return fail(h, HR_ERR_INVALID_ARG, "sample_mis: N exceeds max_points");
+  if (int e = build_light_tables(h, (cudaStream_t)stream)) return e;
+  smp::LightP lp;
+  lp.pmf = h->d_light; lp.cdf = h->d_light + (size_t)h->env.He * h->env.We; lp.He = h->env.He; lp.We = h->env.We;
+  const uint64_t total = N * spp;
+  const uint64_t need = (total + 255) / 256, cap = (uint64_t)h->num_sms * 16;
+  smp::k_sample_mis<<<(int)(need < cap ? need : cap), 256, 0, (cudaStream_t)stream>>>(lp, brdf, wo, N, spp, seed, dir, pdf);
+  h->launches++;
+  HR_CUDA(h, cudaGetLastError());
+  return HR_OK;
+}
+
+int hashrender_sample_stratified(hashrender_t* h, const float* normal, uint64_t rows, uint32_t Sa, uint32_t Sb, uint64_t seed, float* dir,
+                                 float* pdf, void* stream) {
+  if (!h) return HR_ERR_INVALID_ARG;
+  if (rows == 0) return HR_OK;
+  if (!dir || !pdf || Sa == 0 || Sb == 0) return fail(h, HR_ERR_INVALID_ARG, "sample_stratified: NULL dir / pdf or empty strata");
+  const uint64_t total = rows * Sa * Sb;
+  const uint64_t need = (total + 255) / 256, cap = (uint64_t)h->num_sms * 16;
+  smp::k_sample_stratified<<<(int)(need < cap ? need : cap), 256, 0, (cudaStream_t)stream>>>(normal, rows, Sa, Sb, seed, dir, pdf);
+  h->launches++;
+  HR_CUDA(h, cudaGetLastError());
   return HR_OK;
 }
 
