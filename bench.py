@@ -235,7 +235,7 @@ def main():
     from paper_2409_10327_b200 import DirSet, HashRenderer
     from paper_2409_10327_b200 import dist as hd
 
-    def measure(cfg, steps, warmup, e2e_steps, clocks, dense=True):
+    def measure(cfg, steps, warmup, e2e_steps, clocks, dense=True, sampled=False):
         model = gen.make_model(cfg)
         fr = gen.make_frame(cfg, model["env"])
         r = HashRenderer.from_gen(cfg, model, vis_mode=args.vis_mode)
@@ -298,6 +298,47 @@ def main():
             torch.cuda.synchronize()
             out.update(e2e_ms=hd.max_over_ranks(e0.elapsed_time(e1), dev) / e2e_steps, h2d=upb, d2h=downb,
                        e2e_matches=bool(np.allclose(hrgb, rgb.cpu().numpy(), rtol=1e-5, atol=1e-6)))
+        # end to end with the directions generated ON the device: only x, wo travel host->device; the primary
+        # BRDF is decoded (encode + decode), the direct set is the MIS light + GGX set of PAPER.md:122 (spp = S_d / 2), the
+        # secondary set a stratified cosine hemisphere about the decoded normal, the tertiary set a shared stratified sphere
+        if e2e_steps and sampled:
+            import math
+            hx, hwo = torch.from_numpy(fr["x"]).pin_memory(), torch.from_numpy(fr["wo"]).pin_memory()
+            hrgb = torch.empty((cfg.N, 3), dtype=torch.float32).pin_memory()
+            N = cfg.N
+            feat = torch.empty((N, cfg.D), device=dev); brdf = torch.empty((N, 7), device=dev)
+            dd = torch.empty((N, cfg.S_d, 3), device=dev); pd = torch.empty((N, cfg.S_d), device=dev)
+            sa = int(math.isqrt(cfg.S_i)) if indirect else 0
+            if indirect:
+                ds_ = torch.empty((N, sa * sa, 3), device=dev); ps_ = torch.empty((N, sa * sa), device=dev)
+                ta, tb = (cfg.S_2 // 2, 2) if cfg.S_2 % 2 == 0 else (cfg.S_2, 1)
+                dt_ = torch.empty((ta * tb, 3), device=dev); pt_ = torch.empty((ta * tb,), device=dev)
+
+            def sampled_frame():
+                xd = hx.to(dev, non_blocking=True); wod = hwo.to(dev, non_blocking=True)
+                r.encode(xd, feat, stream=stream)
+                r.decode(feat, brdf, stream=stream)
+                r.sample_mis(brdf, wod, cfg.S_d // 2, 2409, dd, pd, stream=stream)
+                sset = tset = None
+                if indirect:
+                    nrm = brdf[:, :3].contiguous()
+                    r.sample_stratified(nrm, N, sa, sa, 10327, ds_, ps_, stream=stream)
+                    r.sample_stratified(None, 1, ta, tb, 7, dt_, pt_, stream=stream)
+                    sset, tset = DirSet(ds_, ps_), DirSet(dt_, pt_)
+                fq = r.make_frame(xd, wod, DirSet(dd, pd), sset, tset, flags=flags)
+                r.render_frame(fq, rgb, stream)
+                hrgb.copy_(rgb, non_blocking=True)
+                torch.cuda.synchronize()
+
+            sampled_frame()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            for _ in range(e2e_steps):
+                sampled_frame()
+            e1.record()
+            torch.cuda.synchronize()
+            out.update(e2e_sampled_ms=e0.elapsed_time(e1) / e2e_steps, e2e_sampled_h2d=int(hx.numel() + hwo.numel()) * 4,
+                       e2e_sampled_finite=bool(torch.isfinite(hrgb).all()), e2e_sampled_mean=float(hrgb.mean()))
         r.destroy()
         del x, wo, d, s, t, rgb
         torch.cuda.empty_cache()
@@ -305,7 +346,7 @@ def main():
 
     peaks = load_peaks()
     clocks = ClockSampler(local) if rank == 0 else None
-    res, model = measure(cfg, args.steps, max(args.warmup, 3), args.e2e_steps, clocks, dense=not args.compact)
+    res, model = measure(cfg, args.steps, max(args.warmup, 3), args.e2e_steps, clocks, dense=not args.compact, sampled=world == 1)
 
     if rank != 0:
         if world > 1:
@@ -359,6 +400,11 @@ def main():
     if "e2e_ms" in res:
         line["e2e"] = {"value": world * cfg.queries / (res["e2e_ms"] * 1e-3), "unit": UNIT, "ms_per_frame": res["e2e_ms"],
                        "h2d_bytes_per_step": res["h2d"], "d2h_bytes_per_step": res["d2h"], "matches_device_path": res["e2e_matches"]}
+    if "e2e_sampled_ms" in res:
+        line["e2e_sampled"] = {"value": cfg.queries / (res["e2e_sampled_ms"] * 1e-3), "unit": UNIT, "ms_per_frame": res["e2e_sampled_ms"],
+                               "h2d_bytes_per_step": res["e2e_sampled_h2d"], "d2h_bytes_per_step": cfg.N * 12, "finite": res["e2e_sampled_finite"],
+                               "what": "same frame shape, but only x and wo travel: B(H(x)) is decoded and the direction sets are generated on the "
+                                       "device (hashrender_encode/decode/sample_mis/sample_stratified/render_frame); PAPER.md:122, 344"}
     if world == 1 and not args.no_extra:
         # the same frame with the default API flags (zero-weight secondary rays compacted out), and the
         # other precision; `value` here is frame-equivalent (queries_per_frame / time), executed queries are stated
