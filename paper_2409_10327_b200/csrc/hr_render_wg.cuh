@@ -49,15 +49,14 @@ static_assert(sizeof(Item) == 48, "Item is three 16-byte words");
 
 template <int PREC, int G> struct Cols {
   static_assert(G >= 1 && G <= kMaxG, "1..4 warpgroups");
-  static_assert(PREC == 0 || G <= 3, "split precision needs 144 TMEM columns per warpgroup");
-  static constexpr uint32_t stride = G == 4 ? 128u : (G == 3 ? 168u : (G == 2 ? 256u : 512u));
-  // A = columns 0..63 (fp16 pairs; hi | lo for the split layers), D = 64 fp32 accumulator columns, and the constant bias
-  // K-step of A, [1, 1, 0 .. 0].  With 128 columns per warpgroup (G = 4) the bias step shares columns 32..39 with the lo
-  // half of A: K = 64 split layers then add their bias in the fp32 epilogue and rewrite the step afterwards.
-  static constexpr bool bias64 = stride >= 144u;
-  static constexpr uint32_t one = bias64 ? 64u : 32u;
-  static constexpr uint32_t d = bias64 ? 80u : 64u;
+    static constexpr uint32_t stride = G == 4 ? 128u : (G == 3 ? 168u : (G == 2 ? 256u : 512u));
+  // A = columns 0..63 (fp16 pairs): hi | lo for the split layers, or two 32-column buffers A0 | A1 that the fp16 query loops
+  // alternate between (the next query's h1 is written while the current MMA runs).  D = 64 fp32 accumulator columns.
+  // The constant operand of the bias K-steps, rows of [1, 1, 0 .. 0], lives in SHARED memory (kOnesBytes of identical
+  // 16-byte chunks, so the swizzle cannot matter), which leaves all 128 columns of a G = 4 warpgroup to A and D.
+  static constexpr uint32_t d = 64u;
 };
+constexpr int kOnesBytes = 128 * 128;         // a 128-row K-major SWIZZLE_128B tile of uniform chunks
 
 struct WgCtx {
   uint32_t tmem;      // TMEM address of the WG's column 0, lane 0
@@ -66,6 +65,7 @@ struct WgCtx {
   uint32_t phase;
   uint32_t tile0;     // shared address of the weight tiles
   uint32_t lo_off;    // byte offset of the lo tiles (PREC = 1)
+  uint32_t ones;      // shared address of the uniform bias operand
   int bar_id;         // named barrier of the WG
   int t;              // thread index in the WG
 };
@@ -87,27 +87,27 @@ __device__ __forceinline__ void issue_layer(const WgCtx& c, uint32_t a_col, int 
   wait_st();
   fence_before();
   wg_sync(c);
-  if (c.t == 0) {
+  if (c.t < 32) {                               // warp 0 of the warpgroup, converged; one elected lane issues
     fence_after();
     const uint32_t d = c.tmem + Cols<PREC, G>::d;
     const uint32_t a = c.tmem + a_col;
     const uint64_t bd = make_bdesc(c.tile0 + tile * kTileBytes);
-    for (int k = 0; k < ksteps; ++k) mma_f16_ts(d, a + 8 * k, bd + 2 * k, idesc, k > 0);
+    for (int k = 0; k < ksteps; ++k) mma_f16_ts_elect(d, a + 8 * k, bd + 2 * k, idesc, k > 0);
     if (split_a)
-      for (int k = 0; k < ksteps; ++k) mma_f16_ts(d, a + 8 * (ksteps + k), bd + 2 * k, idesc, 1u);
+      for (int k = 0; k < ksteps; ++k) mma_f16_ts_elect(d, a + 8 * (ksteps + k), bd + 2 * k, idesc, 1u);
     if (PREC == 1) {
       const uint64_t bl = make_bdesc(c.tile0 + c.lo_off + tile * kTileBytes);
-      for (int k = 0; k < ksteps; ++k) mma_f16_ts(d, a + 8 * k, bl + 2 * k, idesc, 1u);
+      for (int k = 0; k < ksteps; ++k) mma_f16_ts_elect(d, a + 8 * k, bl + 2 * k, idesc, 1u);
     }
-    if (bias_tile >= 0)
-      mma_f16_ts(d, c.tmem + Cols<PREC, G>::one, make_bdesc(c.tile0 + bias_tile * kTileBytes) + 2 * bias_kstep, idesc, 1u);
-    mma_commit(c.mbar);
+    if (bias_tile >= 0)          // D += [1,1,0..|1,1,0..] x K-step: columns 0,1 hold the bias hi/lo, columns 8,9 are zero
+      mma_f16_ss_elect(d, make_bdesc(c.ones), make_bdesc(c.tile0 + bias_tile * kTileBytes) + 2 * bias_kstep, idesc, 1u);
+    mma_commit_elect(c.mbar);
   }
 }
-template <int PREC, int G>
-__device__ __forceinline__ void restore_one(const WgCtx& c) {
-  const uint32_t one[8] = {0x3C003C00u, 0u, 0u, 0u, 0u, 0u, 0u, 0u};
-  tmem_st8(c.tmem + c.lane + Cols<PREC, G>::one, one);
+// every 16-byte chunk of the bias operand = fp16 [1, 1, 0, 0, 0, 0, 0, 0]
+__device__ __forceinline__ void fill_ones(uint8_t* s_ones, int nthreads) {
+  uint4* dst = reinterpret_cast<uint4*>(s_ones);
+  for (int i = threadIdx.x; i < kOnesBytes / 16; i += nthreads) dst[i] = make_uint4(0x3C003C00u, 0u, 0u, 0u);
 }
 __device__ __forceinline__ void wait_layer(WgCtx& c) {
   mbar_wait(c.mbar, c.phase);
@@ -359,8 +359,7 @@ __device__ __forceinline__ void brdf_primary(WgCtx& c, const TcConst& cw, const 
   issue_layer<PREC, G>(c, 0, 1, 2, true, 1, 2);
   wait_layer(c);
   hidden_to_A<true>(tD, tA);
-  constexpr bool bias64 = Cols<PREC, G>::bias64;
-  issue_layer<PREC, G>(c, 0, 3, 4, true, bias64 ? 1 : -1, 3);
+  issue_layer<PREC, G>(c, 0, 3, 4, true, 1, 3);
   wait_layer(c);
   float o[8];
 #pragma unroll
@@ -372,12 +371,11 @@ __device__ __forceinline__ void brdf_primary(WgCtx& c, const TcConst& cw, const 
     wait_ld();
 #pragma unroll
     for (int k = 0; k < 32; ++k) {
-      const float a = fmaxf(bias64 ? __uint_as_float(r[k]) : __uint_as_float(r[k]) + cw.Bb2[32 * h + k], 0.f);
+      const float a = fmaxf(__uint_as_float(r[k]), 0.f);
 #pragma unroll
       for (int q = 0; q < 7; ++q) o[q] = fmaf(a, cw.BW3[q][32 * h + k], o[q]);
     }
   }
-  if (!bias64) restore_one<PREC, G>(c);
   brdf_maps(sp, o, b);
 }
 
@@ -389,7 +387,7 @@ template <int PREC, bool TSHARED, int G> struct SmemPlan {
                                    + kRows * 4 * 4                                     // acc[128][4]
                                    + 64;                                               // queue head/tail, tile slot
   static constexpr size_t shared_set = (size_t)kMaxS2 * kH * 4 + kMaxS2 * 8 * 4;      // Qt, Lt
-  static constexpr size_t bytes = 1024 + tiles + G * per_wg + shared_set + 8 * kMaxG + 16;
+  static constexpr size_t bytes = 1024 + tiles + kOnesBytes + G * per_wg + shared_set + 8 * kMaxG + 16;
 };
 
 // ---------------------------------------------------------------------------------------------------- the kernel
@@ -405,7 +403,8 @@ __global__ void __launch_bounds__(kRows* G, 1)
   extern __shared__ uint8_t smem_raw[];
   uint8_t* sp0 = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
   uint8_t* s_tiles = sp0;
-  uint8_t* s_wg = s_tiles + SP::tiles;
+  uint8_t* s_ones = s_tiles + SP::tiles;
+  uint8_t* s_wg = s_ones + kOnesBytes;
   float* s_Qt = reinterpret_cast<float*>(s_wg + G * SP::per_wg);
   float* s_Lt = s_Qt + kMaxS2 * kH;
   uint64_t* s_mbar = reinterpret_cast<uint64_t*>(s_Lt + kMaxS2 * 8);
@@ -428,6 +427,7 @@ __global__ void __launch_bounds__(kRows* G, 1)
     uint4* dst = reinterpret_cast<uint4*>(s_tiles);
     for (int i = threadIdx.x; i < (int)(SP::tiles / 16); i += kRows * G) dst[i] = __ldg(src + i);
   }
+  fill_ones(s_ones, kRows * G);
   const bool indirect = (fr.flags & 4u) && fr.s.S && fr.t.S;
   if (indirect && TSHARED) {                    // shared tertiary set: Q_k = W1w . w'_k; per k: radiance, pdf, direction
     for (int e = threadIdx.x; e < (int)fr.t.S * kH; e += kRows * G) {
@@ -457,9 +457,8 @@ __global__ void __launch_bounds__(kRows* G, 1)
   c.phase = 0;
   c.tile0 = smem_u32(s_tiles);
   c.lo_off = kHiTileBytes;
+  c.ones = smem_u32(s_ones);
   const uint32_t tA = c.tmem + c.lane, tD = c.tmem + c.lane + CL::d;
-  restore_one<PREC, G>(c);
-  wait_st();
   uint8_t* my = s_wg + wgi * SP::per_wg;
   float* Ps = reinterpret_cast<float*>(my) + c.t;                                     // Ps[k * 128]
   float4* Ps4 = reinterpret_cast<float4*>(my) + c.t;                                  // the same memory as [16][128] float4
@@ -607,12 +606,11 @@ __global__ void __launch_bounds__(kRows* G, 1)
           const float* dp = dir_of(fr.s, i, j);
           const float wx = __ldg(dp), wy = __ldg(dp + 1), wz = __ldg(dp + 2), wp = pdf_of(fr.s, i, j);
           h1_dir<true>(tA, cw, [&](int q) { return Ps4[q * kRows]; }, wx, wy, wz);
-          issue_layer<PREC, G>(c, 0, 2, 4, true, CL::bias64 ? 0 : -1, 3);
+          issue_layer<PREC, G>(c, 0, 2, 4, true, 0, 3);
           const float3 gg = brdf_cos_over_pdf(sp, b, wx, wy, wz, ox, oy, oz, wp);
           wait_layer(c);
           float zv, zt, v, t;
-          epi_precise<!CL::bias64>(tD, cw, zv, zt);
-          if (!CL::bias64) restore_one<PREC, G>(c);
+          epi_precise<false>(tD, cw, zv, zt);
           irt_maps(sp, zv, zt, v, t);
           const float m = (1.f - v) * wscale;
           const float gr = m * gg.x, ggc = m * gg.y, gb = m * gg.z;
@@ -669,7 +667,7 @@ __global__ void __launch_bounds__(kRows* G, 1)
 // x 32 outstanding loads per SM keep the gather pipeline full when the table spills from L2 to HBM.  t is an output, so the
 // fp32 epilogue is used (features hi/lo split for P, fp16 h1).
 constexpr int kTraceG = 4;
-constexpr size_t kTraceSmem = 1024 + kHiTileBytes + (size_t)kTraceG * kH * kRows * 4 + 8 * kMaxG + 16;
+constexpr size_t kTraceSmem = 1024 + kHiTileBytes + kOnesBytes + (size_t)kTraceG * kH * kRows * 4 + 8 * kMaxG + 16;
 
 template <bool F16TAB>
 __global__ void __launch_bounds__(kRows* kTraceG, 1)
@@ -680,7 +678,8 @@ __global__ void __launch_bounds__(kRows* kTraceG, 1)
   using CL = Cols<0, G>;
   extern __shared__ uint8_t smem_raw[];
   uint8_t* s_tiles = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
-  float4* s_P = reinterpret_cast<float4*>(s_tiles + kHiTileBytes);
+  uint8_t* s_ones = s_tiles + kHiTileBytes;
+  float4* s_P = reinterpret_cast<float4*>(s_ones + kOnesBytes);
   uint64_t* s_mbar = reinterpret_cast<uint64_t*>(s_P + (size_t)G * (kH / 4) * kRows);
   uint32_t* s_tmem = reinterpret_cast<uint32_t*>(s_mbar + kMaxG);
   const int wgi = threadIdx.x / kRows, warp = threadIdx.x >> 5;
@@ -698,6 +697,7 @@ __global__ void __launch_bounds__(kRows* kTraceG, 1)
     uint4* dst = reinterpret_cast<uint4*>(s_tiles);
     for (int i = threadIdx.x; i < kHiTileBytes / 16; i += kRows * G) dst[i] = __ldg(src + i);
   }
+  fill_ones(s_ones, kRows * G);
   asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
   fence_before();
   __syncthreads();
@@ -708,9 +708,8 @@ __global__ void __launch_bounds__(kRows* kTraceG, 1)
   c.phase = 0;
   c.tile0 = smem_u32(s_tiles);
   c.lo_off = 0;
+  c.ones = smem_u32(s_ones);
   const uint32_t tA = c.tmem + c.lane, tD = c.tmem + c.lane + CL::d;
-  restore_one<0, G>(c);
-  wait_st();
   float4* Ps4 = s_P + (size_t)wgi * (kH / 4) * kRows + c.t;
   const unsigned long long ntiles = (N + kRows - 1) / kRows;
   for (unsigned long long tile = (unsigned long long)blockIdx.x * G + wgi; tile < ntiles; tile += (unsigned long long)gridDim.x * G) {
