@@ -1,15 +1,7 @@
-// hr_kernels_tc.cuh -- tensor-core (tcgen05 / TMEM) implementation of the fused path for mlp_dtype == HR_F16.
-//
-// Design: a CTA is 128 threads = the 128 TMEM lanes; thread p owns primary point
-// p of the CTA's 128-point tile for the whole frame (direct set, secondary set, and the tertiary set of each of its
-// secondary points), so no activation ever crosses threads.  Every 64-wide MLP layer over the tile is ONE
-// M=128 x N=64 tcgen05.mma group: each thread packs its row of fp16 activations straight into TMEM (tcgen05.st,
-// the A operand is read from TMEM), weights sit in shared memory as K-major SWIZZLE_128B UMMA tiles, the fp32
-// accumulator comes back with tcgen05.ld and the bias/ReLU/last-layer dot products run from constant-bank
-// operands.  Layer-1 biases ride in the MMA as an extra K step (hi + lo fp16 split => exact to 2^-22).
-// The query loops are software-pipelined two deep over two (A, D) TMEM buffer pairs, and the gathers of the next
-// secondary point are spread over the tertiary loop of the current one, so a thread's gathers, packing, MMA and
-// epilogue overlap; two CTAs per SM cover the remaining serial phases.
+// hr_kernels_tc.cuh -- tcgen05 / TMEM building blocks shared by the warpgroup kernels (hr_render_wg.cuh): PTX wrappers
+// (tcgen05.mma / ld / st / commit, mbarrier), fp16x2 packing, the K-major SWIZZLE_128B shared-memory descriptor, the
+// per-level gather + fp16x2 interpolation of the fast encoder, the constant block passed by value (TcConst) and the host-side
+// layout of the UMMA weight tiles.
 //
 // Precision contract (Q34): tables/weights fp16 (rounded once by the caller's generator), hidden activations
 // rounded to fp16 (RNE), accumulation fp32, final-layer outputs / t / x' / the index path / shading fp32.
@@ -25,19 +17,11 @@
 namespace hr {
 namespace tc {
 
-constexpr int kThreads = 128;
-constexpr int kTmemCols = 256;                // per CTA; two CTAs per SM own the whole TMEM
 constexpr int kTileBytes = 64 * 128;          // one 64 x 64 fp16 K-major SW128 weight tile
 constexpr int kNumTiles = 4;                  // I.W1f(+b1,b2), B.W1(+b1,b2), I.W2, B.W2  (64 x 64 each)
 constexpr int kTile3Bytes = 16 * 128;         // B.W3 zero-padded to 16 x 64 (N = 16 MMA)
 constexpr int kAllTileBytes = kNumTiles * kTileBytes + kTile3Bytes;
-constexpr int kCtasPerSm = 2;
 constexpr int kMaxS2 = 16;                    // shared tertiary set staged in smem
-// TMEM column map (per CTA).  Two (A, D) buffer pairs let one query's MMA run under the next query's packing and
-// the previous query's epilogue.  A buffer b: columns 64 b .. 64 b + 31 (fp16 pairs); the split-precision layers use
-// A0 columns 0..63 (hi | lo).  Columns 32..47 stage the NEXT secondary point's features while the tertiary loop of
-// the current one runs.  Columns 96..103 hold the constant bias K-step [1, 1, 0 .. 0].  D buffer b: 128 + 64 b.
-constexpr uint32_t kColA = 0, kColNext = 32, kColOne = 96, kColD = 128, kBufStride = 64;
 
 struct __align__(16) TcConst {                // lives in the kernel-parameter constant bank
   float w1w[3][kH];                           // I layer 1, direction columns
@@ -151,68 +135,11 @@ __device__ __forceinline__ uint64_t make_bdesc(uint32_t smem_addr) {
 constexpr uint32_t kIdesc = (1u << 4) | ((64u >> 3) << 17) | ((128u >> 4) << 24);
 constexpr uint32_t kIdescN16 = (1u << 4) | ((16u >> 3) << 17) | ((128u >> 4) << 24);
 
-
-struct Ctx {
-  uint32_t lane;               // this warp's TMEM lane base (bits 31..16)
-  uint32_t base;               // TMEM base of the CTA's allocation (lane 0, column 0)
-  uint32_t mbar;               // smem address of mbarrier 0 (mbarrier 1 at +8)
-  uint32_t phase;              // bit b = parity to wait for on mbarrier b
-  uint32_t tile0;              // smem address of weight tile 0 (tile t at + t * kTileBytes)
-};
-__device__ __forceinline__ uint32_t colA(const Ctx& c, int buf) { return c.base + c.lane + kColA + kBufStride * buf; }
-__device__ __forceinline__ uint32_t colD(const Ctx& c, int buf) { return c.base + c.lane + kColD + kBufStride * buf; }
-__device__ __forceinline__ uint32_t colNext(const Ctx& c) { return c.base + c.lane + kColNext; }
-
-// Issue one 128 x N layer on buffer pair `buf`: D[buf] = A * W^T where A starts `a_off` columns into the CTA's TMEM
-// (lane 0 address), `ksteps` K-steps of 16; optional split lo block right after the hi block; optional bias K-step
-// (A = [1,1,0..] times K-step `bias_kstep` of tile `bias_tile`).  Every thread must have issued its tcgen05.st of A.
-// Does NOT wait for the MMA: wait_layer(c, buf) does.
-__device__ __forceinline__ void issue_layer(Ctx& c, int buf, uint32_t a_off, int tile, int ksteps, int bias_tile, int bias_kstep,
-                                            bool split = false, uint32_t idesc = kIdesc) {
-  wait_st();
-  fence_before();
-  __syncthreads();
-  if (threadIdx.x == 0) {
-    fence_after();
-    const uint32_t d = c.base + kColD + kBufStride * buf;
-    const uint32_t a = c.base + a_off;
-    const uint64_t bd = make_bdesc(c.tile0 + tile * kTileBytes);
-    for (int k = 0; k < ksteps; ++k) mma_f16_ts(d, a + 8 * k, bd + 2 * k, idesc, k > 0);
-    if (split)
-      for (int k = 0; k < ksteps; ++k) mma_f16_ts(d, a + 8 * (ksteps + k), bd + 2 * k, idesc, 1u);
-    if (bias_tile >= 0) mma_f16_ts(d, c.base + kColOne, make_bdesc(c.tile0 + bias_tile * kTileBytes) + 2 * bias_kstep, idesc, 1u);
-    mma_commit(c.mbar + 8 * buf);
-  }
-}
-__device__ __forceinline__ void wait_layer(Ctx& c, int buf) {
-  mbar_wait(c.mbar + 8 * buf, (c.phase >> buf) & 1u);
-  c.phase ^= 1u << buf;
-  fence_after();
-}
-
 // ---------------------------------------------------------------------------------------------------- encode pieces
 // residual of an fp16x2 pack: (a - fp16(a), b - fp16(b)) packed again (the "lo" half of a hi/lo split)
 __device__ __forceinline__ uint32_t pack_lo(uint32_t hi, float a, float b) {
   const float2 h = __half22float2(*reinterpret_cast<const __half2*>(&hi));
   return pack_rn(a - h.x, b - h.y);
-}
-
-// Primary point: f = H(x) in fp32, level l -> A0 column l (fp16 pair) and its fp16 residual -> column 16 + l
-// (split-precision features for the layer-1 partial P, which feeds the t that moves x').
-template <bool F16>
-__device__ __forceinline__ void encode_split_to_A(const GridP& g, const Ctx& c, float x, float y, float z) {
-  const uint32_t tA = colA(c, 0);
-#pragma unroll 2
-  for (int l = 0; l < kMaxL; ++l) {
-    uint32_t hi = 0u, lo = 0u;
-    if (l < (int)g.L) {
-      const float2 v = encode_level<F16>(g, l, x, y, z, nullptr, nullptr);
-      hi = pack_rn(v.x, v.y);
-      lo = pack_lo(hi, v.x, v.y);
-    }
-    tmem_st1(tA + l, hi);
-    tmem_st1(tA + 16 + l, lo);
-  }
 }
 
 // Secondary points: the gathers of one level (issued early) and their interpolation (consumed late) are separate so
@@ -263,309 +190,8 @@ __device__ __forceinline__ uint32_t lerp_level(const LevelTaps<false>& t) {
   return pack_rn(fmaf(t.w[2], b1x - b0x, b0x), fmaf(t.w[2], b1y - b0y, b0y));
 }
 
-// whole fast encode of one secondary point into the staging columns (used for the first secondary point of a pixel
-// and whenever the tertiary loop cannot carry the gathers)
-template <bool F16>
-__device__ __forceinline__ void encode_next_plain(const GridP& g, const Ctx& c, float x, float y, float z) {
-  const uint32_t tN = colNext(c);
-#pragma unroll 1
-  for (int l0 = 0; l0 < kMaxL; l0 += 2) {
-    LevelTaps<F16> t0, t1;
-    const bool on0 = l0 < (int)g.L, on1 = l0 + 1 < (int)g.L;
-    if (on0) gather_level<F16>(g, l0, x, y, z, t0);
-    if (on1) gather_level<F16>(g, l0 + 1, x, y, z, t1);
-    tmem_st1(tN + l0, on0 ? lerp_level(t0) : 0u);
-    tmem_st1(tN + l0 + 1, on1 ? lerp_level(t1) : 0u);
-  }
-}
-
-// ---------------------------------------------------------------------------------------------------- per-row stages
-// Precise epilogue of I (secondary set: z_t becomes t): (z_v, z_t) = b3 + W3 relu(D + b2), all fp32.
-__device__ __forceinline__ void irt_epilogue_precise(const Ctx& c, const TcConst& cw, int buf, float& zv, float& zt) {
-  float z0[4] = {cw.b3[0], 0.f, 0.f, 0.f}, z1[4] = {cw.b3[1], 0.f, 0.f, 0.f};
-  const uint32_t tD = colD(c, buf);
-#pragma unroll
-  for (int h = 0; h < 2; ++h) {
-    uint32_t r[32];
-    tmem_ld32(tD + 32 * h, r);
-    wait_ld();
-#pragma unroll
-    for (int k = 0; k < 32; ++k) {
-      const float a = fmaxf(__uint_as_float(r[k]) + cw.b2[32 * h + k], 0.f);
-      z0[k & 3] = fmaf(a, cw.w3[0][32 * h + k], z0[k & 3]);
-      z1[k & 3] = fmaf(a, cw.w3[1][32 * h + k], z1[k & 3]);
-    }
-  }
-  zv = (z0[0] + z0[1]) + (z0[2] + z0[3]);
-  zt = (z1[0] + z1[1]) + (z1[2] + z1[3]);
-}
-
-// Fast epilogue of I (direct and tertiary queries need only visibility): b2 already rode in the MMA (bias K-step),
-// h2 = relu(D) is rounded to fp16 by the packing conversion, z_v = b3 + w3v . h2 with fp16x2 FMAs into four short
-// accumulators summed in fp32.
-__device__ __forceinline__ float irt_epilogue_fast(const Ctx& c, const TcConst& cw, int buf) {
-  __half2 acc[4];
-#pragma unroll
-  for (int q = 0; q < 4; ++q) acc[q] = __float2half2_rn(0.f);
-  const uint32_t tD = colD(c, buf);
-#pragma unroll
-  for (int h = 0; h < 2; ++h) {
-    uint32_t r[32];
-    tmem_ld32(tD + 32 * h, r);
-    wait_ld();
-#pragma unroll
-    for (int k = 0; k < 16; ++k) {
-      const uint32_t p = pack_relu(__uint_as_float(r[2 * k]), __uint_as_float(r[2 * k + 1]));
-      const uint32_t w = cw.w3v_h2[16 * h + k];
-      acc[k & 3] = __hfma2(*reinterpret_cast<const __half2*>(&p), *reinterpret_cast<const __half2*>(&w), acc[k & 3]);
-    }
-  }
-  float z = cw.b3[0];
-#pragma unroll
-  for (int q = 0; q < 4; ++q) { const float2 f = __half22float2(acc[q]); z += f.x + f.y; }
-  return z;
-}
-
 __device__ __forceinline__ float vis_of(const ShadeP& sp, float zv) { return sp.vis_mode ? (zv > 0.f ? 1.f : 0.f) : sigmoidf_(zv); }
-
-// D0 -> relu -> fp16 -> A0 columns 0..31
-__device__ __forceinline__ void hidden_to_A(const Ctx& c) {
-  const uint32_t tD = colD(c, 0), tA = colA(c, 0);
-#pragma unroll
-  for (int h = 0; h < 2; ++h) {
-    uint32_t r[32];
-    tmem_ld32(tD + 32 * h, r);
-    wait_ld();
-    uint32_t p[16];
-#pragma unroll
-    for (int k = 0; k < 16; ++k) p[k] = pack_relu(__uint_as_float(r[2 * k]), __uint_as_float(r[2 * k + 1]));
-    tmem_st16(tA + 16 * h, p);
-  }
-}
-
-// B(f) with the fp16 features at column offset f_off: all three layers on the tensor core (layer-1/2 biases ride in
-// the MMAs, layer 3 is an N = 16 MMA over the zero-padded 7-row W3; b3 is added in registers).  Buffer pair 0.
-__device__ __forceinline__ void brdf_from_A(Ctx& c, const TcConst& cw, const ShadeP& sp, uint32_t f_off, float (&b)[7]) {
-  issue_layer(c, 0, f_off, 1, 2, 1, 2);
-  wait_layer(c, 0);
-  hidden_to_A(c);
-  issue_layer(c, 0, kColA, 3, 4, 1, 3);
-  wait_layer(c, 0);
-  hidden_to_A(c);
-  issue_layer(c, 0, kColA, 4, 4, -1, 0, false, kIdescN16);
-  wait_layer(c, 0);
-  uint32_t r[8];
-  tmem_ld8(colD(c, 0), r);
-  wait_ld();
-  float o[8];
-#pragma unroll
-  for (int q = 0; q < 8; ++q) o[q] = __uint_as_float(r[q]) + cw.Bb3[q];
-  brdf_maps(sp, o, b);
-}
-
-// Primary point only (once per pixel): B in split precision.  n = o/||o|| amplifies an absolute error of o by 1/||o||
-// and every sample of the pixel sees the same n, so fp16-grade activations here would be a COHERENT pixel error; the
-// hi/lo split of f (already in A0[0..31]) and of the hidden layer keeps B's inputs to ~2^-22, layer 3 runs in fp32.
-__device__ __forceinline__ void brdf_precise_from_A(Ctx& c, const TcConst& cw, const ShadeP& sp, float (&b)[7]) {
-  issue_layer(c, 0, kColA, 1, 2, 1, 2, true);
-  wait_layer(c, 0);
-  const uint32_t tD = colD(c, 0), tA = colA(c, 0);
-#pragma unroll
-  for (int h = 0; h < 2; ++h) {
-    uint32_t r[32];
-    tmem_ld32(tD + 32 * h, r);
-    wait_ld();
-    uint32_t p[16], q[16];
-#pragma unroll
-    for (int k = 0; k < 16; ++k) {
-      const float a0 = fmaxf(__uint_as_float(r[2 * k]), 0.f), a1 = fmaxf(__uint_as_float(r[2 * k + 1]), 0.f);
-      p[k] = pack_rn(a0, a1);
-      q[k] = pack_lo(p[k], a0, a1);
-    }
-    tmem_st16(tA + 16 * h, p);
-    tmem_st16(tA + 32 + 16 * h, q);
-  }
-  issue_layer(c, 0, kColA, 3, 4, 1, 3, true);
-  wait_layer(c, 0);
-  float o[8];
-#pragma unroll
-  for (int q = 0; q < 8; ++q) o[q] = cw.Bb3[q];
-#pragma unroll
-  for (int h = 0; h < 2; ++h) {
-    uint32_t r[32];
-    tmem_ld32(tD + 32 * h, r);
-    wait_ld();
-#pragma unroll
-    for (int k = 0; k < 32; ++k) {
-      const float a = fmaxf(__uint_as_float(r[k]), 0.f);
-#pragma unroll
-      for (int q = 0; q < 7; ++q) o[q] = fmaf(a, cw.BW3[q][32 * h + k], o[q]);
-    }
-  }
-  brdf_maps(sp, o, b);
-}
-
-// h1 = relu(P + W1w . w) -> A[buf] columns 0..31 (P in registers)
-__device__ __forceinline__ void h1_from_regs(const Ctx& c, const TcConst& cw, int buf, const float (&P)[kH], float wx, float wy, float wz) {
-  const uint32_t tA = colA(c, buf);
-#pragma unroll
-  for (int h = 0; h < 2; ++h) {
-    uint32_t p[16];
-#pragma unroll
-    for (int k = 0; k < 16; ++k) {
-      const int j = 32 * h + 2 * k;
-      float a0 = fmaf(cw.w1w[0][j], wx, P[j]);
-      a0 = fmaf(cw.w1w[1][j], wy, a0); a0 = fmaf(cw.w1w[2][j], wz, a0);
-      float a1 = fmaf(cw.w1w[0][j + 1], wx, P[j + 1]);
-      a1 = fmaf(cw.w1w[1][j + 1], wy, a1); a1 = fmaf(cw.w1w[2][j + 1], wz, a1);
-      p[k] = pack_relu(a0, a1);
-    }
-    tmem_st16(tA + 16 * h, p);
-  }
-}
-// split-precision variant for the secondary set (its z_t becomes t and moves x': SURVEY 8(c) conditioning note):
-// h1 in fp32 -> hi (A0 columns 0..31) + lo (columns 32..63); P from this thread's shared-memory column
-__device__ __forceinline__ void h1_from_smem_split(const Ctx& c, const TcConst& cw, const float* Ps, float wx, float wy, float wz) {
-  const uint32_t tA = colA(c, 0);
-#pragma unroll
-  for (int h = 0; h < 2; ++h) {
-    uint32_t p[16], q[16];
-#pragma unroll
-    for (int k = 0; k < 16; ++k) {
-      const int j = 32 * h + 2 * k;
-      float a0 = fmaf(cw.w1w[0][j], wx, Ps[j * kThreads]);
-      a0 = fmaf(cw.w1w[1][j], wy, a0); a0 = fmaxf(fmaf(cw.w1w[2][j], wz, a0), 0.f);
-      float a1 = fmaf(cw.w1w[0][j + 1], wx, Ps[(j + 1) * kThreads]);
-      a1 = fmaf(cw.w1w[1][j + 1], wy, a1); a1 = fmaxf(fmaf(cw.w1w[2][j + 1], wz, a1), 0.f);
-      p[k] = pack_rn(a0, a1);
-      q[k] = pack_lo(p[k], a0, a1);
-    }
-    tmem_st16(tA + 16 * h, p);
-    tmem_st16(tA + 32 + 16 * h, q);
-  }
-}
-// shared direction set: the direction part Q = W1w . w'_k is precomputed per CTA, h1 = relu(P + Q)
-__device__ __forceinline__ void h1_from_regs_shared(const Ctx& c, int buf, const float (&P)[kH], const float* __restrict__ Q) {
-  const uint32_t tA = colA(c, buf);
-#pragma unroll
-  for (int h = 0; h < 2; ++h) {
-    uint32_t p[16];
-#pragma unroll
-    for (int k = 0; k < 8; ++k) {
-      const float4 q = reinterpret_cast<const float4*>(Q)[8 * h + k];
-      const int j = 32 * h + 4 * k;
-      p[2 * k] = pack_relu(P[j] + q.x, P[j + 1] + q.y);
-      p[2 * k + 1] = pack_relu(P[j + 2] + q.z, P[j + 3] + q.w);
-    }
-    tmem_st16(tA + 16 * h, p);
-  }
-}
-
-// shared direction set, all-fp16x2 form: P and Q both pre-rounded to fp16 pairs, h1 = fma.relu(P, 1, Q): one
-// instruction per pair (the sum is rounded once more: 1.5 ulp of fp16 instead of 0.5 -- tertiary visibility only)
-__device__ __forceinline__ void h1_from_h2_shared(const Ctx& c, int buf, const uint32_t (&Ph)[kH / 2], const uint32_t* __restrict__ Qh) {
-  const uint32_t tA = colA(c, buf);
-#pragma unroll
-  for (int h = 0; h < 2; ++h) {
-    uint32_t p[16];
-#pragma unroll
-    for (int k = 0; k < 4; ++k) {
-      const uint4 q = reinterpret_cast<const uint4*>(Qh)[4 * h + k];
-      const uint32_t qq[4] = {q.x, q.y, q.z, q.w};
-#pragma unroll
-      for (int e = 0; e < 4; ++e)
-        asm("fma.rn.relu.f16x2 %0, %1, %2, %3;" : "=r"(p[4 * k + e]) : "r"(Ph[16 * h + 4 * k + e]), "r"(0x3C003C00u), "r"(qq[e]));
-    }
-    tmem_st16(tA + 16 * h, p);
-  }
-}
-// D0 -> fp16 pairs (32 registers)
-__device__ __forceinline__ void load_D_h2(const Ctx& c, uint32_t (&Ph)[kH / 2]) {
-  const uint32_t tD = colD(c, 0);
-#pragma unroll
-  for (int h = 0; h < 2; ++h) {
-    uint32_t r[32];
-    tmem_ld32(tD + 32 * h, r);
-    wait_ld();
-#pragma unroll
-    for (int k = 0; k < 16; ++k) Ph[16 * h + k] = pack_rn(__uint_as_float(r[2 * k]), __uint_as_float(r[2 * k + 1]));
-  }
-}
-
-// D0 -> registers (64 fp32)
-__device__ __forceinline__ void load_D(const Ctx& c, float (&P)[kH]) {
-  const uint32_t tD = colD(c, 0);
-#pragma unroll
-  for (int h = 0; h < 2; ++h) {
-    uint32_t r[32];
-    tmem_ld32(tD + 32 * h, r);
-    wait_ld();
-#pragma unroll
-    for (int k = 0; k < 32; ++k) P[32 * h + k] = __uint_as_float(r[k]);
-  }
-}
-
-// ---------------------------------------------------------------------------------------------------- shared setup
-struct Smem {
-  uint8_t* tiles;      // 4 x 8 KB + 2 KB, 1024-aligned
-  float* Ps;           // [64][128]
-  float* Qt;           // [kMaxS2][64]
-  float* Lt;           // [kMaxS2][8]: radiance rgb, pdf, direction xyz, pad
-  uint64_t* mbar;      // [2]
-  uint32_t* tmem_slot;
-};
-constexpr size_t kSmemBytes = 1024 + kAllTileBytes + kH * kThreads * 4 + kMaxS2 * kH * 4 + kMaxS2 * 8 * 4 + 64;
-
-__device__ __forceinline__ Smem carve(uint8_t* raw) {
-  Smem s;
-  uint8_t* p = raw + ((1024u - (smem_u32(raw) & 1023u)) & 1023u);      // pointer arithmetic keeps the shared address space
-  s.tiles = p; p += kAllTileBytes;
-  s.Ps = reinterpret_cast<float*>(p); p += kH * kThreads * 4;
-  s.Qt = reinterpret_cast<float*>(p); p += kMaxS2 * kH * 4;
-  s.Lt = reinterpret_cast<float*>(p); p += kMaxS2 * 8 * 4;
-  s.mbar = reinterpret_cast<uint64_t*>(p); p += 16;
-  s.tmem_slot = reinterpret_cast<uint32_t*>(p);
-  return s;
-}
-
-__device__ __forceinline__ void setup(const Smem& s, const uint8_t* __restrict__ wtiles, Ctx& c) {
-  const int warp = threadIdx.x >> 5;
-  if (warp == 0) {
-    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(s.tmem_slot)), "r"((uint32_t)kTmemCols) : "memory");
-    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
-  }
-  if (threadIdx.x == 0) {
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(smem_u32(s.mbar)) : "memory");
-    asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(smem_u32(s.mbar + 1)) : "memory");
-    asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
-  }
-  const uint4* src = reinterpret_cast<const uint4*>(wtiles);
-  uint4* dst = reinterpret_cast<uint4*>(s.tiles);
-  for (int i = threadIdx.x; i < kAllTileBytes / 16; i += kThreads) dst[i] = __ldg(src + i);
-  asm volatile("fence.proxy.async.shared::cta;" ::: "memory");     // generic-proxy writes -> visible to the tensor core
-  fence_before();
-  __syncthreads();
-  fence_after();
-  c.base = *s.tmem_slot;
-  c.lane = (uint32_t)(warp * 32) << 16;
-  c.mbar = smem_u32(s.mbar); c.phase = 0;
-  c.tile0 = smem_u32(s.tiles);
-  uint32_t one[8] = {0x3C003C00u, 0u, 0u, 0u, 0u, 0u, 0u, 0u};     // bias K-step of A: [1, 1, 0, ... 0]
-  tmem_st8(c.base + c.lane + kColOne, one);
-  wait_st();
-}
-
-__device__ __forceinline__ void teardown(const Ctx& c) {
-  fence_before();
-  __syncthreads();
-  if ((threadIdx.x >> 5) == 0) {
-    fence_after();
-    asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(c.base), "r"((uint32_t)kTmemCols) : "memory");
-  }
-}
-
 // ---------------------------------------------------------------------------------------------------- host side
-struct HostWeights { TcConst cw; };
 
 inline size_t tile_off(int j, int k) { return (size_t)(j / 8) * 1024 + (j % 8) * 128 + (((k / 8) ^ (j % 8)) * 16) + (k % 8) * 2; }
 

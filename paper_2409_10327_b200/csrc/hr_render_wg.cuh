@@ -49,9 +49,8 @@ static_assert(sizeof(Item) == 48, "Item is three 16-byte words");
 
 template <int PREC, int G> struct Cols {
   static_assert(G >= 1 && G <= kMaxG, "1..4 warpgroups");
-    static constexpr uint32_t stride = G == 4 ? 128u : (G == 3 ? 168u : (G == 2 ? 256u : 512u));
-  // A = columns 0..63 (fp16 pairs): hi | lo for the split layers, or two 32-column buffers A0 | A1 that the fp16 query loops
-  // alternate between (the next query's h1 is written while the current MMA runs).  D = 64 fp32 accumulator columns.
+  static constexpr uint32_t stride = G == 4 ? 128u : (G == 3 ? 168u : (G == 2 ? 256u : 512u));
+  // A = columns 0..63 (fp16 pairs): 0..31 for the fp16 layers, hi | lo for the split layers.  D = 64 fp32 accumulator columns.
   // The constant operand of the bias K-steps, rows of [1, 1, 0 .. 0], lives in SHARED memory (kOnesBytes of identical
   // 16-byte chunks, so the swizzle cannot matter), which leaves all 128 columns of a G = 4 warpgroup to A and D.
   static constexpr uint32_t d = 64u;
