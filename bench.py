@@ -350,6 +350,19 @@ def main():
             torch.cuda.synchronize()
             out.update(e2e_sampled_ms=e0.elapsed_time(e1) / e2e_steps, e2e_sampled_h2d=int(hx.numel() + hwo.numel()) * 4,
                        e2e_sampled_finite=bool(torch.isfinite(hrgb).all()), e2e_sampled_mean=float(hrgb.mean()))
+        # the step after the path: spatial-only SVGF on the frame just rendered ("Dnsr" column of Table 3)
+        if sampled and cfg.points == "scene" and cfg.N == cfg.width * cfg.width:
+            Wd = cfg.width
+            nimg = up(fr["n_g"]).reshape(Wd, Wd, 3); pimg = x.reshape(Wd, Wd, 3); rimg = rgb.reshape(Wd, Wd, 3)
+            dout = torch.empty_like(rimg)
+            for _ in range(2):
+                r.denoise(rimg, nimg, pimg, (0.5, 0.5, -1.2), dout, stream=stream)
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record()
+            for _ in range(10):
+                r.denoise(rimg, nimg, pimg, (0.5, 0.5, -1.2), dout, stream=stream)
+            e1.record(); torch.cuda.synchronize()
+            out.update(denoise_ms=e0.elapsed_time(e1) / 10, denoise_finite=bool(torch.isfinite(dout).all()))
         r.destroy()
         del x, wo, d, s, t, rgb
         torch.cuda.empty_cache()
@@ -416,6 +429,10 @@ def main():
                                "h2d_bytes_per_step": res["e2e_sampled_h2d"], "d2h_bytes_per_step": cfg.N * 12, "finite": res["e2e_sampled_finite"],
                                "what": "same frame shape, but only x and wo travel: B(H(x)) is decoded and the direction sets are generated on the "
                                        "device (hashrender_encode/decode/sample_mis/sample_stratified/render_frame); PAPER.md:122, 344"}
+    if "denoise_ms" in res:
+        line["denoise"] = {"ms_per_frame": res["denoise_ms"], "finite": res["denoise_finite"], "kernels_per_frame": 7,
+                           "what": "hashrender_denoise: spatial-only SVGF (7x7 variance estimate + five 5x5 a-trous passes) on the rendered "
+                                   "800x800 frame; the paper's Table 3 lists 3.2-3.5 ms for its denoiser on an A100 (context)"}
     if world == 1 and not args.no_extra:
         # the same frame with the default API flags (zero-weight secondary rays compacted out), and the
         # other precision; `value` here is frame-equivalent (queries_per_frame / time), executed queries are stated

@@ -146,6 +146,22 @@ int hashrender_sample_mis(hashrender_t* h, const float* brdf, const float* wo, u
 int hashrender_sample_stratified(hashrender_t* h, const float* normal, uint64_t rows, uint32_t Sa, uint32_t Sb, uint64_t seed,
                                  float* dir, float* pdf, void* stream);
 
+/* Spatial-only SVGF denoiser, the step after the path (SVGF on the raw MC result with the temporal parts removed;
+ * depth gradient by finite differences of the depth derived from the primary surface coordinates; Q39-Q44).
+ * Image arrays are row-major [H][W][.] DEVICE pointers.  rgb / out [H,W,3]; albedo [H,W,3] nullable (given => the illumination
+ * rgb / max(albedo, 1e-3) is filtered and re-multiplied); normal [H,W,3] unit; pos [H,W,3] primary surface points, depth = |pos - cam|;
+ * mask [H,W] nullable (0 => output 0, the pixel contributes to nobody).  iterations 1..8 a-trous passes (5: the published filter);
+ * sigma_z 1, sigma_n 128, sigma_l 4 are the published edge-stopping parameters.  Scratch is grown on demand inside the handle. */
+typedef struct {
+  uint32_t H, W;
+  const float* rgb; const float* albedo; const float* normal; const float* pos;
+  float cam[3];
+  const uint8_t* mask;
+  uint32_t iterations;
+  float sigma_z, sigma_n, sigma_l;
+} hr_denoise;
+int hashrender_denoise(hashrender_t* h, const hr_denoise* d, float* out, void* stream);
+
 /* Secondary-ray accounting of the render_frame calls since the last reset: rays_traced = secondary
  * (point, direction) rays whose (v, t) were evaluated, rays_evaluated = those whose L'_o was evaluated (all of them with
  * HR_DENSE).  Both nullable.  Synchronises the device.  Only the tcgen05 paths count; the FFMA path leaves both at 0. */

@@ -16,7 +16,7 @@ _LIB_PATH = os.path.join(os.path.dirname(os.path.abspath(__file__)), "libhashren
 
 EXPORTS = ["hashrender_create", "hashrender_destroy", "hashrender_set_env", "hashrender_encode", "hashrender_decode",
            "hashrender_trace", "hashrender_shade", "hashrender_render_frame", "hashrender_render_frame_host",
-           "hashrender_sample_mis", "hashrender_sample_stratified", "hashrender_stats", "hashrender_launch_count", "hashrender_last_path", "hashrender_last_error"]
+           "hashrender_sample_mis", "hashrender_sample_stratified", "hashrender_denoise", "hashrender_stats", "hashrender_launch_count", "hashrender_last_path", "hashrender_last_error"]
 
 
 class HashRenderError(RuntimeError):
@@ -35,6 +35,12 @@ class hr_config(C.Structure):
 
 class hr_dirset(C.Structure):
     _fields_ = [("dir", C.c_void_p), ("pdf", C.c_void_p), ("Lin", C.c_void_p), ("S", C.c_uint32), ("point_stride", C.c_uint64)]
+
+
+class hr_denoise(C.Structure):
+    _fields_ = [("H", C.c_uint32), ("W", C.c_uint32), ("rgb", C.c_void_p), ("albedo", C.c_void_p), ("normal", C.c_void_p),
+                ("pos", C.c_void_p), ("cam", C.c_float * 3), ("mask", C.c_void_p), ("iterations", C.c_uint32),
+                ("sigma_z", C.c_float), ("sigma_n", C.c_float), ("sigma_l", C.c_float)]
 
 
 class hr_frame(C.Structure):
@@ -66,6 +72,7 @@ def load_library(path: str | None = None):
         lib.hashrender_render_frame_host.argtypes = [vp, C.POINTER(hr_frame), vp, vp, C.POINTER(u64), C.POINTER(u64)]
         lib.hashrender_sample_mis.argtypes = [vp, vp, vp, u64, u32, u64, vp, vp, vp]
         lib.hashrender_sample_stratified.argtypes = [vp, vp, u64, u32, u32, u64, vp, vp, vp]
+        lib.hashrender_denoise.argtypes = [vp, C.POINTER(hr_denoise), vp, vp]
         lib.hashrender_stats.argtypes = [vp, C.POINTER(u64), C.POINTER(u64), C.c_int]
         lib.hashrender_launch_count.argtypes = [vp]
         lib.hashrender_launch_count.restype = u64
@@ -198,6 +205,14 @@ class HashRenderer:
 
     def sample_stratified(self, normal, rows, Sa, Sb, seed, dir, pdf, stream=None):
         self._check(self._lib.hashrender_sample_stratified(self._h, _ptr(normal), rows, Sa, Sb, seed, _ptr(dir), _ptr(pdf), stream))
+
+    def denoise(self, rgb, normal, pos, cam, out, albedo=None, mask=None, iterations=5, sigma_z=1.0, sigma_n=128.0, sigma_l=4.0,
+                stream=None):
+        """rgb / normal / pos / out: [H, W, 3] device tensors; cam: 3 floats."""
+        d = hr_denoise(H=rgb.shape[0], W=rgb.shape[1], rgb=_ptr(rgb), albedo=_ptr(albedo), normal=_ptr(normal), pos=_ptr(pos),
+                       cam=(C.c_float * 3)(*[float(v) for v in cam]), mask=_ptr(mask), iterations=iterations, sigma_z=sigma_z,
+                       sigma_n=sigma_n, sigma_l=sigma_l)
+        self._check(self._lib.hashrender_denoise(self._h, C.byref(d), _ptr(out), stream))
 
     def stats(self, reset=False):
         """(secondary rays traced, secondary rays whose L'_o was evaluated) since the last reset."""

@@ -13,6 +13,7 @@
 #include "hr_kernels_ffma.cuh"
 #include "hr_kernels_tc.cuh"
 #include "hr_sampler.cuh"
+#include "hr_svgf.cuh"
 #include "hr_wg_api.h"
 
 using namespace hr;
@@ -39,6 +40,8 @@ struct hashrender {
   // staging for render_frame_host
   void* stage[16] = {nullptr};
   size_t stage_cap[16] = {0};
+  void* d_svgf = nullptr;        // denoiser scratch: geo | live | two colour+variance planes
+  size_t svgf_cap = 0;
   float* d_light = nullptr;      // sampler tables: pmf [He*We] then cdf [He*We] (built lazily from the env map)
   size_t light_cap = 0;
   bool light_valid = false;
@@ -247,7 +250,7 @@ int hashrender_destroy(hashrender_t* h) {
   if (!h) return HR_ERR_INVALID_ARG;
   cudaDeviceSynchronize();
   cudaFree(h->d_tables); cudaFree(h->d_wts); cudaFree(h->d_wts_tc); cudaFree(h->d_env);
-  cudaFree(h->d_ring); cudaFree(h->d_counters); cudaFree(h->d_light);
+  cudaFree(h->d_ring); cudaFree(h->d_counters); cudaFree(h->d_light); cudaFree(h->d_svgf);
   if (h->copy_stream) {
     cudaStreamDestroy(h->copy_stream);
     for (int i = 0; i < 9; ++i) cudaEventDestroy(h->ev[i]);
@@ -569,6 +572,45 @@ int hashrender_sample_stratified(hashrender_t* h, const float* normal, uint64_t 
   const uint64_t need = (total + 255) / 256, cap = (uint64_t)h->num_sms * 16;
   smp::k_sample_stratified<<<(int)(need < cap ? need : cap), 256, 0, (cudaStream_t)stream>>>(normal, rows, Sa, Sb, seed, dir, pdf);
   h->launches++;
+  HR_CUDA(h, cudaGetLastError());
+  return HR_OK;
+}
+
+int hashrender_denoise(hashrender_t* h, const hr_denoise* d, float* out, void* stream) {
+  if (!h) return HR_ERR_INVALID_ARG;
+  if (!d) return fail(h, HR_ERR_INVALID_ARG, "denoise: NULL descriptor");
+  if (d->H == 0 || d->W == 0) return HR_OK;
+  if (!d->rgb || !d->normal || !d->pos || !out) return fail(h, HR_ERR_INVALID_ARG, "denoise: NULL rgb / normal / pos / out");
+  if (d->iterations < 1 || d->iterations > 8) return fail(h, HR_ERR_INVALID_ARG, "denoise: iterations must be 1..8");
+  if (!(d->sigma_z > 0.f) || !(d->sigma_l > 0.f) || !(d->sigma_n >= 0.f)) return fail(h, HR_ERR_INVALID_ARG, "denoise: bad sigma");
+  const size_t n = (size_t)d->H * d->W;
+  const size_t geo_b = n * sizeof(svgf::Geo), live_b = (n + 15) / 16 * 16, col_b = n * sizeof(float4);
+  const size_t need = geo_b + live_b + 2 * col_b;
+  if (need > h->svgf_cap) {
+    cudaFree(h->d_svgf); h->d_svgf = nullptr; h->svgf_cap = 0;
+    HR_CUDA(h, cudaMalloc(&h->d_svgf, need));
+    h->svgf_cap = need;
+  }
+  char* base = (char*)h->d_svgf;
+  svgf::Geo* geo = (svgf::Geo*)base;
+  uint8_t* live = (uint8_t*)(base + geo_b);
+  float4* colA = (float4*)(base + geo_b + live_b);
+  float4* colB = colA + n;
+  svgf::Params P;
+  P.H = d->H; P.W = d->W; P.sigma_z = d->sigma_z; P.sigma_n = d->sigma_n; P.sigma_l = d->sigma_l;
+  P.cam[0] = d->cam[0]; P.cam[1] = d->cam[1]; P.cam[2] = d->cam[2];
+  cudaStream_t st = (cudaStream_t)stream;
+  const uint64_t blocks = (n + 255) / 256, cap = (uint64_t)h->num_sms * 16;
+  const int grid = (int)(blocks < cap ? blocks : cap);
+  svgf::k_svgf_prep<<<grid, 256, 0, st>>>(P, d->rgb, d->albedo, d->pos, d->mask, geo, live, colA);
+  svgf::k_svgf_variance<<<grid, 256, 0, st>>>(P, geo, d->normal, live, colA);
+  float4* in = colA; float4* o = colB;
+  for (uint32_t it = 0; it < d->iterations; ++it) {
+    const bool last = it + 1 == d->iterations;
+    svgf::k_svgf_atrous<<<grid, 256, 0, st>>>(P, 1 << it, geo, d->normal, live, in, last ? nullptr : o, d->albedo, last ? out : nullptr);
+    float4* t = in; in = o; o = t;
+  }
+  h->launches += 2 + d->iterations;
   HR_CUDA(h, cudaGetLastError());
   return HR_OK;
 }
