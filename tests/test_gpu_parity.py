@@ -306,6 +306,24 @@ def test_render_frame_host_chunked_pipeline(torch):
     np.testing.assert_allclose(a, b2, rtol=2e-6, atol=1e-7)
 
 
+def test_fp32_model_outside_the_fp16_range_uses_the_ffma_kernels(torch):
+    """The tcgen05 fp32 path carries operands as fp16 hi + lo; a model whose weights / activation bounds do not fit that range must
+    fall back to the plain fp32 kernels (hashrender_last_path says which) and still match the oracle."""
+    cfg = gen.make_config("C0", S_i=4, S_2=3, flags=7)
+    m = gen.make_model(cfg)
+    big = {**m, "brdf_w": m["brdf_w"].copy()}
+    big["brdf_w"][: 64 * cfg.D] *= 4000.0                      # layer-1 weights of B: hidden activations up to ~1e5
+    fr = gen.make_frame(cfg, m["env"], np.arange(300))
+    r = make_renderer(cfg, big)
+    got = gpu_render(r, cfg, fr)
+    assert r.last_path() == "ffma32"
+    ref = oracle_render(_oracle(cfg, big), cfg, fr)
+    check_close(got, ref["rgb"], 4e-4, what="ffma fallback")
+    r2 = make_renderer(cfg, m)
+    gpu_render(r2, cfg, fr)
+    assert r2.last_path() == "tcgen05-f16x3"
+
+
 def test_frame_errors(torch):
     from paper_2409_10327_b200 import DirSet, HashRenderError
     cfg = gen.make_config("C0")
