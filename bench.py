@@ -112,6 +112,23 @@ def oracle_sample(cfg, model, pix, vis_mode):
     return dt, len(pix) * cfg.queries // cfg.N
 
 
+def _oracle_worker(job):
+    name, pix, vis_mode = job
+    cfg = gen.make_config(name)
+    model = gen.make_model(cfg)
+    return oracle_sample(cfg, model, pix, vis_mode)
+
+
+def oracle_all_cores(cfg, pix, vis_mode, procs):
+    """The same oracle, one single-threaded instance per host core over disjoint pixel ranges.  Each worker rebuilds the
+    model from the seed (untimed) and times only its render; the rate is total queries / slowest worker."""
+    import multiprocessing as mp
+    parts = [p for p in np.array_split(pix, procs) if len(p)]
+    with mp.get_context("spawn").Pool(len(parts)) as pool:
+        res = pool.map(_oracle_worker, [(cfg.name, p, vis_mode) for p in parts])
+    return max(r[0] for r in res), sum(r[1] for r in res), len(parts)
+
+
 def sample_pixels(cfg, n, seed=1234):
     return np.sort(np.random.default_rng(seed).choice(cfg.N, n, replace=False))
 
@@ -220,6 +237,7 @@ def main():
     ap.add_argument("--cpu-pixels", type=int, default=2048, help="pixels of the frame the cpu_baseline leg evaluates")
     ap.add_argument("--ref-pixels", type=int, default=256, help="pixels per step for --impl reference")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-cpu-all-cores", action="store_true", help="skip the all-host-cores oracle leg")
     ap.add_argument("--also", default="C3", help="second workload measured briefly and reported under `also` ('' = none)")
     ap.add_argument("--compact", action="store_true", help="headline with the default API flags (zero-weight secondary rays skipped) "
                     "instead of HR_DENSE")
@@ -460,6 +478,14 @@ def main():
                                 "sample": f"{len(pix)} seeded pixels of the same {cfg.name} frame ({q} queries) in {dt:.1f} s; "
                                           f"full frame extrapolates to {dt * cfg.N / len(pix):.0f} s",
                                 "host_cores_available": os.cpu_count()}
+        avail = len(os.sched_getaffinity(0))
+        if not args.no_cpu_all_cores and avail > 1:
+            procs = min(avail, 64)
+            npx = min(cfg.N, max(1, args.cpu_pixels // 2) * procs)
+            dta, qa, used = oracle_all_cores(cfg, sample_pixels(cfg, npx, seed=4321), args.vis_mode, procs)
+            line["cpu_baseline"]["all_cores"] = {"value": qa / dta, "unit": UNIT, "cores": used,
+                                                 "sample": f"{npx} seeded pixels split over {used} single-threaded oracle "
+                                                           f"processes; slowest took {dta:.1f} s"}
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()

@@ -348,7 +348,7 @@ def test_frame_errors(torch):
 
 
 # ---------------------------------------------------------------------------------------------- full size, bench configuration
-@pytest.mark.parametrize("name", ["C2", "C3"])
+@pytest.mark.parametrize("name", ["C1", "C2", "C3"])
 def test_full_size_sampled_pixels(torch, name):
     """BASELINE full size (800x800, 128 + 64x8 directions) in the launch configuration bench.py times; the oracle
     checks a seeded sample of pixels one by one (it needs ~6 ms per pixel)."""
