@@ -115,10 +115,38 @@ __device__ __forceinline__ void wait_layer(WgCtx& c) {
 }
 
 // ---------------------------------------------------------------------------------------------------- row stages
-// fp32 pair -> hi fp16x2 word and the fp16x2 word of the residual
+// packed fp32 pairs (sm_100 FFMA2 / FADD2): one issue slot for two lanes of fp32 work.  A scalar multiplicand is passed
+// twice and ptxas folds it into the broadcast form of the instruction; constant-bank pairs ride as uniform-register operands.
+__device__ __forceinline__ void fma2(float a0, float a1, float b0, float b1, float& c0, float& c1) {
+  asm("{\n\t.reg .b64 a, b, c;\n\tmov.b64 a, {%2, %3};\n\tmov.b64 b, {%4, %5};\n\tmov.b64 c, {%0, %1};\n\t"
+      "fma.rn.f32x2 c, a, b, c;\n\tmov.b64 {%0, %1}, c;\n\t}"
+      : "+f"(c0), "+f"(c1) : "f"(a0), "f"(a1), "f"(b0), "f"(b1));
+}
+__device__ __forceinline__ void add2(float a0, float a1, float b0, float b1, float& c0, float& c1) {
+  asm("{\n\t.reg .b64 a, b, c;\n\tmov.b64 a, {%2, %3};\n\tmov.b64 b, {%4, %5};\n\tadd.rn.f32x2 c, a, b;\n\tmov.b64 {%0, %1}, c;\n\t}"
+      : "=f"(c0), "=f"(c1) : "f"(a0), "f"(a1), "f"(b0), "f"(b1));
+}
+__device__ __forceinline__ void sub2(float a0, float a1, float b0, float b1, float& c0, float& c1) {
+  asm("{\n\t.reg .b64 a, b, c;\n\tmov.b64 a, {%2, %3};\n\tmov.b64 b, {%4, %5};\n\tsub.rn.f32x2 c, a, b;\n\tmov.b64 {%0, %1}, c;\n\t}"
+      : "=f"(c0), "=f"(c1) : "f"(a0), "f"(a1), "f"(b0), "f"(b1));
+}
+// fp32 pair -> hi fp16x2 word and the fp16x2 word of the residual.  hi is the fp32 value with its low 13 mantissa bits cleared
+// (10 kept = fp16's, so the conversion is exact inside the fp16 normal range the split_ok check of hashrender_create
+// guarantees), the residual a - hi is exact in fp32 and is rounded once to fp16: a = hi + lo to 2^-21 relative.
 __device__ __forceinline__ void split_pair(float a0, float a1, uint32_t& hi, uint32_t& lo) {
-  hi = pack_rn(a0, a1);
-  lo = pack_lo(hi, a0, a1);
+  const float m0 = __uint_as_float(__float_as_uint(a0) & 0xFFFFE000u), m1 = __uint_as_float(__float_as_uint(a1) & 0xFFFFE000u);
+  float l0, l1;
+  sub2(a0, a1, m0, m1, l0, l1);
+  hi = pack_rn(m0, m1);
+  lo = pack_rn(l0, l1);
+}
+// the same split of (max(a0, 0), max(a1, 0)): truncation keeps the sign of a and of a - hi, so the relu rides in both conversions
+__device__ __forceinline__ void split_pair_relu(float a0, float a1, uint32_t& hi, uint32_t& lo) {
+  const float m0 = __uint_as_float(__float_as_uint(a0) & 0xFFFFE000u), m1 = __uint_as_float(__float_as_uint(a1) & 0xFFFFE000u);
+  float l0, l1;
+  sub2(a0, a1, m0, m1, l0, l1);
+  hi = pack_relu(m0, m1);
+  lo = pack_relu(l0, l1);
 }
 
 // z_v = b3 + w3v . relu(D) with fp16x2 FMAs (b2 rode in the MMA); PREC = 0 direct / tertiary queries
@@ -151,10 +179,11 @@ __device__ __forceinline__ void epi_precise(uint32_t tD, const TcConst& cw, floa
     tmem_ld32(tD + 32 * h, r);
     wait_ld();
 #pragma unroll
-    for (int k = 0; k < 32; ++k) {
-      const float a = fmaxf(ADD_B2 ? __uint_as_float(r[k]) + cw.b2[32 * h + k] : __uint_as_float(r[k]), 0.f);
-      z0[k & 3] = fmaf(a, cw.w3[0][32 * h + k], z0[k & 3]);
-      z1[k & 3] = fmaf(a, cw.w3[1][32 * h + k], z1[k & 3]);
+    for (int k = 0; k < 32; k += 2) {
+      const float a0 = fmaxf(ADD_B2 ? __uint_as_float(r[k]) + cw.b2[32 * h + k] : __uint_as_float(r[k]), 0.f);
+      const float a1 = fmaxf(ADD_B2 ? __uint_as_float(r[k + 1]) + cw.b2[32 * h + k + 1] : __uint_as_float(r[k + 1]), 0.f);
+      fma2(cw.w3[0][32 * h + k], cw.w3[0][32 * h + k + 1], a0, a1, z0[k & 2], z0[(k & 2) + 1]);
+      fma2(cw.w3[1][32 * h + k], cw.w3[1][32 * h + k + 1], a0, a1, z1[k & 2], z1[(k & 2) + 1]);
     }
   }
   zv = (z0[0] + z0[1]) + (z0[2] + z0[3]);
@@ -168,7 +197,9 @@ __device__ __forceinline__ float epi_precise_v(uint32_t tD, const TcConst& cw) {
     tmem_ld32(tD + 32 * h, r);
     wait_ld();
 #pragma unroll
-    for (int k = 0; k < 32; ++k) z0[k & 3] = fmaf(fmaxf(__uint_as_float(r[k]), 0.f), cw.w3[0][32 * h + k], z0[k & 3]);
+    for (int k = 0; k < 32; k += 2)
+      fma2(cw.w3[0][32 * h + k], cw.w3[0][32 * h + k + 1], fmaxf(__uint_as_float(r[k]), 0.f), fmaxf(__uint_as_float(r[k + 1]), 0.f),
+           z0[k & 2], z0[(k & 2) + 1]);
   }
   return (z0[0] + z0[1]) + (z0[2] + z0[3]);
 }
@@ -184,7 +215,7 @@ __device__ __forceinline__ void hidden_to_A(uint32_t tD, uint32_t tA) {
     uint32_t p[16], q[16];
 #pragma unroll
     for (int k = 0; k < 16; ++k) {
-      if (SPLIT) split_pair(fmaxf(__uint_as_float(r[2 * k]), 0.f), fmaxf(__uint_as_float(r[2 * k + 1]), 0.f), p[k], q[k]);
+      if (SPLIT) split_pair_relu(__uint_as_float(r[2 * k]), __uint_as_float(r[2 * k + 1]), p[k], q[k]);
       else p[k] = pack_relu(__uint_as_float(r[2 * k]), __uint_as_float(r[2 * k + 1]));
     }
     tmem_st16(tA + 16 * h, p);
@@ -202,17 +233,17 @@ __device__ __forceinline__ void h1_dir(uint32_t tA, const TcConst& cw, PF P4, fl
     for (int k = 0; k < 8; ++k) {
       const float4 pv = P4(8 * h + k);
       const float pin[4] = {pv.x, pv.y, pv.z, pv.w};
-      float a[4];
+      float a[4] = {pin[0], pin[1], pin[2], pin[3]};
 #pragma unroll
-      for (int e = 0; e < 4; ++e) {
+      for (int e = 0; e < 4; e += 2) {
         const int j = 32 * h + 4 * k + e;
-        a[e] = fmaf(cw.w1w[0][j], wx, pin[e]);
-        a[e] = fmaf(cw.w1w[1][j], wy, a[e]);
-        a[e] = fmaf(cw.w1w[2][j], wz, a[e]);
+        fma2(cw.w1w[0][j], cw.w1w[0][j + 1], wx, wx, a[e], a[e + 1]);
+        fma2(cw.w1w[1][j], cw.w1w[1][j + 1], wy, wy, a[e], a[e + 1]);
+        fma2(cw.w1w[2][j], cw.w1w[2][j + 1], wz, wz, a[e], a[e + 1]);
       }
       if (SPLIT) {
-        split_pair(fmaxf(a[0], 0.f), fmaxf(a[1], 0.f), p[2 * k], q[2 * k]);
-        split_pair(fmaxf(a[2], 0.f), fmaxf(a[3], 0.f), p[2 * k + 1], q[2 * k + 1]);
+        split_pair_relu(a[0], a[1], p[2 * k], q[2 * k]);
+        split_pair_relu(a[2], a[3], p[2 * k + 1], q[2 * k + 1]);
       } else {
         p[2 * k] = pack_relu(a[0], a[1]);
         p[2 * k + 1] = pack_relu(a[2], a[3]);
@@ -260,8 +291,11 @@ __device__ __forceinline__ void h1_shared_split(uint32_t tA, const float (&P)[kH
     for (int k = 0; k < 8; ++k) {
       const float4 v = reinterpret_cast<const float4*>(Q)[8 * h + k];
       const int j = 32 * h + 4 * k;
-      split_pair(fmaxf(P[j] + v.x, 0.f), fmaxf(P[j + 1] + v.y, 0.f), p[2 * k], q[2 * k]);
-      split_pair(fmaxf(P[j + 2] + v.z, 0.f), fmaxf(P[j + 3] + v.w, 0.f), p[2 * k + 1], q[2 * k + 1]);
+      float a[4];
+      add2(P[j], P[j + 1], v.x, v.y, a[0], a[1]);
+      add2(P[j + 2], P[j + 3], v.z, v.w, a[2], a[3]);
+      split_pair_relu(a[0], a[1], p[2 * k], q[2 * k]);
+      split_pair_relu(a[2], a[3], p[2 * k + 1], q[2 * k + 1]);
     }
     tmem_st16(tA + 16 * h, p);
     tmem_st16(tA + 32 + 16 * h, q);
