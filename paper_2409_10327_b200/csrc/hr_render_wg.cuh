@@ -85,8 +85,10 @@ __device__ __forceinline__ void issue_layer(const WgCtx& c, uint32_t a_col, int 
                                             int bias_kstep, uint32_t idesc = kIdesc) {
   wait_st();
   fence_before();
-  wg_sync(c);
-  if (c.t < 32) {                               // warp 0 of the warpgroup, converged; one elected lane issues
+  if (c.t >= 32) {                              // warps 1..3 only announce their rows and go on to the work that needs no D
+    asm volatile("bar.arrive %0, 128;" ::"r"(c.bar_id) : "memory");
+  } else {                                      // warp 0 of the warpgroup, converged; one elected lane issues
+    wg_sync(c);
     fence_after();
     const uint32_t d = c.tmem + Cols<PREC, G>::d;
     const uint32_t a = c.tmem + a_col;
