@@ -417,7 +417,7 @@ def main():
         roof["kernel_ms"] = kernel_ms
         roof["algorithmic_flops_per_launch"] = flops
         roof["note"] = ("the MLP contractions run on the tensor pipe, but the kernel's binding unit is the SM issue slots: per query the "
-                        "fp16 pack / epilogue / shading ALU work exceeds the 64x64 MMA (DESIGN.md 6.2); see profiles/ for issue-slot "
+                        "fp16 pack / epilogue / shading ALU work exceeds the 64x64 MMA (DESIGN.md 6.1); see profiles/ for issue-slot "
                         "and tensor-pipe utilisation")
         tpath = os.path.join(ROOT, "profiles", "traffic.json")
         roof["traffic"] = None
