@@ -37,14 +37,8 @@ __device__ __forceinline__ void fence_after() { asm volatile("tcgen05.fence::aft
 __device__ __forceinline__ void wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 __device__ __forceinline__ void wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
 
-__device__ __forceinline__ void mma_f16_ts(uint32_t d_tmem, uint32_t a_tmem, uint64_t b_desc, uint32_t idesc, uint32_t accum) {
-  asm volatile(
-      "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
-      "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n\t}\n" ::"r"(d_tmem), "r"(a_tmem), "l"(b_desc), "r"(idesc), "r"(accum)
-      : "memory");
-}
-// Warp-level variants: the whole (converged) warp executes them and one elected lane issues, so the operands stay in the
-// uniform datapath instead of being broadcast lane by lane inside a divergent branch.
+// The whole (converged) warp executes these and one elected lane issues, so the operands stay in the uniform datapath
+// instead of being broadcast lane by lane inside a divergent branch.
 __device__ __forceinline__ void mma_f16_ts_elect(uint32_t d_tmem, uint32_t a_tmem, uint64_t b_desc, uint32_t idesc, uint32_t accum) {
   asm volatile(
       "{\n\t.reg .pred p, e;\n\tsetp.ne.b32 p, %4, 0;\n\telect.sync _|e, 0xffffffff;\n\t"
@@ -61,9 +55,6 @@ __device__ __forceinline__ void mma_f16_ss_elect(uint32_t d_tmem, uint64_t a_des
 __device__ __forceinline__ void mma_commit_elect(uint32_t mbar) {
   asm volatile("{\n\t.reg .pred e;\n\telect.sync _|e, 0xffffffff;\n\t"
                "@e tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];\n\t}\n" ::"r"(mbar) : "memory");
-}
-__device__ __forceinline__ void mma_commit(uint32_t mbar) {
-  asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(mbar) : "memory");
 }
 __device__ __forceinline__ void mbar_wait(uint32_t mbar, uint32_t parity) {
   uint32_t done;
@@ -136,12 +127,6 @@ constexpr uint32_t kIdesc = (1u << 4) | ((64u >> 3) << 17) | ((128u >> 4) << 24)
 constexpr uint32_t kIdescN16 = (1u << 4) | ((16u >> 3) << 17) | ((128u >> 4) << 24);
 
 // ---------------------------------------------------------------------------------------------------- encode pieces
-// residual of an fp16x2 pack: (a - fp16(a), b - fp16(b)) packed again (the "lo" half of a hi/lo split)
-__device__ __forceinline__ uint32_t pack_lo(uint32_t hi, float a, float b) {
-  const float2 h = __half22float2(*reinterpret_cast<const __half2*>(&hi));
-  return pack_rn(a - h.x, b - h.y);
-}
-
 // Secondary points: the gathers of one level (issued early) and their interpolation (consumed late) are separate so
 // the caller can put a whole tertiary query between them.  fp16 tables: the 8 half2 rows are interpolated with fp16x2
 // lerps (x, y, z: 7 sub + 7 fma) and the result IS the packed A-operand word.  The cell / index path is fp32 + integer,
