@@ -486,13 +486,15 @@ __global__ void __launch_bounds__(kRows* G, 1)
   fence_before();
   __syncthreads();
   fence_after();
-  c.tmem = *s_tmem + CL::stride * wgi;
+  // warp-uniform by construction; the reductions tell the compiler so, which keeps the MMA operands (TMEM addresses, smem
+  // descriptors, the mbarrier) in uniform registers instead of re-broadcasting them from a lane before every tcgen05.mma
+  c.tmem = __reduce_min_sync(0xFFFFFFFFu, *s_tmem + CL::stride * wgi);
   c.lane = (uint32_t)((warp & 3) * 32) << 16;
-  c.mbar = smem_u32(s_mbar + wgi);
+  c.mbar = __reduce_min_sync(0xFFFFFFFFu, smem_u32(s_mbar + wgi));
   c.phase = 0;
-  c.tile0 = smem_u32(s_tiles);
+  c.tile0 = __reduce_min_sync(0xFFFFFFFFu, smem_u32(s_tiles));
   c.lo_off = kHiTileBytes;
-  c.ones = smem_u32(s_ones);
+  c.ones = __reduce_min_sync(0xFFFFFFFFu, smem_u32(s_ones));
   const uint32_t tA = c.tmem + c.lane, tD = c.tmem + c.lane + CL::d;
   uint8_t* my = s_wg + wgi * SP::per_wg;
   float* Ps = reinterpret_cast<float*>(my) + c.t;                                     // Ps[k * 128]
@@ -737,9 +739,11 @@ __global__ void __launch_bounds__(kRows* kTraceG, 1)
   fence_before();
   __syncthreads();
   fence_after();
-  c.tmem = *s_tmem + CL::stride * wgi;
+  // warp-uniform by construction; the reductions tell the compiler so, which keeps the MMA operands (TMEM addresses, smem
+  // descriptors, the mbarrier) in uniform registers instead of re-broadcasting them from a lane before every tcgen05.mma
+  c.tmem = __reduce_min_sync(0xFFFFFFFFu, *s_tmem + CL::stride * wgi);
   c.lane = (uint32_t)((warp & 3) * 32) << 16;
-  c.mbar = smem_u32(s_mbar + wgi);
+  c.mbar = __reduce_min_sync(0xFFFFFFFFu, smem_u32(s_mbar + wgi));
   c.phase = 0;
   c.tile0 = smem_u32(s_tiles);
   c.lo_off = 0;
