@@ -489,7 +489,7 @@ __global__ void __launch_bounds__(kRows* G, 1)
   // warp-uniform by construction; the reductions tell the compiler so, which keeps the MMA operands (TMEM addresses, smem
   // descriptors, the mbarrier) in uniform registers instead of re-broadcasting them from a lane before every tcgen05.mma
   c.tmem = __reduce_min_sync(0xFFFFFFFFu, *s_tmem + CL::stride * wgi);
-  c.lane = (uint32_t)((warp & 3) * 32) << 16;
+  c.lane = __reduce_min_sync(0xFFFFFFFFu, (uint32_t)((warp & 3) * 32) << 16);     // tcgen05.ld / st addresses are uniform operands too
   c.mbar = __reduce_min_sync(0xFFFFFFFFu, smem_u32(s_mbar + wgi));
   c.phase = 0;
   c.tile0 = __reduce_min_sync(0xFFFFFFFFu, smem_u32(s_tiles));
@@ -742,7 +742,7 @@ __global__ void __launch_bounds__(kRows* kTraceG, 1)
   // warp-uniform by construction; the reductions tell the compiler so, which keeps the MMA operands (TMEM addresses, smem
   // descriptors, the mbarrier) in uniform registers instead of re-broadcasting them from a lane before every tcgen05.mma
   c.tmem = __reduce_min_sync(0xFFFFFFFFu, *s_tmem + CL::stride * wgi);
-  c.lane = (uint32_t)((warp & 3) * 32) << 16;
+  c.lane = __reduce_min_sync(0xFFFFFFFFu, (uint32_t)((warp & 3) * 32) << 16);     // tcgen05.ld / st addresses are uniform operands too
   c.mbar = __reduce_min_sync(0xFFFFFFFFu, smem_u32(s_mbar + wgi));
   c.phase = 0;
   c.tile0 = smem_u32(s_tiles);
