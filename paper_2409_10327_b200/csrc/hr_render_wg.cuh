@@ -364,12 +364,43 @@ __device__ __forceinline__ void encode_fast_to(uint32_t tA, const GridP& g, floa
   }
 }
 
+// One level of the fp32 encode in two halves, so that the caller can put a whole tertiary query between the gathers and
+// their first use (the arithmetic is encode_level's).
+template <bool F16TAB> struct Taps32 { float2 v[8]; float w[3]; };
+template <bool F16TAB>
+__device__ __forceinline__ void gather32(const GridP& g, int l, float x, float y, float z, Taps32<F16TAB>& t) {
+  const uint32_t N = g.res[l];
+  const Cell c = cell_of(N, x, y, z);
+  uint32_t idx[8];
+  corner_indices(c, N, (g.dense_mask >> l) & 1u, g.log2_T, idx);
+  const void* lb = level_base<F16TAB>(g.tables, g.log2_T, l);
+#pragma unroll
+  for (int k = 0; k < 8; ++k) t.v[k] = table_load<F16TAB>(lb, idx[k]);
+  t.w[0] = c.w[0]; t.w[1] = c.w[1]; t.w[2] = c.w[2];
+}
+// interpolate, split, store the level's fp16x2 words to TMEM columns tF + l (hi) and tF + 16 + l (lo)
+template <bool F16TAB>
+__device__ __forceinline__ void finish32(uint32_t tF, int l, const Taps32<F16TAB>& t) {
+  const float wx[2] = {1.f - t.w[0], t.w[0]}, wy[2] = {1.f - t.w[1], t.w[1]}, wz[2] = {1.f - t.w[2], t.w[2]};
+  float2 f = make_float2(0.f, 0.f);
+#pragma unroll
+  for (int k = 0; k < 8; ++k) {
+    const float wt = wx[k & 1] * wy[(k >> 1) & 1] * wz[(k >> 2) & 1];
+    f.x = fmaf(wt, t.v[k].x, f.x);
+    f.y = fmaf(wt, t.v[k].y, f.y);
+  }
+  uint32_t hi, lo;
+  split_pair(f.x, f.y, hi, lo);
+  asm volatile("tcgen05.st.sync.aligned.32x32b.x1.b32 [%0], {%1};" ::"r"(tF + l), "r"(hi) : "memory");
+  asm volatile("tcgen05.st.sync.aligned.32x32b.x1.b32 [%0], {%1};" ::"r"(tF + 16 + l), "r"(lo) : "memory");
+}
+
 // B over the features at A columns 0.. (hi | lo when PREC = 1): all three layers on the tensor core, biases of layers 1-2
 // ride as K-steps, layer 3 is an N = 16 MMA over the zero-padded 7-row W3; b3 is added in registers.
 template <int PREC, int G>
-__device__ __forceinline__ void brdf_mma(WgCtx& c, const TcConst& cw, const ShadeP& sp, float (&b)[7]) {
+__device__ __forceinline__ void brdf_mma(WgCtx& c, const TcConst& cw, const ShadeP& sp, float (&b)[7], uint32_t f_col = 0) {
   const uint32_t tA = c.tmem + c.lane, tD = c.tmem + c.lane + Cols<PREC, G>::d;
-  issue_layer<PREC, G>(c, 0, 1, 2, PREC == 1, 1, 2);
+  issue_layer<PREC, G>(c, f_col, 1, 2, PREC == 1, 1, 2);
   wait_layer(c);
   hidden_to_A<PREC == 1>(tD, tA);
   issue_layer<PREC, G>(c, 0, 3, 4, PREC == 1, 1, 3);
@@ -513,7 +544,15 @@ __global__ void __launch_bounds__(kRows* G, 1)
   uint32_t head = 0;                                                                  // mirrored in registers (uniform in the WG)
 
   // ---- phase C: one 128-item group, one item per thread -------------------------------------------------------------
-  auto drain_group = [&](uint32_t count, unsigned long long tile_base) {
+  // Split-precision kernel at G = 3: the warpgroup's 168 TMEM columns leave 40 beside A and D.  Columns 128..159 hold the
+  // features f' (hi | lo) of a group, and while a group runs its tertiary queries it encodes the NEXT group's points into
+  // them, two levels per query: the gathers of a level are issued before the query's row arithmetic / MMA wait and used
+  // after it, so their L2 latency costs nothing (it was 19 % of the kernel's stall samples).
+  constexpr bool kPre = PREC == 1 && TSHARED && G == 3;
+  constexpr uint32_t kFCol = kPre ? 128u : 0u;
+  const uint32_t tF = tA + kFCol;
+  bool pre_done = false;                                                              // tF holds the features of the next group
+  auto drain_group = [&](uint32_t count, unsigned long long tile_base, uint32_t next_count) {
     const bool on = (uint32_t)c.t < count;
     float ix = 0.5f, iy = 0.5f, iz = 0.5f, iwx = 0.f, iwy = 0.f, iwz = 1.f, wr = 0.f, wgc = 0.f, wb = 0.f;
     uint32_t owner = 0;
@@ -524,9 +563,16 @@ __global__ void __launch_bounds__(kRows* G, 1)
       owner = __float_as_uint(c4.y);
     }
     // a1-a4 at x', then P' = W1f f' + b1
-    if (PREC == 1) encode_split_to<F16TAB, LIF>(tA, g, ix, iy, iz);
+    if (PREC == 1) { if (!(kPre && pre_done)) encode_split_to<F16TAB, LIF>(tF, g, ix, iy, iz); }
     else encode_fast_to<F16TAB, LIF>(tA, g, ix, iy, iz);
-    issue_layer<PREC, G>(c, 0, 0, 2, PREC == 1, 0, 2);
+    issue_layer<PREC, G>(c, kFCol, 0, 2, PREC == 1, 0, 2);
+    // the next group's points (kPre): positions only, the rest of the item is read when its turn comes
+    float nx = 0.5f, ny = 0.5f, nz = 0.5f;
+    const bool pre = kPre && next_count > 0u && S2 >= 8u;                              // WG-uniform
+    if (pre && (uint32_t)c.t < next_count) {
+      const float4 a = __ldcg(reinterpret_cast<const float4*>(myring + ((head + count + c.t) & (kRing - 1))));
+      nx = a.x; ny = a.y; nz = a.z;
+    }
     wait_layer(c);
     uint32_t P2h[kH / 2];                                             // only the one the instantiation uses survives
     float P2[kH];
@@ -536,13 +582,16 @@ __global__ void __launch_bounds__(kRows* G, 1)
       store_D_f4(tD, P2s4);
     }
     float bb[7];
-    brdf_mma<PREC, G>(c, cw, sp, bb);                                 // a5 at x' (A columns 0.. still hold f')
+    brdf_mma<PREC, G>(c, cw, sp, bb, kFCol);                          // a5 at x' (the feature columns still hold f')
     // a8: Eq. 1 at x' over the tertiary set, w_o' = -w_j
     const unsigned long long trow = TSHARED ? 0ull : (tile_base + (owner & 0xFFu)) * (unsigned long long)fr.s.S + (owner >> 8);
     float lr = 0.f, lg = 0.f, lb = 0.f;
     for (uint32_t k = 0; k < S2; ++k) {
       float tx, ty, tz, tpdf;
       float3 L;
+      Taps32<F16TAB> taps;
+      const bool pre_k = pre && k < 8u;                               // levels 2k, 2k+1 of the next group ride in this query
+      if (kPre && pre_k) gather32<F16TAB>(g, 2 * (int)k, nx, ny, nz, taps);
       if constexpr (TSHARED) {
         if constexpr (PREC == 0) h1_shared_h2(tA, P2h, reinterpret_cast<const uint32_t*>(s_Qt) + k * (kH / 2));
         else h1_shared_split(tA, P2, s_Qt + k * kH);
@@ -550,7 +599,9 @@ __global__ void __launch_bounds__(kRows* G, 1)
         const float* tp = dir_of(fr.t, trow, k);
         h1_dir<PREC == 1>(tA, cw, [&](int q) { return P2s4[q * kRows]; }, __ldg(tp), __ldg(tp + 1), __ldg(tp + 2));
       }
+      if (kPre && pre_k) finish32<F16TAB>(tF, 2 * (int)k, taps);
       issue_layer<PREC, G>(c, 0, 2, 4, PREC == 1, 0, 3);
+      if (kPre && pre_k) gather32<F16TAB>(g, 2 * (int)k + 1, nx, ny, nz, taps);
       if (TSHARED) {                                                  // shading factors: they do not need the MMA
         const float4 a = reinterpret_cast<const float4*>(s_Lt)[2 * k], d = reinterpret_cast<const float4*>(s_Lt)[2 * k + 1];
         L = make_float3(a.x, a.y, a.z); tpdf = a.w; tx = d.x; ty = d.y; tz = d.z;
@@ -561,9 +612,11 @@ __global__ void __launch_bounds__(kRows* G, 1)
       }
       const float3 gg = brdf_cos_over_pdf(sp, bb, tx, ty, tz, -iwx, -iwy, -iwz, tpdf);
       wait_layer(c);
+      if (kPre && pre_k) finish32<F16TAB>(tF, 2 * (int)k + 1, taps);
       const float v2 = vis_of(sp, PREC == 0 ? epi_fast(tD, cw) : epi_precise_v(tD, cw));
       lr = fmaf(v2 * L.x, gg.x, lr); lg = fmaf(v2 * L.y, gg.y, lg); lb = fmaf(v2 * L.z, gg.z, lb);
     }
+    pre_done = pre;
     if (on) {
       float* a = acc + 4 * (owner & 0xFFu);
       atomicAdd(a, wr * lr); atomicAdd(a + 1, wgc * lg); atomicAdd(a + 2, wb * lb);
@@ -672,7 +725,9 @@ __global__ void __launch_bounds__(kRows* G, 1)
         const bool last = j1 == S_i;
         while (__any_sync(0xFFFFFFFFu, count >= (uint32_t)kRows || (last && count > 0u))) {
           const uint32_t n = count < (uint32_t)kRows ? count : (uint32_t)kRows;
-          drain_group(n, tile_base);
+          const uint32_t rest = count - n;                            // the group after this one, if it will be drained next
+          const uint32_t nn = (rest >= (uint32_t)kRows || (last && rest > 0u)) ? (rest < (uint32_t)kRows ? rest : (uint32_t)kRows) : 0u;
+          drain_group(n, tile_base, nn);
           head += n; count -= n;
           n_items += (uint32_t)c.t < n ? 1u : 0u;
         }
