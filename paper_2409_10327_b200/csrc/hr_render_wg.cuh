@@ -34,8 +34,8 @@ namespace wg {
 using namespace hr::tc;
 
 constexpr int kRows = 128;                    // rows (threads) per warpgroup
-constexpr int kRing = 1024;                   // work items per WG ring (power of two, >= 127 + kChunkJ * 128)
-constexpr int kChunkJ = 4;                    // secondary directions traced between two drains
+constexpr int kRing = 2048;                   // work items per WG ring (power of two, >= 127 + kChunkJ * 128)
+constexpr int kChunkJ = 8;                    // secondary directions traced between two drains
 constexpr int kMaxG = 4;
 constexpr int kMaxS2 = tc::kMaxS2;              // shared tertiary set staged in shared memory
 constexpr int kHiTileBytes = kNumTiles * kTileBytes + kTile3Bytes;       // 34 KB: I.W1f, B.W1, I.W2, B.W2, B.W3
@@ -548,8 +548,10 @@ __global__ void __launch_bounds__(kRows* G, 1)
   // features f' (hi | lo) of a group, and while a group runs its tertiary queries it encodes the NEXT group's points into
   // them, two levels per query: the gathers of a level are issued before the query's row arithmetic / MMA wait and used
   // after it, so their L2 latency costs nothing (it was 19 % of the kernel's stall samples).
-  constexpr bool kPre = PREC == 1 && TSHARED && G == 3;
-  constexpr uint32_t kFCol = kPre ? 128u : 0u;
+  // (The fp16 kernel has columns 32..63 free and the code below serves it too, but at its 128-register budget the extra
+  // live taps spill and its queries are too short to cover a gather: measured 18.5 ms against 16.7 ms, so it stays off.)
+  constexpr bool kPre = TSHARED && PREC == 1 && G == 3;
+  constexpr uint32_t kFCol = !kPre ? 0u : (PREC == 1 ? 128u : 32u);
   const uint32_t tF = tA + kFCol;
   bool pre_done = false;                                                              // tF holds the features of the next group
   auto drain_group = [&](uint32_t count, unsigned long long tile_base, uint32_t next_count) {
@@ -564,7 +566,7 @@ __global__ void __launch_bounds__(kRows* G, 1)
     }
     // a1-a4 at x', then P' = W1f f' + b1
     if (PREC == 1) { if (!(kPre && pre_done)) encode_split_to<F16TAB, LIF>(tF, g, ix, iy, iz); }
-    else encode_fast_to<F16TAB, LIF>(tA, g, ix, iy, iz);
+    else { if (!(kPre && pre_done)) encode_fast_to<F16TAB, LIF>(tF, g, ix, iy, iz); }
     issue_layer<PREC, G>(c, kFCol, 0, 2, PREC == 1, 0, 2);
     // the next group's points (kPre): positions only, the rest of the item is read when its turn comes
     float nx = 0.5f, ny = 0.5f, nz = 0.5f;
@@ -589,9 +591,17 @@ __global__ void __launch_bounds__(kRows* G, 1)
     for (uint32_t k = 0; k < S2; ++k) {
       float tx, ty, tz, tpdf;
       float3 L;
-      Taps32<F16TAB> taps;
+      Taps32<F16TAB> taps;                                            // PREC 1: fp32 taps; PREC 0: fp16x2 taps (only one survives)
+      LevelTaps<F16TAB> htaps;
+      auto pre_gather = [&](int l) {
+        if constexpr (PREC == 1) gather32<F16TAB>(g, l, nx, ny, nz, taps); else gather_level<F16TAB>(g, l, nx, ny, nz, htaps);
+      };
+      auto pre_finish = [&](int l) {
+        if constexpr (PREC == 1) finish32<F16TAB>(tF, l, taps);
+        else asm volatile("tcgen05.st.sync.aligned.32x32b.x1.b32 [%0], {%1};" ::"r"(tF + l), "r"(lerp_level(htaps)) : "memory");
+      };
       const bool pre_k = pre && k < 8u;                               // levels 2k, 2k+1 of the next group ride in this query
-      if (kPre && pre_k) gather32<F16TAB>(g, 2 * (int)k, nx, ny, nz, taps);
+      if (kPre && pre_k) pre_gather(2 * (int)k);
       if constexpr (TSHARED) {
         if constexpr (PREC == 0) h1_shared_h2(tA, P2h, reinterpret_cast<const uint32_t*>(s_Qt) + k * (kH / 2));
         else h1_shared_split(tA, P2, s_Qt + k * kH);
@@ -599,9 +609,9 @@ __global__ void __launch_bounds__(kRows* G, 1)
         const float* tp = dir_of(fr.t, trow, k);
         h1_dir<PREC == 1>(tA, cw, [&](int q) { return P2s4[q * kRows]; }, __ldg(tp), __ldg(tp + 1), __ldg(tp + 2));
       }
-      if (kPre && pre_k) finish32<F16TAB>(tF, 2 * (int)k, taps);
+      if (kPre && pre_k) pre_finish(2 * (int)k);
       issue_layer<PREC, G>(c, 0, 2, 4, PREC == 1, 0, 3);
-      if (kPre && pre_k) gather32<F16TAB>(g, 2 * (int)k + 1, nx, ny, nz, taps);
+      if (kPre && pre_k) pre_gather(2 * (int)k + 1);
       if (TSHARED) {                                                  // shading factors: they do not need the MMA
         const float4 a = reinterpret_cast<const float4*>(s_Lt)[2 * k], d = reinterpret_cast<const float4*>(s_Lt)[2 * k + 1];
         L = make_float3(a.x, a.y, a.z); tpdf = a.w; tx = d.x; ty = d.y; tz = d.z;
@@ -612,7 +622,7 @@ __global__ void __launch_bounds__(kRows* G, 1)
       }
       const float3 gg = brdf_cos_over_pdf(sp, bb, tx, ty, tz, -iwx, -iwy, -iwz, tpdf);
       wait_layer(c);
-      if (kPre && pre_k) finish32<F16TAB>(tF, 2 * (int)k + 1, taps);
+      if (kPre && pre_k) pre_finish(2 * (int)k + 1);
       const float v2 = vis_of(sp, PREC == 0 ? epi_fast(tD, cw) : epi_precise_v(tD, cw));
       lr = fmaf(v2 * L.x, gg.x, lr); lg = fmaf(v2 * L.y, gg.y, lg); lb = fmaf(v2 * L.z, gg.z, lb);
     }
