@@ -125,6 +125,7 @@ __device__ __forceinline__ uint64_t make_bdesc(uint32_t smem_addr) {
 // kind::f16, A/B = F16 K-major, D = F32, M = 128, N = 64
 constexpr uint32_t kIdesc = (1u << 4) | ((64u >> 3) << 17) | ((128u >> 4) << 24);
 constexpr uint32_t kIdescN16 = (1u << 4) | ((16u >> 3) << 17) | ((128u >> 4) << 24);
+constexpr uint32_t kIdescN128 = (1u << 4) | ((128u >> 3) << 17) | ((128u >> 4) << 24);
 
 // ---------------------------------------------------------------------------------------------------- encode pieces
 // Secondary points: the gathers of one level (issued early) and their interpolation (consumed late) are separate so

@@ -82,7 +82,7 @@ __device__ __forceinline__ void wg_sync(const WgCtx& c) { asm volatile("bar.sync
 // block follows the hi block; PREC = 1 adds the pass against the lo weights.  All threads must have stored their A rows.
 template <int PREC, int G>
 __device__ __forceinline__ void issue_layer(const WgCtx& c, uint32_t a_col, int tile, int ksteps, bool split_a, int bias_tile,
-                                            int bias_kstep, uint32_t idesc = kIdesc) {
+                                            int bias_kstep, uint32_t idesc = kIdesc, uint32_t d_col = Cols<PREC, G>::d) {
   wait_st();
   fence_before();
   if (c.t >= 32) {                              // warps 1..3 only announce their rows and go on to the work that needs no D
@@ -90,7 +90,7 @@ __device__ __forceinline__ void issue_layer(const WgCtx& c, uint32_t a_col, int 
   } else {                                      // warp 0 of the warpgroup, converged; one elected lane issues
     wg_sync(c);
     fence_after();
-    const uint32_t d = c.tmem + Cols<PREC, G>::d;
+    const uint32_t d = c.tmem + d_col;
     const uint32_t a = c.tmem + a_col;
     const uint64_t bd = make_bdesc(c.tile0 + tile * kTileBytes);
     for (int k = 0; k < ksteps; ++k) mma_f16_ts_elect(d, a + 8 * k, bd + 2 * k, idesc, k > 0);
@@ -398,10 +398,13 @@ __device__ __forceinline__ void finish32(uint32_t tF, int l, const Taps32<F16TAB
 // B over the features at A columns 0.. (hi | lo when PREC = 1): all three layers on the tensor core, biases of layers 1-2
 // ride as K-steps, layer 3 is an N = 16 MMA over the zero-padded 7-row W3; b3 is added in registers.
 template <int PREC, int G>
-__device__ __forceinline__ void brdf_mma(WgCtx& c, const TcConst& cw, const ShadeP& sp, float (&b)[7], uint32_t f_col = 0) {
+__device__ __forceinline__ void brdf_mma(WgCtx& c, const TcConst& cw, const ShadeP& sp, float (&b)[7], uint32_t f_col = 0,
+                                         bool l1_done = false) {
   const uint32_t tA = c.tmem + c.lane, tD = c.tmem + c.lane + Cols<PREC, G>::d;
-  issue_layer<PREC, G>(c, f_col, 1, 2, PREC == 1, 1, 2);
-  wait_layer(c);
+  if (!l1_done) {                               // l1_done: the caller's N = 128 MMA has already left layer 1 in D
+    issue_layer<PREC, G>(c, f_col, 1, 2, PREC == 1, 1, 2);
+    wait_layer(c);
+  }
   hidden_to_A<PREC == 1>(tD, tA);
   issue_layer<PREC, G>(c, 0, 3, 4, PREC == 1, 1, 3);
   wait_layer(c);
@@ -567,7 +570,11 @@ __global__ void __launch_bounds__(kRows* G, 1)
     // a1-a4 at x', then P' = W1f f' + b1
     if (PREC == 1) { if (!(kPre && pre_done)) encode_split_to<F16TAB, LIF>(tF, g, ix, iy, iz); }
     else { if (!(kPre && pre_done)) encode_fast_to<F16TAB, LIF>(tF, g, ix, iy, iz); }
-    issue_layer<PREC, G>(c, kFCol, 0, 2, PREC == 1, 0, 2);
+    // kPre: the features sit outside columns 0..127, so P' (I.W1f, tile 0) and layer 1 of B (B.W1, tile 1: the next 64 rows of
+    // the same shared-memory tile, its bias in the same K-step) are ONE N = 128 MMA set into columns 0..127: P' lands in
+    // 0..63, B's layer 1 in 64..127 where D always is -- one barrier / commit / wait round trip less per group.
+    if constexpr (kPre) issue_layer<PREC, G>(c, kFCol, 0, 2, true, 0, 2, kIdescN128, 0u);
+    else issue_layer<PREC, G>(c, kFCol, 0, 2, PREC == 1, 0, 2);
     // the next group's points (kPre): positions only, the rest of the item is read when its turn comes
     float nx = 0.5f, ny = 0.5f, nz = 0.5f;
     const bool pre = kPre && next_count > 0u && S2 >= 8u;                              // WG-uniform
@@ -579,12 +586,12 @@ __global__ void __launch_bounds__(kRows* G, 1)
     uint32_t P2h[kH / 2];                                             // only the one the instantiation uses survives
     float P2[kH];
     if constexpr (TSHARED) {
-      if constexpr (PREC == 0) load_D_h2(tD, P2h); else load_D_f32(tD, P2);
+      if constexpr (PREC == 0) load_D_h2(tD, P2h); else load_D_f32(kPre ? tA : tD, P2);
     } else {
       store_D_f4(tD, P2s4);
     }
     float bb[7];
-    brdf_mma<PREC, G>(c, cw, sp, bb, kFCol);                          // a5 at x' (the feature columns still hold f')
+    brdf_mma<PREC, G>(c, cw, sp, bb, kFCol, kPre);                    // a5 at x' (the feature columns still hold f')
     // a8: Eq. 1 at x' over the tertiary set, w_o' = -w_j
     const unsigned long long trow = TSHARED ? 0ull : (tile_base + (owner & 0xFFu)) * (unsigned long long)fr.s.S + (owner >> 8);
     float lr = 0.f, lg = 0.f, lb = 0.f;
