@@ -616,9 +616,8 @@ __global__ void __launch_bounds__(kRows* G, 1)
         const float* tp = dir_of(fr.t, trow, k);
         h1_dir<PREC == 1>(tA, cw, [&](int q) { return P2s4[q * kRows]; }, __ldg(tp), __ldg(tp + 1), __ldg(tp + 2));
       }
-      if (kPre && pre_k) pre_finish(2 * (int)k);
       issue_layer<PREC, G>(c, 0, 2, 4, PREC == 1, 0, 3);
-      if (kPre && pre_k) pre_gather(2 * (int)k + 1);
+      if (kPre && pre_k) { pre_finish(2 * (int)k); pre_gather(2 * (int)k + 1); }
       if (TSHARED) {                                                  // shading factors: they do not need the MMA
         const float4 a = reinterpret_cast<const float4*>(s_Lt)[2 * k], d = reinterpret_cast<const float4*>(s_Lt)[2 * k + 1];
         L = make_float3(a.x, a.y, a.z); tpdf = a.w; tx = d.x; ty = d.y; tz = d.z;
