@@ -212,7 +212,7 @@ def run_c4_sweep(args):
     print(json.dumps({"metric": "encode+IRT points/s (BASELINE.json configs[4] sweep)", "value": best["points_per_s"], "unit": "points/s", "n_gpus": 1,
                       "steps": args.steps, "warmup": 3, "ms_per_step": best["ms"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
                       "dtype": "f16", "data": "synthetic", "config": {"workload": "C4 sweep: uniform random points x 1 direction, fp16 L=16 F=2",
-                      "points": "generated on device (torch Philox); parity of this path is covered by tests at C0/C1/C3 shapes"},
+                      "points": "generated on device (torch Philox); parity of this call at every table size of the sweep: tests/test_gpu_parity.py::test_c4_sweep_full_size_sampled_points"},
                       "hbm_peak_GBps": peaks["hbm"], "roofline": roof, "sweep": rows}))
 
 

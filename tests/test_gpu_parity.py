@@ -369,3 +369,62 @@ def test_full_size_sampled_pixels(torch, name):
     # a generator subset reproduces the same inputs as the full frame (so bench's CPU sample is the same workload)
     fr_sub = gen.make_frame(cfg, m["env"], pix)
     assert np.array_equal(fr_sub["dir_d"], sub["dir_d"]) and np.array_equal(fr_sub["x"], sub["x"])
+
+
+@pytest.mark.parametrize("log2_T", [16, 19, 22, 24])
+def test_c4_sweep_full_size_sampled_points(torch, log2_T):
+    """BASELINE.json configs[4]: encode + IRT over 2^20 uniform random points x 1 direction (fp16, L=16, F=2) at every table
+    size of the sweep, through the call bench.py --workload C4 times (hashrender_trace with the encode fused, full N in one
+    launch).  The oracle checks a seeded sample of points one by one: indices / fractional positions bit-exact at this T
+    (the dense / hashed split of the levels moves with T), v / t / x' within the fp16 tolerance, hard
+    visibility equal wherever |z_v| >= delta."""
+    from paper_2409_10327_b200 import DirSet
+    cfg = gen.make_config("C4", log2_T=log2_T)
+    assert cfg.N == 1 << 20 and cfg.S_d == 1
+    m = gen.make_model(cfg)
+    fr = gen.make_frame(cfg, m["env"])
+    N = cfg.N
+    rng = np.random.default_rng(44)
+    pix = np.sort(np.concatenate([rng.choice(N, 3000, replace=False), np.arange(N - 77, N), [0, 127, 128]]))
+    xs_in, ds_in = fr["x"][pix], fr["dir_d"][pix]
+    o = _oracle(cfg, m)
+    feat_o, idx_o, w_o = o.encode(xs_in)
+    vis_o, zv_o, t_o, x2_o = o.trace(xs_in, feat_o, ds_in)
+    n_dense = int(sum((int(n) + 1) ** 3 <= cfg.T for n in m["res"]))
+    assert n_dense == {16: 3, 19: 5, 22: 8, 24: 9}[log2_T]              # SURVEY Q3's list
+    assert idx_o.max() < cfg.T and (log2_T < 22 or idx_o.max() >= (1 << (log2_T - 1)))
+    r = make_renderer(cfg, m, max_points=N)
+    xd = to_dev(fr["x"]); ds = DirSet(to_dev(fr["dir_d"]), to_dev(fr["pdf_d"]))
+    vis = torch.empty((N, 1), device="cuda"); zv = torch.empty((N, 1), device="cuda"); t = torch.empty((N, 1), device="cuda")
+    x2 = torch.empty((N, 1, 3), device="cuda")
+    r.trace(xd, None, ds, vis, zv, t, x2, N=N)
+    torch.cuda.synchronize()
+    assert r.last_path() == "tcgen05-f16", r.last_path()                # k_trace_wg, the kernel the sweep times
+    pd = to_dev(pix)
+    got = [a[pd].cpu().numpy() for a in (vis, zv, t, x2)]
+    assert all(np.all(np.isfinite(g)) for g in got)
+    assert bool(torch.isfinite(t).all()) and float(t.min()) >= 0.05 and float(t.max()) <= 1.5
+    check_close(got[0], vis_o, TOL16, what=f"C4 T=2^{log2_T} vis")
+    check_close(got[1], zv_o, TOL16, extra=TOL16 * 0.05, what=f"C4 T=2^{log2_T} zv")
+    check_close(got[2], t_o, TOL16, what=f"C4 T=2^{log2_T} t")
+    check_close(got[3], x2_o, TOL16, what=f"C4 T=2^{log2_T} x'")
+    # the index path at this table size, bit-exact
+    n = len(pix)
+    feat = torch.empty((n, cfg.D), device="cuda"); idx = torch.empty((n, cfg.L, 8), device="cuda", dtype=torch.int32)
+    w = torch.empty((n, cfg.L, 3), device="cuda")
+    r.encode(to_dev(xs_in), feat, idx, w)
+    torch.cuda.synchronize()
+    assert np.array_equal(idx.cpu().numpy().view(np.uint32), idx_o)
+    assert np.array_equal(w.cpu().numpy(), w_o)
+    check_close(feat.cpu().numpy(), feat_o, 2e-6, what=f"C4 T=2^{log2_T} encode")
+    # hard visibility, same launch shape without the optional outputs (what bench.py passes)
+    r.destroy()
+    rh = make_renderer(cfg, m, vis_mode=1, max_points=N)
+    rh.trace(xd, None, ds, vis, None, t, N=N)
+    torch.cuda.synchronize()
+    vh = vis[pd].cpu().numpy()
+    assert set(np.unique(vh)) <= {0.0, 1.0}
+    sure = np.abs(zv_o) >= DELTA16
+    assert np.array_equal(vh[sure], (zv_o[sure] > 0).astype(np.float32)) and sure.mean() > 0.9
+    check_close(t[pd].cpu().numpy(), t_o, TOL16, what=f"C4 T=2^{log2_T} t (hard)")
+    rh.destroy()
