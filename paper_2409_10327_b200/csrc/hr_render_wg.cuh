@@ -667,6 +667,12 @@ __global__ void __launch_bounds__(kRows* G, 1)
       brdf_decode_scr<kRows>(sp, wts32, Ps, b);
     }
     wait_layer(c);
+    // Ps (one float column per thread, used by brdf_decode_scr as its 64-entry scratch) and Ps4 (one float4 column per thread)
+    // are two layouts of the SAME shared memory: a thread's float4 entries cover other threads' scratch entries.  Warps run
+    // ahead of one another between barriers (warps 1-3 only bar.arrive in issue_layer), so every warp must have left
+    // brdf_decode_scr before any warp stores P in the float4 layout -- without this barrier a fast warp corrupted a slow
+    // warp's primary BRDF (or had its P overwritten) in about one frame out of ten: 32 pixels of one warp, errors up to 0.5.
+    if (PREC == 1 && decode) wg_sync(c);
     store_D_f4(tD, Ps4);
     if (!decode) {
 #pragma unroll
