@@ -63,17 +63,22 @@ def load_peaks():
 
 
 class ClockSampler:
-    """Samples nvidia-smi clocks + throttle reasons while the timed region runs (B200_PROFILING.md clocks line)."""
+    """Samples nvidia-smi clocks + throttle reasons while the timed region runs (B200_PROFILING.md clocks line).  The nvidia-smi
+    loop is started before the warm-up (it needs ~0.2 s to come up) and every row is stamped on arrival; stop() keeps the rows
+    that arrived between begin() and end()."""
     Q = ("clocks.sm,clocks.max.sm,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
          "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
 
     def __init__(self, index: int):
         self.index, self.rows, self.proc = index, [], None
+        self.t0, self.t1, self.window = None, None, "timed region"
 
     def start(self):
+        if self.proc:
+            return
         try:
             self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-i", str(self.index),
-                                          "-lms", "100"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+                                          "-lms", "50"], stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
             self.th = threading.Thread(target=self._read, daemon=True)
             self.th.start()
         except Exception:
@@ -81,22 +86,34 @@ class ClockSampler:
 
     def _read(self):
         for line in self.proc.stdout:
-            self.rows.append([c.strip() for c in line.split(",")])
+            self.rows.append((time.time(), [c.strip() for c in line.split(",")]))
+
+    def begin(self):
+        self.t0 = time.time()
+
+    def end(self, window=None):
+        self.t1 = time.time()
+        if window:
+            self.window = window
+
+    def in_window(self):
+        return [r for (ts, r) in self.rows if len(r) >= 6 and self.t0 is not None and self.t0 <= ts <= (self.t1 or time.time()) + 0.06]
 
     def stop(self):
         if not self.proc:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        rows = self.in_window()
         self.proc.terminate()
         try:
             self.proc.wait(timeout=5)
         except Exception:
             self.proc.kill()
-        sm = [float(r[0]) for r in self.rows if len(r) >= 6 and r[0].replace(".", "").isdigit()]
-        mx = [float(r[1]) for r in self.rows if len(r) >= 6 and r[1].replace(".", "").isdigit()]
+        sm = [float(r[0]) for r in rows if r[0].replace(".", "").isdigit()]
+        mx = [float(r[1]) for r in rows if r[1].replace(".", "").isdigit()]
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
-        reasons = sorted({names[i] for r in self.rows if len(r) >= 6 for i in range(4) if r[2 + i].lower().startswith("active")})
+        reasons = sorted({names[i] for r in rows for i in range(4) if r[2 + i].lower().startswith("active")})
         return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None, "reasons": reasons,
-                "samples": len(sm)}
+                "samples": len(sm), "window": self.window}
 
 
 def oracle_sample(cfg, model, pix, vis_mode):
@@ -279,6 +296,8 @@ def main():
         frame = r.make_frame(x, wo, d, s, t, flags=flags)
         rgb = torch.empty((cfg.N, 3), device=dev)
         stream = torch.cuda.current_stream().cuda_stream
+        if clocks:
+            clocks.start()
         for _ in range(warmup):
             r.render_frame(frame, rgb, stream)
         torch.cuda.synchronize()
@@ -287,7 +306,7 @@ def main():
         r.stats(reset=True)
         l0 = r.launch_count()
         if clocks:
-            clocks.start()
+            clocks.begin()
         ev = [torch.cuda.Event(enable_timing=True) for _ in range(steps + 1)]
         torch.cuda.synchronize()
         ev[0].record()
@@ -297,13 +316,25 @@ def main():
         torch.cuda.synchronize()
         if world > 1:
             dist.barrier()
-        clk = clocks.stop() if clocks else None
         launches = r.launch_count() - l0
+        traced, evaluated = r.stats()
+        clk = None
+        if clocks:
+            clocks.end()
+            if len(clocks.in_window()) < 8:
+                # a short timed region (K x ~20 ms) sees only a few 50 ms samples: keep sampling over an UNTIMED continuation of the
+                # same launches, so the reported clocks and throttle reasons are those of this kernel under sustained load
+                t_end = time.time() + 1.0
+                while time.time() < t_end:
+                    for _ in range(4):
+                        r.render_frame(frame, rgb, stream)
+                    torch.cuda.synchronize()
+                clocks.end("timed region + 1 s untimed continuation of the same launches")
+            clk = clocks.stop()
         total_ms = ev[0].elapsed_time(ev[-1])
         per = [ev[k].elapsed_time(ev[k + 1]) for k in range(steps)]
         total_ms = hd.max_over_ranks(total_ms, dev)
         assert torch.isfinite(rgb).all()
-        traced, evaluated = r.stats()
         out = dict(total_ms=total_ms, per=per, launches=launches, clk=clk, path=r.last_path(), mean_rgb=float(rgb.mean().item()),
                    traced=traced // max(steps, 1), evaluated=(evaluated // max(steps, 1)) if traced else None)
         # end to end through the public host-buffer entry point: pinned host inputs, H2D + D2H inside the timed region
