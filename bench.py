@@ -225,7 +225,10 @@ def run_c4_sweep(args):
             "frac": alg / (hb["ms"] * 1e-3) / 1e9 / peaks["hbm"], "traffic": traffic, "kernel": "k_trace_wg", "kernel_ms": hb["ms"],
             "point": {"log2_T": hb["log2_T"], "N": hb["N"]}, "peak_source": f"MEASURED_PEAKS.json hbm_gbs ({peaks['which']})",
             "note": "a 4-byte gather moves a 32-byte sector, so sector traffic is up to 8x the algorithmic bytes; ncu: 4.03 KB of DRAM "
-                    "traffic per point = 62 % of the measured HBM peak (profiles/r01c_README.md)"}
+                    "traffic per point = 5.06 TB/s = 61.8 % of ncu's DRAM peak, 77 % of the measured copy bandwidth (profiles/r01c_README.md)"}
+    if traffic:
+        roof["traffic_GBps"] = traffic / (hb["ms"] * 1e-3) / 1e9
+        roof["traffic_frac_of_peak"] = roof["traffic_GBps"] / peaks["hbm"]
     print(json.dumps({"metric": "encode+IRT points/s (BASELINE.json configs[4] sweep)", "value": best["points_per_s"], "unit": "points/s", "n_gpus": 1,
                       "steps": args.steps, "warmup": 3, "ms_per_step": best["ms"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
                       "dtype": "f16", "data": "synthetic", "config": {"workload": "C4 sweep: uniform random points x 1 direction, fp16 L=16 F=2",
