@@ -55,6 +55,8 @@ class Config:
     rough_min: float = 0.09
     fresnel_f0: float = 0.04
     depth_bias: float = -1.5    # keeps x' inside the cube
+    vis_bias: float = 0.0       # I's visibility bias b_v: centres z_v so hard visibility is neither all 0 nor all 1
+                                # (presets: tests/golden/vis_bias.txt, written by tests/golden/make_vis_bias.py from the oracle)
     tol: float = 1e-4
 
     @property
@@ -77,19 +79,19 @@ class Config:
 def make_config(name: str, **over) -> Config:
     """Named presets C0..C4 (BASELINE.json configs[0..4]); C3a = C1 in fp16; `over` overrides fields."""
     c0 = dict(seed=0, N=4096, S_d=8, S_i=0, S_2=8, L=8, F=2, log2_T=14, base_res=16, max_res=256,
-              table_scale=1.0, table_dtype="f32", mlp_dtype="f32", env_hw=(16, 32), points="sphere")
+              table_scale=1.0, table_dtype="f32", mlp_dtype="f32", env_hw=(16, 32), points="sphere", vis_bias=0.0986328125)
     c1 = dict(seed=1, N=640_000, S_d=128, S_i=0, S_2=8, L=16, F=2, log2_T=19, base_res=16, max_res=2048,
-              table_scale=0.1, table_dtype="f32", mlp_dtype="f32", env_hw=(32, 64), points="scene", width=800)
+              table_scale=0.1, table_dtype="f32", mlp_dtype="f32", env_hw=(32, 64), points="scene", width=800, vis_bias=0.001953125)
     presets = {
         "C0": c0,
         "C1": c1,
-        "C2": {**c1, "seed": 2, "S_i": 64, "flags": HR_DIRECT | HR_SHADOW | HR_INDIRECT},
+        "C2": {**c1, "seed": 2, "S_i": 64, "flags": HR_DIRECT | HR_SHADOW | HR_INDIRECT, "vis_bias": -0.041015625},
         "C3": {**c1, "seed": 3, "S_i": 64, "flags": HR_DIRECT | HR_SHADOW | HR_INDIRECT,
-               "table_dtype": "f16", "mlp_dtype": "f16", "tol": 3e-3},
-        "C3a": {**c1, "seed": 3, "table_dtype": "f16", "mlp_dtype": "f16", "tol": 3e-3},
+               "table_dtype": "f16", "mlp_dtype": "f16", "tol": 3e-3, "vis_bias": 0.1259765625},
+        "C3a": {**c1, "seed": 3, "table_dtype": "f16", "mlp_dtype": "f16", "tol": 3e-3, "vis_bias": 0.1259765625},
         "C4": dict(seed=4, N=1 << 20, S_d=1, S_i=0, S_2=0, L=16, F=2, log2_T=19, base_res=16, max_res=2048,
                    table_scale=0.1, table_dtype="f16", mlp_dtype="f16", env_hw=(0, 0), points="uniform",
-                   tol=3e-3),
+                   tol=3e-3, vis_bias=-0.0166015625),
     }
     d = dict(presets[name])
     d.update(over)
@@ -148,6 +150,7 @@ def make_mlp(cfg: Config, which: str) -> np.ndarray:
         W = (g.random((o, i)) * 2.0 - 1.0) * a
         b = (g.random(o) * 2.0 - 1.0) * 0.05
         if which == "irt" and li == len(shapes) - 1:
+            b[0] = cfg.vis_bias
             b[1] = cfg.depth_bias
         parts += [W.ravel(), b]
     return _round_dtype(np.concatenate(parts), cfg.mlp_dtype)
