@@ -176,64 +176,102 @@ def run_reference(args, cfg):
     }))
 
 
+def ncu_record(key):
+    """Counters of the dominant kernel copied from the ncu --set full capture named in the record (profiles/ncu_metrics.json;
+    `capture` says which report).  They are NOT measured by this run: traffic = dram__bytes_read.sum + dram__bytes_write.sum
+    per launch, issue_slots_busy / tensor_pipe_active in % of active cycles, warp_inst = smsp__inst_executed.sum."""
+    pth = os.path.join(ROOT, "profiles", "ncu_metrics.json")
+    if not os.path.exists(pth):
+        return None
+    return json.load(open(pth)).get(key)
+
+
+C4_ALG_BYTES = 16 * 8 * 4 + 24 + 8      # per point: 128 gathers x one fp16 pair + position / direction in + (v, t) out (SURVEY 8(d))
+
+
+def measure_c4(log2_T, Ns, steps, vis_mode, peaks, clock_index=None):
+    """encode + IRT (hashrender_trace, encode fused, 1 direction / point; BASELINE.json configs[4]) at one table size for the
+    point counts `Ns`.  One row per N, each with its own clock record when clock_index is given."""
+    import torch
+    from paper_2409_10327_b200 import DirSet, HashRenderer
+    dev = torch.device("cuda", torch.cuda.current_device())
+    cfg = gen.make_config("C4", log2_T=log2_T, N=max(Ns))
+    model = gen.make_model(cfg)
+    r = HashRenderer.from_gen(cfg, model, vis_mode=vis_mode, max_points=max(Ns))
+    del model
+    g = torch.Generator(device=dev); g.manual_seed(4)
+    x = torch.rand((max(Ns), 3), device=dev, generator=g)
+    d = torch.randn((max(Ns), 1, 3), device=dev, generator=g); d = (d / d.norm(dim=2, keepdim=True)).contiguous()
+    pdf = torch.ones((max(Ns), 1), device=dev)
+    vis = torch.empty((max(Ns), 1), device=dev); t = torch.empty((max(Ns), 1), device=dev)
+    rows = []
+    for N in Ns:
+        ds = DirSet(d[:N], pdf[:N])
+        clocks = ClockSampler(clock_index) if clock_index is not None else None
+        if clocks:
+            clocks.start()
+        for _ in range(3):
+            r.trace(x[:N], None, ds, vis, None, t, N=N)
+        torch.cuda.synchronize()
+        if clocks:
+            clocks.begin()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        for _ in range(steps):
+            r.trace(x[:N], None, ds, vis, None, t, N=N)
+        e1.record(); torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1) / steps
+        clk = None
+        if clocks:
+            clocks.end()
+            if len(clocks.in_window()) < 8:          # short timed region: sample over an untimed continuation of the same launches
+                t_end = time.time() + 1.0
+                while time.time() < t_end:
+                    for _ in range(4):
+                        r.trace(x[:N], None, ds, vis, None, t, N=N)
+                    torch.cuda.synchronize()
+                clocks.end("timed region + 1 s untimed continuation of the same launches")
+            clk = clocks.stop()
+        useful = N * 16 * 8 * 4            # bytes actually used: 8 corners x 16 levels x one fp16 pair
+        alg = N * C4_ALG_BYTES
+        path = r.last_path()
+        rec = ncu_record(f"C4:T{log2_T}:N{N.bit_length() - 1}:{path}") or {}
+        roof = {"bound": "hbm", "achieved": alg / (ms * 1e-3) / 1e9, "peak": peaks["hbm"], "unit": "GB/s",
+                "frac": alg / (ms * 1e-3) / 1e9 / peaks["hbm"], "traffic": rec.get("traffic"), "kernel": "k_trace_wg", "kernel_ms": ms,
+                "algorithmic_bytes_per_point": C4_ALG_BYTES, "peak_source": f"MEASURED_PEAKS.json hbm_gbs ({peaks['which']})",
+                "capture": rec.get("capture"),
+                "note": "a 4-byte gather moves a 32-byte sector, so sector traffic is up to 8x the algorithmic bytes; tables <= 32 MiB "
+                        "(T <= 2^19) are L2-resident and the bound there is the L1/L2 gather rate, not HBM"}
+        if rec.get("traffic"):
+            roof["traffic_GBps"] = rec["traffic"] / (ms * 1e-3) / 1e9
+            roof["traffic_frac_of_peak"] = roof["traffic_GBps"] / peaks["hbm"]
+        rows.append({"log2_T": log2_T, "table_MiB": 16 * (1 << log2_T) * 4 / 2 ** 20, "N": N, "ms": ms, "points_per_s": N / (ms * 1e-3),
+                     "useful_gather_GBps": useful / (ms * 1e-3) / 1e9, "sector_GBps_upper": useful * 8 / (ms * 1e-3) / 1e9,
+                     "path": path, "roofline": roof, "clocks": clk})
+    r.destroy(); del x, d, pdf, vis, t
+    torch.cuda.empty_cache()
+    return rows
+
+
 def run_c4_sweep(args):
     """BASELINE.json configs[4]: encode + IRT throughput (hashrender_trace, encode fused, 1 direction / point) over
     N = 2^20..2^26 uniform random points x T = 2^16, 2^19, 2^22, 2^24 (fp16, F=2, L=16): where the gather leaves L2."""
     import torch
-    from paper_2409_10327_b200 import DirSet, HashRenderer
-    dev = torch.device("cuda", 0)
+    torch.cuda.set_device(0)
     peaks = load_peaks()
     rows = []
     Ns = [1 << 20, 1 << 22, 1 << 24] + ([1 << 26] if args.full_sweep else [])
     if args.c4_n:
         Ns = [args.c4_n]
     for log2_T in ((args.c4_log2t,) if args.c4_log2t else (16, 19, 22, 24)):
-        cfg = gen.make_config("C4", log2_T=log2_T, N=max(Ns))
-        model = gen.make_model(cfg)
-        r = HashRenderer.from_gen(cfg, model, vis_mode=args.vis_mode, max_points=max(Ns))
-        del model
-        g = torch.Generator(device=dev); g.manual_seed(4)
-        x = torch.rand((max(Ns), 3), device=dev, generator=g)
-        d = torch.randn((max(Ns), 1, 3), device=dev, generator=g); d = (d / d.norm(dim=2, keepdim=True)).contiguous()
-        pdf = torch.ones((max(Ns), 1), device=dev)
-        vis = torch.empty((max(Ns), 1), device=dev); t = torch.empty((max(Ns), 1), device=dev)
-        for N in Ns:
-            ds = DirSet(d[:N], pdf[:N])
-            for _ in range(3):
-                r.trace(x[:N], None, ds, vis, None, t, N=N)
-            torch.cuda.synchronize()
-            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-            e0.record()
-            for _ in range(args.steps):
-                r.trace(x[:N], None, ds, vis, None, t, N=N)
-            e1.record(); torch.cuda.synchronize()
-            ms = e0.elapsed_time(e1) / args.steps
-            useful = N * 16 * 8 * 4            # bytes actually used: 8 corners x 16 levels x one fp16 pair
-            rows.append({"log2_T": log2_T, "table_MiB": 16 * (1 << log2_T) * 4 / 2 ** 20, "N": N, "ms": ms, "points_per_s": N / (ms * 1e-3),
-                         "useful_gather_GBps": useful / (ms * 1e-3) / 1e9, "sector_GBps_upper": useful * 8 / (ms * 1e-3) / 1e9,
-                         "path": r.last_path()})
-        r.destroy(); del x, d, pdf, vis, t
-        torch.cuda.empty_cache()
+        rows += measure_c4(log2_T, Ns, args.steps, args.vis_mode, peaks, clock_index=0)
     best = max(rows, key=lambda q: q["points_per_s"])
-    # roofline of the HBM end of the sweep (largest table, most points): algorithmic bytes per point = 128 gathers x 4 B
-    # + 24 B of position / direction in + 8 B of (v, t) out (SURVEY 8(d)); every 4-byte gather moves a 32-byte sector
-    hb = max(rows, key=lambda q: (q["log2_T"], q["N"]))
-    alg = hb["N"] * (16 * 8 * 4 + 24 + 8)
-    tj = os.path.join(ROOT, "profiles", "traffic.json")
-    traffic = json.load(open(tj)).get(f"C4:T{hb['log2_T']}:N{hb['N'].bit_length() - 1}:{hb['path']}") if os.path.exists(tj) else None
-    roof = {"bound": "hbm", "achieved": alg / (hb["ms"] * 1e-3) / 1e9, "peak": peaks["hbm"], "unit": "GB/s",
-            "frac": alg / (hb["ms"] * 1e-3) / 1e9 / peaks["hbm"], "traffic": traffic, "kernel": "k_trace_wg", "kernel_ms": hb["ms"],
-            "point": {"log2_T": hb["log2_T"], "N": hb["N"]}, "peak_source": f"MEASURED_PEAKS.json hbm_gbs ({peaks['which']})",
-            "note": "a 4-byte gather moves a 32-byte sector, so sector traffic is up to 8x the algorithmic bytes; ncu: 4.03 KB of DRAM "
-                    "traffic per point = 5.06 TB/s = 61.8 % of ncu's DRAM peak, 77 % of the measured copy bandwidth (profiles/r01c_README.md)"}
-    if traffic:
-        roof["traffic_GBps"] = traffic / (hb["ms"] * 1e-3) / 1e9
-        roof["traffic_frac_of_peak"] = roof["traffic_GBps"] / peaks["hbm"]
+    hb = max(rows, key=lambda q: (q["log2_T"], q["N"]))          # the HBM end of the sweep: largest table, most points
     print(json.dumps({"metric": "encode+IRT points/s (BASELINE.json configs[4] sweep)", "value": best["points_per_s"], "unit": "points/s", "n_gpus": 1,
                       "steps": args.steps, "warmup": 3, "ms_per_step": best["ms"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
                       "dtype": "f16", "data": "synthetic", "config": {"workload": "C4 sweep: uniform random points x 1 direction, fp16 L=16 F=2",
                       "points": "generated on device (torch Philox); parity of this call at every table size of the sweep: tests/test_gpu_parity.py::test_c4_sweep_full_size_sampled_points"},
-                      "hbm_peak_GBps": peaks["hbm"], "roofline": roof, "sweep": rows}))
+                      "hbm_peak_GBps": peaks["hbm"], "clocks": hb["clocks"], "gpu_launches": args.steps, "roofline": hb["roofline"], "sweep": rows}))
 
 
 def workload_name(cfg):
@@ -258,7 +296,8 @@ def main():
     ap.add_argument("--ref-pixels", type=int, default=256, help="pixels per step for --impl reference")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-cpu-all-cores", action="store_true", help="skip the all-host-cores oracle leg")
-    ap.add_argument("--also", default="C3", help="second workload measured briefly and reported under `also` ('' = none)")
+    ap.add_argument("--also", default="C1,C3,C4", help="comma-separated workloads measured briefly and reported under `also` ('' = none); "
+                    "C4 = the T = 2^19 and T = 2^24 points of the sweep at 2^24 points")
     ap.add_argument("--compact", action="store_true", help="headline with the default API flags (zero-weight secondary rays skipped) "
                     "instead of HR_DENSE")
     ap.add_argument("--no-extra", action="store_true", help="skip the `also` measurements")
@@ -435,28 +474,31 @@ def main():
     def roofline(cfg, path, kernel_ms, evaluated):
         flops = algorithmic_flops(cfg, evaluated)
         ach = flops / (kernel_ms * 1e-3) / 1e12
-        if path == "tcgen05-f16":
+        if path.startswith("tcgen05"):
+            # the contraction's own dtype is fp16 with fp32 accumulate for BOTH tensor paths: the peak is the measured sustained
+            # fp16 / bf16 rate, undivided.  (The split-precision path spends three MMA passes per product; that is this
+            # implementation's cost, not a smaller roofline.)
             roof = {"bound": "tensor", "achieved": ach, "peak": peaks["tensor_sustained"], "unit": "TFLOP/s",
                     "peak_source": f"MEASURED_PEAKS.json bf16_tflops_sustained ({peaks['which']}; fp16 = bf16 rate; kernel runs back to back for the whole step)"}
-        elif path == "tcgen05-f16x3":
-            roof = {"bound": "tensor", "achieved": ach, "peak": peaks["tensor_sustained"] / 3.0, "unit": "TFLOP/s",
-                    "peak_source": f"MEASURED_PEAKS.json bf16_tflops_sustained ({peaks['which']}) / 3: an fp32-grade product on the fp16 tensor "
-                                   "cores is three MMA passes (hi*Whi + lo*Whi + hi*Wlo), only one of which is algorithmic work"}
         else:
             alu_peak = 148 * 128 * 2 * peaks["sm_max_mhz"] * 1e6 / 1e12
             roof = {"bound": "alu", "achieved": ach, "peak": alu_peak, "unit": "TFLOP/s",
                     "peak_source": "derived: 148 SM x 128 fp32 lanes x 2 flop x sm_max_mhz (DESIGN.md)"}
         roof["frac"] = roof["achieved"] / roof["peak"]
+        if path == "tcgen05-f16x3":
+            roof["frac_over_3pass"] = 3.0 * roof["frac"]       # share of the tensor pipe's time the three passes would need at peak; not `frac`
         roof["kernel"] = "k_render_wg" if path.startswith("tcgen05") else "k_render_ffma"
         roof["kernel_ms"] = kernel_ms
         roof["algorithmic_flops_per_launch"] = flops
         roof["note"] = ("the MLP contractions run on the tensor pipe, but the kernel's binding unit is the SM issue slots: per query the "
                         "fp16 pack / epilogue / shading ALU work exceeds the 64x64 MMA (DESIGN.md 6.1); see profiles/ for issue-slot "
                         "and tensor-pipe utilisation")
-        tpath = os.path.join(ROOT, "profiles", "traffic.json")
-        roof["traffic"] = None
-        if os.path.exists(tpath):
-            roof["traffic"] = json.load(open(tpath)).get(f"{cfg.name}:{path}")
+        rec = ncu_record(f"{cfg.name}:{path}") or {}
+        roof["traffic"] = rec.get("traffic")
+        for k in ("issue_slots_busy", "tensor_pipe_active", "capture"):
+            roof[k] = rec.get(k)
+        if rec.get("warp_inst"):                               # thread instructions per executed query, from the capture's dense frame
+            roof["thread_inst_per_query"] = rec["warp_inst"] * 32 / cfg.queries
         return roof
 
     roof = roofline(cfg, res["path"], kernel_ms, res["evaluated"])
@@ -471,7 +513,7 @@ def main():
                    "executed_queries_per_frame": executed_queries(cfg, res["evaluated"]),
                    "path": res["path"], "l2": "per-frame inputs (2.0 GB of directions/pdfs) exceed the 126 MB L2; the hash table is "
                    "L2-resident by design", "multi_gpu": "independent frames per rank, no collective"},
-        "clocks": res["clk"], "gpu_launches": res["launches"], "roofline": roof,
+        "clocks": res["clk"], "gpu_launches": res["launches"], "mean_rgb": res["mean_rgb"], "roofline": roof,
     }
     if "e2e_ms" in res:
         line["e2e"] = {"value": world * cfg.queries / (res["e2e_ms"] * 1e-3), "unit": UNIT, "ms_per_frame": res["e2e_ms"],
@@ -479,6 +521,9 @@ def main():
     if "e2e_sampled_ms" in res:
         line["e2e_sampled"] = {"value": cfg.queries / (res["e2e_sampled_ms"] * 1e-3), "unit": UNIT, "ms_per_frame": res["e2e_sampled_ms"],
                                "h2d_bytes_per_step": res["e2e_sampled_h2d"], "d2h_bytes_per_step": cfg.N * 12, "finite": res["e2e_sampled_finite"],
+                               "mean_rgb": res["e2e_sampled_mean"],
+                               "parity": "tests/test_gpu_sampler.py::test_sampled_frame_composition_matches_oracle checks this composition against the "
+                                         "composition of the oracles",
                                "what": "same frame shape, but only x and wo travel: B(H(x)) is decoded and the direction sets are generated on the "
                                        "device (hashrender_encode/decode/sample_mis/sample_stratified/render_frame); PAPER.md:122, 344"}
     if "denoise_ms" in res:
@@ -486,25 +531,34 @@ def main():
                            "what": "hashrender_denoise: spatial-only SVGF (7x7 variance estimate + five 5x5 a-trous passes) on the rendered "
                                    "800x800 frame; the paper's Table 3 lists 3.2-3.5 ms for its denoiser on an A100 (context)"}
     if world == 1 and not args.no_extra:
-        # the same frame with the default API flags (zero-weight secondary rays compacted out), and the
-        # other precision; `value` here is frame-equivalent (queries_per_frame / time), executed queries are stated
+        # the same frame with the default API flags (zero-weight secondary rays compacted out), the other
+        # BASELINE configs (C1 direct only, C3 fp16) and two points of the C4 sweep (T = 2^19 L2-resident, T = 2^24 HBM, both at
+        # 2^24 points); `value` here is frame-equivalent (queries_per_frame / time), executed queries are stated
         extra = []
         if cfg.flags & gen.HR_INDIRECT:
             extra.append((cfg, args.compact))
-        if args.also and args.also != args.workload:
-            cfg2 = gen.make_config(args.also)
+        for nm in [w for w in args.also.split(",") if w and w != args.workload and w != "C4"]:
+            cfg2 = gen.make_config(nm)
             extra += [(cfg2, True), (cfg2, False)] if cfg2.flags & gen.HR_INDIRECT else [(cfg2, True)]
         line["also"] = []
         for c2, dense in extra:
             st = max(args.steps // 2, 3)
-            r2, _ = measure(c2, st, 3, 0, None, dense=dense)
+            r2, _ = measure(c2, st, 3, 0, ClockSampler(local), dense=dense)
             ms2 = r2["total_ms"] / st
             rf = roofline(c2, r2["path"], ms2, r2["evaluated"])
             line["also"].append({"workload": workload_name(c2), "secondary_rays": "dense" if dense else "compacted", "ms_per_frame": ms2,
                                  "frame_equivalent_queries_per_s": c2.queries / (ms2 * 1e-3),
                                  "executed_queries_per_frame": executed_queries(c2, r2["evaluated"]),
                                  "executed_queries_per_s": executed_queries(c2, r2["evaluated"]) / (ms2 * 1e-3), "path": r2["path"],
-                                 "achieved_tflops": rf["achieved"], "roofline_frac": rf["frac"], "roofline_peak": rf["peak"]})
+                                 "mean_rgb": r2["mean_rgb"], "achieved_tflops": rf["achieved"], "roofline_frac": rf["frac"],
+                                 "roofline_peak": rf["peak"], "roofline": rf, "clocks": r2["clk"]})
+        if "C4" in args.also.split(","):
+            for log2_T in (19, 24):
+                for row in measure_c4(log2_T, [1 << 24], max(args.steps // 2, 3), args.vis_mode, peaks, clock_index=local):
+                    line["also"].append({"workload": f"C4: encode + IRT, 2^24 uniform random points x 1 direction, fp16 L=16 F=2 T=2^{log2_T} "
+                                                     f"({row['table_MiB']:.0f} MiB table; BASELINE.json configs[4])", "ms": row["ms"],
+                                         "points_per_s": row["points_per_s"], "path": row["path"], "roofline_frac": row["roofline"]["frac"],
+                                         "roofline": row["roofline"], "clocks": row["clocks"]})
     if not args.no_cpu_baseline and world == 1:
         pix = sample_pixels(cfg, args.cpu_pixels)
         dt, q = oracle_sample(cfg, model, pix, args.vis_mode)

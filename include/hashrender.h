@@ -14,12 +14,17 @@
  *    hashrender_last_error(h) returns a NUL-terminated string owned by the handle (valid until the next
  *    failing call on that handle or its destruction).
  *  - Pointers are DEVICE pointers unless the comment says `host`.  All device work is enqueued
- *    asynchronously on the caller's cudaStream_t (passed as void*, NULL = legacy default stream); no call
- *    synchronises except hashrender_create, hashrender_destroy and hashrender_render_frame_host.
+ *    asynchronously on the caller's cudaStream_t (passed as void*, NULL = legacy default stream).  Calls that
+ *    synchronise: hashrender_create, hashrender_destroy, hashrender_render_frame_host (the stream, before it returns),
+ *    hashrender_stats (the device) and the FIRST hashrender_sample_mis after a set_env (the stream, once: it reads the
+ *    env map back to build the light tables on the host).  Nothing else synchronises.
  *  - Outputs are caller-allocated.  The library neither frees nor keeps caller memory after a call
  *    returns; hashrender_create COPIES (and re-lays-out / converts) tables and weights.
- *  - No allocation after create, except hashrender_render_frame_host's staging buffers, copy stream and events
- *    (created / grown on demand, released by destroy).
+ *  - No allocation after create, except scratch that is created / grown on demand inside the handle and released by
+ *    destroy: hashrender_render_frame_host's staging buffers, copy stream and events; hashrender_set_env's copy of the
+ *    map (grown when a larger map arrives); hashrender_sample_mis's light tables; hashrender_denoise's image planes.
+ *  - Alignment: every array 4-byte aligned; `feat` passed to hashrender_trace and `pdf` written by hashrender_sample_mis
+ *    8-byte aligned (read / written as float2).
  *  - Arrays are row-major, innermost index last; float = IEEE binary32.  Directions and w_o are assumed
  *    unit length (not re-normalised).  Positions outside [0,1]^3 are clamped per component (Q6).
  *  - N == 0 is a no-op returning HR_OK.  NULL handle / NULL required pointer / S == 0 where a set is
@@ -112,7 +117,9 @@ int hashrender_decode(hashrender_t* h, const float* feat, uint64_t N, float* brd
 
 /* v, t = I(f, w) for every direction of `ds` (step a6) and x' = clamp(x + t w) (
  * step a7).  feat NULL => the encode is fused (x required).  vis [N,S] (sigma(z_v) or {0,1}); zv nullable
- * [N,S] raw logit; t [N,S]; xsec nullable [N,S,3] (x required). ds->pdf and ds->Lin are not read. */
+ * [N,S] raw logit; t [N,S]; xsec nullable [N,S,3] (x required). ds->pdf and ds->Lin are not read.
+ * Runs the arithmetic hashrender_render_frame uses for its direct / secondary queries on this model (see
+ * hashrender_last_path), so the production path's z_v, t, x' can be checked stage by stage. */
 int hashrender_trace(hashrender_t* h, const float* x, const float* feat, uint64_t N, const hr_dirset* ds,
                      float* vis, float* zv, float* t, float* xsec, void* stream);
 

@@ -98,17 +98,48 @@ def _ptr(a):
     return C.c_void_p(a.data_ptr())
 
 
+_DT = {"f32": ("float32", 4), "u8": ("uint8", 1), "u32": ("uint32", 4), "i32": ("int32", 4)}
+
+
+def _arg(a, what, dt="f32", where="device", align=4):
+    """Marshals one array argument after checking what the C side cannot: element type, placement (the device entry points
+    take device pointers, render_frame_host takes host pointers) and alignment.  A wrong dtype or a host array passed to a
+    device call would otherwise be misread silently.  None -> NULL."""
+    if a is None:
+        return None
+    names = [_DT[d][0] for d in (dt if isinstance(dt, tuple) else (dt,))]
+    if isinstance(a, np.ndarray):
+        kind, on_dev = a.dtype.name, False
+    else:
+        kind, on_dev = str(a.dtype).replace("torch.", ""), bool(a.is_cuda)
+    if kind not in names:
+        raise TypeError(f"{what}: expected {' / '.join(names)}, got {kind}")
+    if where == "device" and not on_dev:
+        raise TypeError(f"{what}: expected a CUDA tensor (device pointer), got a host array")
+    if where == "host" and on_dev:
+        raise TypeError(f"{what}: expected a host array, got a CUDA tensor")
+    p = _ptr(a)
+    if p.value is not None and p.value % align:
+        raise ValueError(f"{what}: pointer must be {align}-byte aligned")
+    return p
+
+
 @dataclass
 class DirSet:
     """dir [N,S,3] (or [S,3] = one shared set), pdf [N,S] (or [S]), optional Lin like dir."""
     dir: object
     pdf: object
     Lin: object = None
+    S: int | None = None                 # directions used per point when the rows are padded (default: dir.shape[-2])
+    point_stride: int | None = None      # floats of `dir` between points (default 3 * dir.shape[-2]; 0 = one shared set)
 
-    def c(self) -> hr_dirset:
+    def c(self, where="device") -> hr_dirset:
+        for nm in ("dir", "pdf", "Lin"):
+            _arg(getattr(self, nm), f"DirSet.{nm}", "f32", where)
         shared = self.dir.ndim == 2
-        S = self.dir.shape[-2]
-        return hr_dirset(dir=_ptr(self.dir), pdf=_ptr(self.pdf), Lin=_ptr(self.Lin), S=S, point_stride=0 if shared else 3 * S)
+        S = self.dir.shape[-2] if self.S is None else self.S
+        stride = (0 if shared else 3 * self.dir.shape[-2]) if self.point_stride is None else self.point_stride
+        return hr_dirset(dir=_ptr(self.dir), pdf=_ptr(self.pdf), Lin=_ptr(self.Lin), S=S, point_stride=stride)
 
 
 class HashRenderer:
@@ -166,53 +197,65 @@ class HashRenderer:
 
     # ---- C ABI mirrors (device pointers; stream = int cudaStream_t handle or None) -----------------------
     def set_env(self, env, stream=None):
-        self._check(self._lib.hashrender_set_env(self._h, _ptr(env), env.shape[0], env.shape[1], stream))
+        self._check(self._lib.hashrender_set_env(self._h, _arg(env, "env"), env.shape[0], env.shape[1], stream))
 
     def encode(self, x, feat, idx=None, w=None, stream=None, N=None):
-        self._check(self._lib.hashrender_encode(self._h, _ptr(x), x.shape[0] if N is None else N, _ptr(feat), _ptr(idx), _ptr(w), stream))
+        n = N if N is not None else x.shape[0]
+        self._check(self._lib.hashrender_encode(self._h, _arg(x, "x"), n, _arg(feat, "feat"), _arg(idx, "idx", ("u32", "i32")), _arg(w, "w"), stream))
 
     def decode(self, feat, brdf, stream=None):
-        self._check(self._lib.hashrender_decode(self._h, _ptr(feat), feat.shape[0], _ptr(brdf), stream))
+        self._check(self._lib.hashrender_decode(self._h, _arg(feat, "feat"), feat.shape[0], _arg(brdf, "brdf"), stream))
 
     def trace(self, x, feat, ds: DirSet, vis, zv, t, xsec=None, stream=None, N=None):
         n = N if N is not None else (x.shape[0] if x is not None else feat.shape[0])
         d = ds.c()
-        self._check(self._lib.hashrender_trace(self._h, _ptr(x), _ptr(feat), n, C.byref(d), _ptr(vis), _ptr(zv), _ptr(t), _ptr(xsec), stream))
+        self._check(self._lib.hashrender_trace(self._h, _arg(x, "x"), _arg(feat, "feat", align=8), n, C.byref(d), _arg(vis, "vis"), _arg(zv, "zv"),
+                                               _arg(t, "t"), _arg(xsec, "xsec"), stream))
 
     def shade(self, brdf, wo, ds: DirSet, vis, Lind, terms, rgb, stream=None):
         d = ds.c()
-        self._check(self._lib.hashrender_shade(self._h, _ptr(brdf), _ptr(wo), brdf.shape[0], C.byref(d), _ptr(vis), _ptr(Lind), terms, _ptr(rgb), stream))
+        self._check(self._lib.hashrender_shade(self._h, _arg(brdf, "brdf"), _arg(wo, "wo"), brdf.shape[0], C.byref(d), _arg(vis, "vis"),
+                                               _arg(Lind, "Lind"), terms, _arg(rgb, "rgb"), stream))
 
     def make_frame(self, x, wo, direct: DirSet | None, secondary: DirSet | None = None, tertiary: DirSet | None = None,
                    flags=HR_DIRECT | HR_SHADOW, brdf=None, mask=None, N=None) -> hr_frame:
         z = hr_dirset()
-        fr = hr_frame(N=x.shape[0] if N is None else N, x=_ptr(x), brdf=_ptr(brdf), wo=_ptr(wo), mask=_ptr(mask),
-                      direct=direct.c() if direct else z, secondary=secondary.c() if secondary else z,
-                      tertiary=tertiary.c() if tertiary else z, flags=flags)
+        where = "host" if isinstance(x, np.ndarray) or not getattr(x, "is_cuda", False) else "device"    # all arrays of a frame live together
+        fr = hr_frame(N=x.shape[0] if N is None else N, x=_arg(x, "x", "f32", where), brdf=_arg(brdf, "brdf", "f32", where),
+                      wo=_arg(wo, "wo", "f32", where), mask=_arg(mask, "mask", "u8", where, 1),
+                      direct=direct.c(where) if direct else z, secondary=secondary.c(where) if secondary else z,
+                      tertiary=tertiary.c(where) if tertiary else z, flags=flags)
+        fr._where = where
         fr._keep = (x, wo, direct, secondary, tertiary, brdf, mask)
         return fr
 
     def render_frame(self, frame: hr_frame, rgb, stream=None):
-        self._check(self._lib.hashrender_render_frame(self._h, C.byref(frame), _ptr(rgb), stream))
+        if getattr(frame, "_where", "device") != "device":
+            raise TypeError("render_frame takes a frame of device arrays (use render_frame_host for host arrays)")
+        self._check(self._lib.hashrender_render_frame(self._h, C.byref(frame), _arg(rgb, "rgb"), stream))
 
     def render_frame_host(self, frame: hr_frame, rgb, stream=None):
         up, down = C.c_uint64(), C.c_uint64()
-        self._check(self._lib.hashrender_render_frame_host(self._h, C.byref(frame), _ptr(rgb), stream, C.byref(up), C.byref(down)))
+        if getattr(frame, "_where", "host") != "host":
+            raise TypeError("render_frame_host takes a frame of host arrays")
+        self._check(self._lib.hashrender_render_frame_host(self._h, C.byref(frame), _arg(rgb, "rgb", "f32", "host"), stream, C.byref(up), C.byref(down)))
         return up.value, down.value
 
     def sample_mis(self, brdf, wo, spp, seed, dir, pdf, stream=None):
-        self._check(self._lib.hashrender_sample_mis(self._h, _ptr(brdf), _ptr(wo), brdf.shape[0], spp, seed, _ptr(dir), _ptr(pdf), stream))
+        # k_sample_mis stores the (light, GGX) pdf pair of a sample as one float2
+        self._check(self._lib.hashrender_sample_mis(self._h, _arg(brdf, "brdf"), _arg(wo, "wo"), brdf.shape[0], spp, seed, _arg(dir, "dir"),
+                                                    _arg(pdf, "pdf", align=8), stream))
 
     def sample_stratified(self, normal, rows, Sa, Sb, seed, dir, pdf, stream=None):
-        self._check(self._lib.hashrender_sample_stratified(self._h, _ptr(normal), rows, Sa, Sb, seed, _ptr(dir), _ptr(pdf), stream))
+        self._check(self._lib.hashrender_sample_stratified(self._h, _arg(normal, "normal"), rows, Sa, Sb, seed, _arg(dir, "dir"), _arg(pdf, "pdf"), stream))
 
     def denoise(self, rgb, normal, pos, cam, out, albedo=None, mask=None, iterations=5, sigma_z=1.0, sigma_n=128.0, sigma_l=4.0,
                 stream=None):
         """rgb / normal / pos / out: [H, W, 3] device tensors; cam: 3 floats."""
-        d = hr_denoise(H=rgb.shape[0], W=rgb.shape[1], rgb=_ptr(rgb), albedo=_ptr(albedo), normal=_ptr(normal), pos=_ptr(pos),
-                       cam=(C.c_float * 3)(*[float(v) for v in cam]), mask=_ptr(mask), iterations=iterations, sigma_z=sigma_z,
-                       sigma_n=sigma_n, sigma_l=sigma_l)
-        self._check(self._lib.hashrender_denoise(self._h, C.byref(d), _ptr(out), stream))
+        d = hr_denoise(H=rgb.shape[0], W=rgb.shape[1], rgb=_arg(rgb, "rgb"), albedo=_arg(albedo, "albedo"), normal=_arg(normal, "normal"),
+                       pos=_arg(pos, "pos"), cam=(C.c_float * 3)(*[float(v) for v in cam]), mask=_arg(mask, "mask", "u8", align=1),
+                       iterations=iterations, sigma_z=sigma_z, sigma_n=sigma_n, sigma_l=sigma_l)
+        self._check(self._lib.hashrender_denoise(self._h, C.byref(d), _arg(out, "out"), stream))
 
     def stats(self, reset=False):
         """(secondary rays traced, secondary rays whose L'_o was evaluated) since the last reset."""

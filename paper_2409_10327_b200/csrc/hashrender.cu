@@ -47,7 +47,6 @@ struct hashrender {
   bool light_valid = false;
   cudaStream_t copy_stream = nullptr;   // render_frame_host: H2D copies of chunk c+1 overlap the render of chunk c
   cudaEvent_t ev[9] = {nullptr};
-  int force_path = 0;            // 0 auto, 1 ffma  (env HASHRENDER_PATH=ffma, for A/B tests)
 };
 
 namespace {
@@ -127,7 +126,7 @@ int check_dirset(hashrender* h, const hr_dirset* d, const char* name, bool need_
 
 // 0 = fp32 FFMA kernels, 1 = tcgen05 with fp16 activations, 2 = tcgen05 in hi/lo split precision (fp32 models)
 int render_path(const hashrender* h) {
-  if (h->force_path == 1 || !h->d_wts_tc) return 0;
+  if (!h->d_wts_tc) return 0;
   if (h->cfg.mlp_dtype == HR_F16) return 1;
   return h->split_ok ? 2 : 0;
 }
@@ -176,8 +175,6 @@ int hashrender_create(const hr_config* cfg, const float* tables, const float* br
   int dev = 0;
   HR_CUDA(h, cudaGetDevice(&dev));
   HR_CUDA(h, cudaDeviceGetAttribute(&h->num_sms, cudaDevAttrMultiProcessorCount, dev));
-  const char* fp = getenv("HASHRENDER_PATH");
-  if (fp) h->force_path = !strcmp(fp, "ffma") ? 1 : 0;
 
   // grid parameters
   GridP& g = h->grid;
@@ -243,6 +240,8 @@ int hashrender_create(const hr_config* cfg, const float* tables, const float* br
   HR_CUDA(h, cudaFuncSetAttribute(k_trace_ffma<false, NT_FFMA>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_half));
   HR_CUDA(h, cudaFuncSetAttribute(k_trace_ffma<true, NT_FFMA>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_half));
   HR_CUDA(h, cudaFuncSetAttribute(k_decode_ffma<NT_FFMA>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_half));
+  HR_CUDA(h, wg::init_device_p0());      // per device (a second handle on another device opts in there too)
+  HR_CUDA(h, wg::init_device_p1());
   return HR_OK;
 }
 
@@ -310,10 +309,16 @@ int hashrender_trace(hashrender_t* h, const float* x, const float* feat, uint64_
   if (xsec && !x) return fail(h, HR_ERR_INVALID_ARG, "trace: xsec needs x");
   if (N > h->cfg.max_points) return fail(h, HR_ERR_INVALID_ARG, "trace: N exceeds max_points");
   const DirsetP d = to_dev(*ds);
-  if (render_path(h) == 1 && !feat) {
-    h->last_path = "tcgen05-f16";
-    HR_CUDA(h, wg::launch_trace_p0(h->grid.f16, h->grid, h->shade, h->h_wts_tc.data(), h->d_wts_tc, x, N, d, vis, zv, t, xsec, h->num_sms,
-                                   (cudaStream_t)stream));
+  // the tensor-core kernel runs the arithmetic of render_frame's direct / secondary queries for this model (fp16 activations,
+  // or hi/lo split precision for fp32 models), so v, z_v, t, x' of the production path are checked stage by stage
+  if (const int path = render_path(h)) {
+    h->last_path = path == 1 ? "tcgen05-f16" : "tcgen05-f16x3";
+    if (path == 1)
+      HR_CUDA(h, wg::launch_trace_p0(h->grid.f16, h->grid, h->shade, h->h_wts_tc.data(), h->d_wts_tc, x, feat, N, d, vis, zv, t, xsec,
+                                     h->num_sms, (cudaStream_t)stream));
+    else
+      HR_CUDA(h, wg::launch_trace_p1(h->grid.f16, h->grid, h->shade, h->h_wts_tc.data(), h->d_wts_tc, x, feat, N, d, vis, zv, t, xsec,
+                                     h->num_sms, (cudaStream_t)stream));
     h->launches++;
     return HR_OK;
   }

@@ -600,12 +600,19 @@ __global__ void __launch_bounds__(kRows* G, 1)
       float3 L;
       Taps32<F16TAB> taps;                                            // PREC 1: fp32 taps; PREC 0: fp16x2 taps (only one survives)
       LevelTaps<F16TAB> htaps;
+      // levels l >= g.L do not exist (their table slice would lie past the allocation): no gather, zero features
       auto pre_gather = [&](int l) {
+        if (l >= (int)g.L) return;
         if constexpr (PREC == 1) gather32<F16TAB>(g, l, nx, ny, nz, taps); else gather_level<F16TAB>(g, l, nx, ny, nz, htaps);
       };
       auto pre_finish = [&](int l) {
+        if (l >= (int)g.L) {
+          tmem_st1(tF + l, 0u);
+          if constexpr (PREC == 1) tmem_st1(tF + 16 + l, 0u);
+          return;
+        }
         if constexpr (PREC == 1) finish32<F16TAB>(tF, l, taps);
-        else asm volatile("tcgen05.st.sync.aligned.32x32b.x1.b32 [%0], {%1};" ::"r"(tF + l), "r"(lerp_level(htaps)) : "memory");
+        else tmem_st1(tF + l, lerp_level(htaps));
       };
       const bool pre_k = pre && k < 8u;                               // levels 2k, 2k+1 of the next group ride in this query
       if (kPre && pre_k) pre_gather(2 * (int)k);
@@ -781,18 +788,43 @@ __global__ void __launch_bounds__(kRows* G, 1)
 // x 32 outstanding loads per SM keep the gather pipeline full when the table spills from L2 to HBM.  t is an output, so the
 // fp32 epilogue is used (features hi/lo split for P, fp16 h1).
 constexpr int kTraceG = 4;
-constexpr size_t kTraceSmem = 1024 + kHiTileBytes + kOnesBytes + (size_t)kTraceG * kH * kRows * 4 + 8 * kMaxG + 16;
+template <int PREC> constexpr size_t trace_smem() {
+  return 1024 + (size_t)kHiTileBytes * (PREC ? 2 : 1) + kOnesBytes + (size_t)kTraceG * kH * kRows * 4 + 8 * kMaxG + 16;
+}
 
-template <bool F16TAB>
+// caller-supplied features f[2 L] (fp32) -> A columns 0..15 (hi) | 16..31 (lo), as encode_split_to leaves them
+template <int LIF>
+__device__ __forceinline__ void feat_split_to(uint32_t tA, const GridP& g, const float* __restrict__ f) {
+#pragma unroll 1
+  for (int l0 = 0; l0 < kMaxL; l0 += LIF) {
+    uint32_t hi[LIF], lo[LIF];
+#pragma unroll
+    for (int q = 0; q < LIF; ++q) {
+      hi[q] = 0u; lo[q] = 0u;
+      if (l0 + q < (int)g.L) {
+        const float2 v = __ldg(reinterpret_cast<const float2*>(f) + l0 + q);
+        split_pair(v.x, v.y, hi[q], lo[q]);
+      }
+    }
+    tmem_stN(tA + l0, hi);
+    tmem_stN(tA + 16 + l0, lo);
+  }
+}
+
+// PREC = 0: fp16 models (fp16 h1, one MMA pass).  PREC = 1: fp32 models in hi/lo split precision -- exactly the arithmetic
+// k_render_wg<PREC = 1> runs for its direct / secondary queries (h1_dir<true>, three passes, epi_precise), so hashrender_trace
+// on an fp32 model checks z_v, t, x' of the production path stage by stage.  feat != nullptr: the caller's features replace H(x).
+template <bool F16TAB, int PREC>
 __global__ void __launch_bounds__(kRows* kTraceG, 1)
     k_trace_wg(const __grid_constant__ GridP g, ShadeP sp, const __grid_constant__ TcConst cw, const uint8_t* __restrict__ wtiles,
-               const float* __restrict__ x, unsigned long long N, DirsetP ds, float* __restrict__ vis, float* __restrict__ zvo,
-               float* __restrict__ to, float* __restrict__ xsec) {
+               const float* __restrict__ x, const float* __restrict__ feat, unsigned long long N, DirsetP ds, float* __restrict__ vis,
+               float* __restrict__ zvo, float* __restrict__ to, float* __restrict__ xsec) {
   constexpr int G = kTraceG;
-  using CL = Cols<0, G>;
+  using CL = Cols<PREC, G>;
+  constexpr int kTiles = kHiTileBytes * (PREC ? 2 : 1);
   extern __shared__ uint8_t smem_raw[];
   uint8_t* s_tiles = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
-  uint8_t* s_ones = s_tiles + kHiTileBytes;
+  uint8_t* s_ones = s_tiles + kTiles;
   float4* s_P = reinterpret_cast<float4*>(s_ones + kOnesBytes);
   uint64_t* s_mbar = reinterpret_cast<uint64_t*>(s_P + (size_t)G * (kH / 4) * kRows);
   uint32_t* s_tmem = reinterpret_cast<uint32_t*>(s_mbar + kMaxG);
@@ -809,7 +841,7 @@ __global__ void __launch_bounds__(kRows* kTraceG, 1)
   {
     const uint4* src = reinterpret_cast<const uint4*>(wtiles);
     uint4* dst = reinterpret_cast<uint4*>(s_tiles);
-    for (int i = threadIdx.x; i < kHiTileBytes / 16; i += kRows * G) dst[i] = __ldg(src + i);
+    for (int i = threadIdx.x; i < kTiles / 16; i += kRows * G) dst[i] = __ldg(src + i);
   }
   fill_ones(s_ones, kRows * G);
   asm volatile("fence.proxy.async.shared::cta;" ::: "memory");
@@ -823,25 +855,28 @@ __global__ void __launch_bounds__(kRows* kTraceG, 1)
   c.mbar = __reduce_min_sync(0xFFFFFFFFu, smem_u32(s_mbar + wgi));
   c.phase = 0;
   c.tile0 = smem_u32(s_tiles);
-  c.lo_off = 0;
+  c.lo_off = kHiTileBytes;
   c.ones = smem_u32(s_ones);
   const uint32_t tA = c.tmem + c.lane, tD = c.tmem + c.lane + CL::d;
   float4* Ps4 = s_P + (size_t)wgi * (kH / 4) * kRows + c.t;
   const unsigned long long ntiles = (N + kRows - 1) / kRows;
+  const uint32_t D = g.L * 2u;
   for (unsigned long long tile = (unsigned long long)blockIdx.x * G + wgi; tile < ntiles; tile += (unsigned long long)gridDim.x * G) {
     const unsigned long long i_raw = tile * kRows + c.t;
     const bool valid = i_raw < N;
     const unsigned long long i = valid ? i_raw : N - 1;
-    const float px = __ldg(x + 3 * i), py = __ldg(x + 3 * i + 1), pz = __ldg(x + 3 * i + 2);
-    encode_split_to<F16TAB, 4>(tA, g, px, py, pz);
-    issue_layer<0, G>(c, 0, 0, 2, true, 0, 2);                        // P = W1f f + b1, split-precision f
+    float px = 0.f, py = 0.f, pz = 0.f;
+    if (x) { px = __ldg(x + 3 * i); py = __ldg(x + 3 * i + 1); pz = __ldg(x + 3 * i + 2); }
+    if (feat) feat_split_to<4>(tA, g, feat + i * D);
+    else encode_split_to<F16TAB, 4>(tA, g, px, py, pz);
+    issue_layer<PREC, G>(c, 0, 0, 2, true, 0, 2);                     // P = W1f f + b1, split-precision f
     wait_layer(c);
     store_D_f4(tD, Ps4);
     for (uint32_t sidx = 0; sidx < ds.S; ++sidx) {
       const float* dp = dir_of(ds, i, sidx);
       const float wx = __ldg(dp), wy = __ldg(dp + 1), wz = __ldg(dp + 2);
-      h1_dir<false>(tA, cw, [&](int q) { return Ps4[q * kRows]; }, wx, wy, wz);
-      issue_layer<0, G>(c, 0, 2, 4, false, 0, 3);
+      h1_dir<PREC == 1>(tA, cw, [&](int q) { return Ps4[q * kRows]; }, wx, wy, wz);
+      issue_layer<PREC, G>(c, 0, 2, 4, PREC == 1, 0, 3);
       wait_layer(c);
       float zv, zt, v, t;
       epi_precise<false>(tD, cw, zv, zt);
@@ -862,21 +897,19 @@ __global__ void __launch_bounds__(kRows* kTraceG, 1)
   }
 }
 
-template <bool F16TAB>
+template <bool F16TAB, int PREC>
 inline cudaError_t launch_trace_one(const GridP& g, const ShadeP& sp, const TcConst& cw, const uint8_t* d_tiles, const float* x,
-                                    unsigned long long N, const DirsetP& ds, float* vis, float* zv, float* t, float* xsec, int num_sms,
-                                    cudaStream_t st) {
-  static bool attr_done = false;
-  auto kern = k_trace_wg<F16TAB>;
-  if (!attr_done) {
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kTraceSmem);
-    if (e != cudaSuccess) return e;
-    attr_done = true;
-  }
+                                    const float* feat, unsigned long long N, const DirsetP& ds, float* vis, float* zv, float* t,
+                                    float* xsec, int num_sms, cudaStream_t st) {
   const unsigned long long need = ((N + kRows - 1) / kRows + kTraceG - 1) / kTraceG;
   const int grid = (int)(need < (unsigned long long)num_sms ? need : (unsigned long long)num_sms);
-  kern<<<grid, kRows * kTraceG, kTraceSmem, st>>>(g, sp, cw, d_tiles, x, N, ds, vis, zv, t, xsec);
+  k_trace_wg<F16TAB, PREC><<<grid, kRows * kTraceG, trace_smem<PREC>(), st>>>(g, sp, cw, d_tiles, x, feat, N, ds, vis, zv, t, xsec);
   return cudaGetLastError();
+}
+// the opt-in to > 48 KB of dynamic shared memory is per device: hashrender_create calls this for the handle's device
+template <bool F16TAB, int PREC>
+inline cudaError_t trace_attr() {
+  return cudaFuncSetAttribute(k_trace_wg<F16TAB, PREC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)trace_smem<PREC>());
 }
 
 // ---------------------------------------------------------------------------------------------------- host side
@@ -907,13 +940,7 @@ template <bool F16TAB, int PREC, bool TSHARED, int G>
 inline cudaError_t launch_one(const GridP& g, const EnvP& env, const ShadeP& sp, const TcConst& cw, const uint8_t* d_tiles,
                               const float* wts32, const FrameP& fr, float* rgb, Item* ring, unsigned long long* counters, int num_sms, cudaStream_t st) {
   using SP = SmemPlan<PREC, TSHARED, G>;
-  static bool attr_done = false;
   auto kern = k_render_wg<F16TAB, PREC, TSHARED, G>;
-  if (!attr_done) {
-    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SP::bytes);
-    if (e != cudaSuccess) return e;
-    attr_done = true;
-  }
   cudaError_t e = cudaMemsetAsync(counters, 0, 8, st);                // the tile counter; the statistics keep accumulating
   if (e != cudaSuccess) return e;
   const unsigned long long tiles = (fr.N + kRows - 1) / kRows;
@@ -921,6 +948,12 @@ inline cudaError_t launch_one(const GridP& g, const EnvP& env, const ShadeP& sp,
   const int grid = (int)(need < (unsigned long long)num_sms ? need : (unsigned long long)num_sms);
   kern<<<grid, kRows * G, SP::bytes, st>>>(g, env, sp, cw, d_tiles, wts32, fr, rgb, ring, counters);
   return cudaGetLastError();
+}
+
+template <bool F16TAB, int PREC, bool TSHARED, int G>
+inline cudaError_t render_attr() {
+  return cudaFuncSetAttribute(k_render_wg<F16TAB, PREC, TSHARED, G>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                              (int)SmemPlan<PREC, TSHARED, G>::bytes);
 }
 
 }  // namespace wg

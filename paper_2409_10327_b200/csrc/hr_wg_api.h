@@ -26,10 +26,18 @@ cudaError_t launch_p0(bool f16tab, const GridP& g, const EnvP& env, const ShadeP
 cudaError_t launch_p1(bool f16tab, const GridP& g, const EnvP& env, const ShadeP& sp, const void* tc_const, const uint8_t* d_tiles,
                       const float* wts32, const FrameP& fr, float* rgb, void* ring, unsigned long long* counters, int num_sms, cudaStream_t st);
 
-// hashrender_trace with the encode fused, fp16 models (k_trace_wg)
+// hashrender_trace (k_trace_wg): p0 = fp16 models, p1 = fp32 models in split precision (the arithmetic launch_p1 runs).
+// feat == nullptr: the encode is fused; otherwise the caller's features [N, 2 L] are used and x is only needed for xsec.
 cudaError_t launch_trace_p0(bool f16tab, const GridP& g, const ShadeP& sp, const void* tc_const, const uint8_t* d_tiles, const float* x,
-                            unsigned long long N, const DirsetP& ds, float* vis, float* zv, float* t, float* xsec, int num_sms,
-                            cudaStream_t st);
+                            const float* feat, unsigned long long N, const DirsetP& ds, float* vis, float* zv, float* t, float* xsec,
+                            int num_sms, cudaStream_t st);
+cudaError_t launch_trace_p1(bool f16tab, const GridP& g, const ShadeP& sp, const void* tc_const, const uint8_t* d_tiles, const float* x,
+                            const float* feat, unsigned long long N, const DirsetP& ds, float* vis, float* zv, float* t, float* xsec,
+                            int num_sms, cudaStream_t st);
+
+// Opt-in of every kernel of the family to its dynamic shared-memory size, for the CURRENT device (hashrender_create calls both).
+cudaError_t init_device_p0();
+cudaError_t init_device_p1();
 
 }  // namespace wg
 }  // namespace hr

@@ -32,11 +32,21 @@ cudaError_t launch_p0(bool f16tab, const GridP& g, const EnvP& env, const ShadeP
 }
 
 cudaError_t launch_trace_p0(bool f16tab, const GridP& g, const ShadeP& sp, const void* tc_const, const uint8_t* d_tiles, const float* x,
-                            unsigned long long N, const DirsetP& ds, float* vis, float* zv, float* t, float* xsec, int num_sms,
-                            cudaStream_t st) {
+                            const float* feat, unsigned long long N, const DirsetP& ds, float* vis, float* zv, float* t, float* xsec,
+                            int num_sms, cudaStream_t st) {
   const TcConst& cw = *reinterpret_cast<const TcConst*>(tc_const);
-  if (f16tab) return launch_trace_one<true>(g, sp, cw, d_tiles, x, N, ds, vis, zv, t, xsec, num_sms, st);
-  return launch_trace_one<false>(g, sp, cw, d_tiles, x, N, ds, vis, zv, t, xsec, num_sms, st);
+  if (f16tab) return launch_trace_one<true, 0>(g, sp, cw, d_tiles, x, feat, N, ds, vis, zv, t, xsec, num_sms, st);
+  return launch_trace_one<false, 0>(g, sp, cw, d_tiles, x, feat, N, ds, vis, zv, t, xsec, num_sms, st);
+}
+
+cudaError_t init_device_p0() {
+  cudaError_t e;
+  if ((e = render_attr<true, 0, true, HR_G_P0>()) != cudaSuccess) return e;
+  if ((e = render_attr<true, 0, false, 2>()) != cudaSuccess) return e;
+  if ((e = render_attr<false, 0, true, HR_G_P0>()) != cudaSuccess) return e;
+  if ((e = render_attr<false, 0, false, 2>()) != cudaSuccess) return e;
+  if ((e = trace_attr<true, 0>()) != cudaSuccess) return e;
+  return trace_attr<false, 0>();
 }
 
 }  // namespace wg

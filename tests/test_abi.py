@@ -76,3 +76,28 @@ def test_binding_fails_loudly_without_library(tmp_path):
             binding.load_library(str(tmp_path / "nope.so"))
     finally:
         binding._lib = old
+
+
+def test_binding_rejects_wrong_dtype_placement_and_alignment():
+    """The binding marshals raw pointers, so it must refuse what the C side cannot see: a float64 array, a host array handed to a
+    device entry point (or the reverse), a misaligned pdf buffer."""
+    import numpy as np
+    from paper_2409_10327_b200 import binding as B
+    a32, a64 = np.zeros((4, 3), np.float32), np.zeros((4, 3), np.float64)
+    assert B._arg(None, "x") is None
+    assert B._arg(a32, "x", "f32", "host").value == a32.ctypes.data
+    with pytest.raises(TypeError):
+        B._arg(a64, "x", "f32", "host")
+    with pytest.raises(TypeError):
+        B._arg(a32, "x", "f32", "device")                     # a host array is not a device pointer
+    with pytest.raises(ValueError):
+        B._arg(np.zeros(9, np.float32)[1:], "pdf", "f32", "host", align=8)
+    import torch
+    t = torch.zeros((4, 3))
+    assert B._arg(t, "x", "f32", "host").value == t.data_ptr()
+    with pytest.raises(TypeError):
+        B._arg(t.double(), "x", "f32", "host")
+    with pytest.raises(TypeError):
+        B.DirSet(a32.reshape(1, 4, 3), a64[:, 0].reshape(1, 4)).c("host")
+    d = B.DirSet(np.zeros(40, np.float32), np.zeros(13, np.float32), S=3, point_stride=12).c("host")
+    assert d.S == 3 and d.point_stride == 12

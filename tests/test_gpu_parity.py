@@ -13,7 +13,13 @@ from hr_testutil import check_close, gpu_render, make_renderer, oracle_render, t
 pytestmark = pytest.mark.gpu
 
 TOL32, TOL16 = 1e-4, 3e-3
-DELTA32, DELTA16 = 1e-4, 4e-3      # |z_v| band in which a hard-visibility flip is legitimate (Q33)
+# |z_v| band in which a hard-visibility flip is legitimate (Q33): <= 3x the largest |z_v(gpu) - z_v(oracle)|
+# the stage-wise tests below measure on the production arithmetic (test_decode_trace_shade_stagewise prints and bounds it).
+DELTA32, DELTA16 = 2e-5, 4e-3
+# share of the reference radiance that the hard-mode flip allowance may amount to (mean flipbound / mean |o|): the allowance
+# must stay an exception.  fp16: a sample flips inside |z_v| < 4e-3 while the logits of these synthetic models spread over
+# only +-0.1, so ~5 % of the samples sit in the band.
+FLIPSHARE32, FLIPSHARE16 = 2e-3, 0.12
 
 
 @pytest.fixture(scope="module")
@@ -82,9 +88,12 @@ def test_encode_empty_and_errors(torch):
 
 
 # ---------------------------------------------------------------------------------------------- decode / trace / shade
-@pytest.mark.parametrize("name", ["C0", "C1", "C3"])
+@pytest.mark.parametrize("name", ["C0", "C1", "C2", "C3"])
 def test_decode_trace_shade_stagewise(torch, name):
-    """Stage-wise parity on ORACLE-supplied inputs (the strict test, SURVEY 8(c) conditioning note)."""
+    """Stage-wise parity on ORACLE-supplied inputs (the strict test, SURVEY 8(c) conditioning note).  hashrender_trace runs the
+    tensor-core arithmetic render_frame runs for this model (fp32 models: hi/lo split precision, `tcgen05-f16x3`), with the
+    oracle's features and with the encode fused; the largest |z_v(gpu) - z_v(oracle)| is printed and must stay below a third
+    of the hard-visibility flip band."""
     cfg = gen.make_config(name)
     m = gen.make_model(cfg)
     n = 777
@@ -105,15 +114,21 @@ def test_decode_trace_shade_stagewise(torch, name):
     # trace on oracle features, then with the encode fused
     from paper_2409_10327_b200 import DirSet
     ds = DirSet(to_dev(fr["dir_d"]), to_dev(fr["pdf_d"]))
+    delta = DELTA16 if cfg.mlp_dtype == "f16" else DELTA32
     for fused in (False, True):
         vis = torch.empty((n, S), device="cuda"); zv = torch.empty((n, S), device="cuda"); t = torch.empty((n, S), device="cuda")
         xs = torch.empty((n, S, 3), device="cuda")
         r.trace(to_dev(fr["x"]), None if fused else featd, ds, vis, zv, t, xs)
         torch.cuda.synchronize()
+        assert r.last_path() == ("tcgen05-f16" if cfg.mlp_dtype == "f16" else "tcgen05-f16x3"), r.last_path()
         check_close(vis.cpu().numpy(), vis_o, tol, what="trace vis")
         check_close(t.cpu().numpy(), t_o, tol, what="trace t")
         check_close(zv.cpu().numpy(), zv_o, tol, extra=tol * 0.05, what="trace zv")
         check_close(xs.cpu().numpy(), xs_o, tol, what="trace x'")
+        dzv = float(np.abs(zv.cpu().numpy() - zv_o).max())
+        dt = float(np.abs(t.cpu().numpy() - t_o).max())
+        print(f"[stagewise {name} fused={fused}] path={r.last_path()} max|dz_v|={dzv:.3e} max|dt|={dt:.3e} (delta={delta:g})")
+        assert 3.0 * dzv <= delta, f"flip band {delta} must be >= 3x the measured z_v error {dzv:.3e}"
     # hard mode: bits agree wherever |z_v| >= delta
     oh = _oracle(cfg, m, vis_mode=1)
     vh_o, zvh_o, _, _ = oh.trace(fr["x"], feat_o, fr["dir_d"])
@@ -122,10 +137,10 @@ def test_decode_trace_shade_stagewise(torch, name):
     rh.trace(to_dev(fr["x"]), featd, ds, vis, None, t)
     vh = vis.cpu().numpy()
     assert set(np.unique(vh)) <= {0.0, 1.0}
-    delta = DELTA16 if cfg.mlp_dtype == "f16" else DELTA32
     sure = np.abs(zvh_o) >= delta
     assert np.array_equal(vh[sure], vh_o[sure])
     assert sure.mean() > 0.9
+    assert 0.2 <= vh_o.mean() <= 0.8, "hard visibility must be balanced (gen vis_bias)"
     # shade: direct only, then Eq. 2 on one set with a synthetic L'_o
     rng = np.random.default_rng(5)
     Lind = rng.random((n, S, 3)).astype(np.float32)
@@ -167,7 +182,28 @@ def _frame_case(torch, name, pix, vis_mode, flags=None, over=None, tol=None, del
     r = make_renderer(cfg, m, vis_mode=vis_mode)
     got = gpu_render(r, cfg, fr, flags=flags, brdf=brdf, mask=mask)
     worst = check_close(got, ref["rgb"], tol, extra=ref["flipbound"] if vis_mode else None, what=f"{name} vis_mode={vis_mode}")
+    _nontrivial(name, cfg, m, fr, ref, vis_mode, mask, worst)
     return cfg, ref, got, worst, r
+
+
+def _nontrivial(name, cfg, m, fr, ref, vis_mode, mask=None, worst=float("nan")):
+    """The reference must be a real image, hard visibility must be balanced, and the flip allowance an exception."""
+    live = np.ones(len(fr["x"]), bool) if mask is None else np.asarray(mask, bool)
+    mean_o = float(np.abs(ref["rgb"][live]).mean())
+    assert mean_o > 0.05, f"{name}: reference image is (nearly) black: mean|o| = {mean_o:.4g}"
+    msg = f"[frame {name} vis_mode={vis_mode}] pixels={len(fr['x'])} mean|o|={mean_o:.4f} worst err/allowed={worst:.3f}"
+    if vis_mode:
+        o = _oracle(cfg, m, vis_mode=1)
+        feat, _, _ = o.encode(fr["x"])
+        vfrac = float(o.trace(fr["x"], feat, fr["dir_d"])[0].mean())
+        assert 0.2 <= vfrac <= 0.8, f"{name}: hard-visibility visible fraction {vfrac:.3f} outside [0.2, 0.8]"
+        fb = ref["flipbound"][live]
+        share_el = float((fb > 0).mean())
+        share_mag = float(fb.mean() / mean_o)
+        lim = FLIPSHARE16 if cfg.mlp_dtype == "f16" else FLIPSHARE32
+        assert share_mag <= lim, f"{name}: flip allowance is {share_mag:.3g} of the mean radiance (limit {lim})"
+        msg += f" visible={vfrac:.3f} elements with a flip allowance={share_el:.3f} mean flipbound/mean|o|={share_mag:.2e}"
+    print(msg)
 
 
 @pytest.mark.parametrize("vis_mode", [0, 1])
@@ -199,31 +235,31 @@ def test_frame_C3_fp16_subset(torch, name, vis_mode):
     _frame_case(torch, name, pix, vis_mode)
 
 
-def test_frame_variants_small(torch):
-    """External BRDF (Q30), mask (Q27), Lambert model, flag subsets, per-secondary-point tertiary sets, ragged N."""
+@pytest.mark.parametrize("table_scale,tolv", [(0.1, TOL32), (1.0, 4e-4)])
+def test_frame_variants_small(torch, table_scale, tolv):
+    """External BRDF (Q30), mask (Q27), Lambert model, flag subsets, per-secondary-point tertiary sets (the TSHARED = false,
+    G = 2 kernels), ragged N.  On a 0.1-scale table (the scale of BASELINE configs 1-3) every variant holds north_star's 1e-4.
+    The second run keeps C0's own U(-1,1) table WITH an indirect bounce, an off-spec combination: the fp32 error of t (~4e-6)
+    moves x' and is amplified by N_max * |grad tab| ~ 256 * 2 into a ~1e-3 feature error at the finest level (SURVEY 8(c)
+    conditioning note), so it is an extra at 4e-4, not the bar."""
     rng = np.random.default_rng(9)
     n = 333
     pix = np.arange(n)
-    over = dict(S_i=4, S_2=3, flags=7)
+    over = dict(S_i=4, S_2=3, flags=7, table_scale=table_scale)
     cfg = gen.make_config("C0", **over)
     brdf = np.concatenate([gen._normalize(rng.standard_normal((n, 3))), rng.random((n, 3)), 0.09 + 0.91 * rng.random((n, 1))], 1).astype(np.float32)
     mask = (rng.random(n) > 0.3).astype(np.uint8)
-    # Off-spec combination (C0's U(-1,1) tables WITH an indirect bounce): the fp32 error of t (~4e-6, 64-term fp32 dot
-    # products) moves x' and is amplified by N_max * |grad tab| ~ 256 * 2 into a ~1e-3 feature error at the finest level
-    # (SURVEY 8(c) conditioning note), so end-to-end radiance is only good to a few 1e-4 here; the BASELINE configs
-    # (C0 direct-only, C1/C2 with 0.1-scale tables) keep the stated 1e-4.
-    TOLV = 4e-4
-    _frame_case(torch, "C0", pix, 0, over=over, brdf=brdf, mask=mask, tol=TOLV)
+    _frame_case(torch, "C0", pix, 0, over=over, brdf=brdf, mask=mask, tol=tolv)
     for flags in (1, 3):
         _frame_case(torch, "C0", pix, 0, flags=flags, over=over)
     for flags in (4, 6, 5):
-        _frame_case(torch, "C0", pix, 0, flags=flags, over=over, tol=TOLV)
+        _frame_case(torch, "C0", pix, 0, flags=flags, over=over, tol=tolv)
     # Lambert
     m = gen.make_model(cfg); fr = gen.make_frame(cfg, m["env"], pix)
     o = _oracle(cfg, m, brdf_model=0)
     ref = oracle_render(o, cfg, fr, flags=7)
     got = gpu_render(make_renderer(cfg, m, brdf_model=0), cfg, fr, flags=7)
-    check_close(got, ref["rgb"], TOLV, what="lambert")
+    check_close(got, ref["rgb"], tolv, what="lambert")
     # per-secondary-point tertiary sets (point_stride != 0, the paper's literal reading of PAPER.md:344)
     dt = gen._normalize(rng.standard_normal((n * 4, 3, 3))).astype(np.float32)
     dt = gen._normalize(dt.astype(np.float64)).astype(np.float32)
@@ -231,8 +267,36 @@ def test_frame_variants_small(torch):
     fr2 = dict(fr); fr2["dir_t"], fr2["pdf_t"] = dt, pt
     o = _oracle(cfg, m)
     ref = oracle_render(o, cfg, fr2, flags=7)
-    got = gpu_render(make_renderer(cfg, m), cfg, fr2, flags=7)
-    check_close(got, ref["rgb"], TOLV, what="per-point tertiary")
+    r = make_renderer(cfg, m)
+    got = gpu_render(r, cfg, fr2, flags=7)
+    assert r.last_path() == "tcgen05-f16x3"
+    check_close(got, ref["rgb"], tolv, what="per-point tertiary")
+    # the same per-point sets with an fp16 model (the G = 2 instantiation of the fp16 kernel)
+    cfgh = gen.make_config("C0", **over, table_dtype="f16", mlp_dtype="f16")
+    mh = gen.make_model(cfgh)
+    ref = oracle_render(_oracle(cfgh, mh), cfgh, fr2, flags=7)
+    rh = make_renderer(cfgh, mh)
+    got = gpu_render(rh, cfgh, fr2, flags=7)
+    assert rh.last_path() == "tcgen05-f16"
+    check_close(got, ref["rgb"], TOL16 if table_scale < 1 else 4 * TOL16, what="per-point tertiary fp16")
+
+
+@pytest.mark.parametrize("L,S_2", [(8, 8), (14, 8), (5, 16)])
+def test_prefetched_encode_with_fewer_than_16_levels(torch, L, S_2):
+    """fp32 model, indirect bounce, SHARED tertiary set with S_2 >= 8: the split-precision kernel encodes the next group of
+    secondary points while it runs the tertiary queries of the current one (two levels per query).  Levels l >= L do not
+    exist -- their table slice would lie past the allocation -- so they must be skipped and read as zero features.  L = 14 is
+    the paper's own grid, S_2 = 8 its tertiary count."""
+    over = dict(S_i=8, S_2=S_2, flags=7, L=L, table_scale=0.1, max_res=256 if L <= 8 else 1024, log2_T=14 if L <= 8 else 17)
+    n = 700                                               # 5600 secondary items: many 128-item groups follow one another
+    cfg, ref, got, worst, r = _frame_case(torch, "C0", np.arange(n), 0, over=over)
+    assert r.last_path() == "tcgen05-f16x3" and ref["n_sec"] == n * 8
+    # the table is the last allocation the handle made that a stray gather could run past: render again right after creating and
+    # destroying a neighbour handle, and with HR_DENSE
+    from paper_2409_10327_b200 import HR_DENSE
+    m = gen.make_model(cfg); fr = gen.make_frame(cfg, m["env"], np.arange(n))
+    got2 = gpu_render(r, cfg, fr, flags=7 | HR_DENSE)
+    np.testing.assert_allclose(got2, got, rtol=5e-6, atol=1e-7)
 
 
 def test_frame_closed_form_on_gpu(torch):
@@ -306,6 +370,55 @@ def test_render_frame_host_chunked_pipeline(torch):
     np.testing.assert_allclose(a, b2, rtol=2e-6, atol=1e-7)
 
 
+def test_render_frame_host_chunks_per_point_tertiary_and_padded_rows(torch):
+    """The multi-chunk host path with everything that moves per chunk: per-point direct / secondary sets whose rows are PADDED
+    (point_stride > 3 S, so the last row is shorter than the stride), per-SECONDARY-point tertiary sets (row i S_i + j), a mask."""
+    from paper_2409_10327_b200 import DirSet
+    cfg = gen.make_config("C2", N=400_000, S_d=3, S_i=2, S_2=2)
+    m = gen.make_model(cfg)
+    fr = gen.make_frame(cfg, m["env"])
+    N = cfg.N
+    rng = np.random.default_rng(12)
+
+    def padded(d, p, pad):                                 # [N,S,3] -> rows of S + pad directions; the last point's row is cut short
+        S = d.shape[1]
+        dd = np.full((N, S + pad, 3), np.nan, np.float32); dd[:, :S] = d
+        pp = np.full((N, S + pad), np.nan, np.float32); pp[:, :S] = p
+        return dd.reshape(-1)[: (N - 1) * 3 * (S + pad) + 3 * S].copy(), pp.reshape(-1)[: (N - 1) * (S + pad) + S].copy(), S, 3 * (S + pad)
+
+    dd, pd_, Sd, std = padded(fr["dir_d"], fr["pdf_d"], 2)
+    sd, ps_, Ss, sts = padded(fr["dir_s"], fr["pdf_s"], 1)
+    dt = gen._normalize(rng.standard_normal((N * cfg.S_i, cfg.S_2, 3)))
+    dt = gen._normalize(dt.astype(np.float32).astype(np.float64)).astype(np.float32)
+    pt = np.full((N * cfg.S_i, cfg.S_2), 1 / (4 * np.pi), np.float32)
+    mask = (np.arange(N) % 5 != 0).astype(np.uint8)
+    r = make_renderer(cfg, m)
+    outs = []
+    for host in (False, True):
+        up = (lambda a: np.ascontiguousarray(a)) if host else to_dev
+        sets = [DirSet(up(dd), up(pd_), S=Sd, point_stride=std), DirSet(up(sd), up(ps_), S=Ss, point_stride=sts), DirSet(up(dt), up(pt))]
+        frame = r.make_frame(up(fr["x"]), up(fr["wo"]), *sets, flags=7, mask=up(mask))
+        if host:
+            rgb = np.empty((N, 3), np.float32)
+            l0 = r.launch_count()
+            r.render_frame_host(frame, rgb)
+            assert r.launch_count() - l0 >= 2, "the frame must have been cut into several chunks"
+        else:
+            t = torch.empty((N, 3), device="cuda")
+            r.render_frame(frame, t)
+            rgb = t.cpu().numpy()
+        assert np.all(np.isfinite(rgb))
+        outs.append(rgb)
+    np.testing.assert_allclose(outs[0], outs[1], rtol=2e-6, atol=1e-7)
+    assert np.all(outs[0][mask == 0] == 0) and np.abs(outs[0]).mean() > 0.05
+    # and against the oracle on a pixel sample (tight rows of the same values)
+    pix = np.sort(rng.choice(N, 150, replace=False))
+    sub = dict(x=fr["x"][pix], wo=fr["wo"][pix], dir_d=fr["dir_d"][pix], pdf_d=fr["pdf_d"][pix], dir_s=fr["dir_s"][pix], pdf_s=fr["pdf_s"][pix],
+               dir_t=dt.reshape(N, cfg.S_i, cfg.S_2, 3)[pix].reshape(-1, cfg.S_2, 3), pdf_t=pt.reshape(N, cfg.S_i, cfg.S_2)[pix].reshape(-1, cfg.S_2))
+    ref = oracle_render(_oracle(cfg, m), cfg, sub, flags=7, mask=mask[pix])
+    check_close(outs[1][pix], ref["rgb"], TOL32, what="host path, per-point tertiary, padded rows")
+
+
 def test_fp32_model_outside_the_fp16_range_uses_the_ffma_kernels(torch):
     """The tcgen05 fp32 path carries operands as fp16 hi + lo; a model whose weights / activation bounds do not fit that range must
     fall back to the plain fp32 kernels (hashrender_last_path says which) and still match the oracle."""
@@ -350,25 +463,80 @@ def test_frame_errors(torch):
 # ---------------------------------------------------------------------------------------------- full size, bench configuration
 @pytest.mark.parametrize("name", ["C1", "C2", "C3"])
 def test_full_size_sampled_pixels(torch, name):
-    """BASELINE full size (800x800, 128 + 64x8 directions) in the launch configuration bench.py times; the oracle
-    checks a seeded sample of pixels one by one (it needs ~6 ms per pixel)."""
+    """BASELINE full size (800x800, 128 + 64x8 directions) in the launch configurations bench.py times -- both visibility
+    modes, the default flags (compacted) and HR_DENSE (bench's headline); the oracle checks a seeded sample of pixels one by
+    one (it needs ~6 ms per pixel).  The reference must be a real image in both modes."""
+    from paper_2409_10327_b200 import HR_DENSE
     cfg = gen.make_config(name)
     m = gen.make_model(cfg)
     fr = gen.make_frame(cfg, m["env"])
-    r = make_renderer(cfg, m, vis_mode=1)
-    got = gpu_render(r, cfg, fr)
-    assert np.all(np.isfinite(got)) and got.shape == (cfg.N, 3)
     rng = np.random.default_rng(77)
     pix = np.sort(np.concatenate([rng.choice(cfg.N, 188, replace=False), [0, 799, 639200, 639999]]))
     sub = {k: (v[pix] if k not in ("dir_t", "pdf_t") else v) for k, v in fr.items()}
     f16 = cfg.mlp_dtype == "f16"
-    o = _oracle(cfg, m, vis_mode=1)
-    ref = oracle_render(o, cfg, sub, delta=DELTA16 if f16 else DELTA32)
-    # tolerance scale s (mean |o|) from the sample itself
-    check_close(got[pix], ref["rgb"], TOL16 if f16 else TOL32, extra=ref["flipbound"], what=f"{name} full-size sample")
+    indirect = bool(cfg.flags & gen.HR_INDIRECT)
+    for vis_mode in (1, 0):
+        r = make_renderer(cfg, m, vis_mode=vis_mode)
+        o = _oracle(cfg, m, vis_mode=vis_mode)
+        ref = oracle_render(o, cfg, sub, delta=(DELTA16 if f16 else DELTA32) if vis_mode else 0.0)
+        for flags in ([cfg.flags, cfg.flags | HR_DENSE] if indirect else [cfg.flags]):
+            got = gpu_render(r, cfg, fr, flags=flags)
+            assert np.all(np.isfinite(got)) and got.shape == (cfg.N, 3)
+            assert r.last_path() == ("tcgen05-f16" if f16 else "tcgen05-f16x3")
+            # tolerance scale s (mean |o|) from the sample itself
+            worst = check_close(got[pix], ref["rgb"], TOL16 if f16 else TOL32, extra=ref["flipbound"] if vis_mode else None,
+                                what=f"{name} full-size sample vis_mode={vis_mode} flags={flags}")
+            assert abs(float(got.mean()) / float(got[pix].mean()) - 1) < 0.25      # the whole frame looks like its sample
+        _nontrivial(f"{name} full size", cfg, m, sub, ref, vis_mode, worst=worst)
+        r.destroy()
     # a generator subset reproduces the same inputs as the full frame (so bench's CPU sample is the same workload)
     fr_sub = gen.make_frame(cfg, m["env"], pix)
     assert np.array_equal(fr_sub["dir_d"], sub["dir_d"]) and np.array_equal(fr_sub["x"], sub["x"])
+
+
+@pytest.mark.parametrize("name", ["C1", "C3a"])
+def test_direct_visibility_bits_of_the_render_kernel(torch, name):
+    """Hard visibility as the RENDER kernel decides it, read back bit by bit.  Direct term only, external Lambert BRDF with
+    albedo 1 and normal n_g, pdf = (n.w)/pi (so f_r (n.w)/p = 1) and caller-supplied radiance Lin_k = 2^k: the pixel value
+    times S is the integer sum_k v_k 2^k, exactly.  Every bit must equal the oracle's [z_v > 0] wherever |z_v| >= delta, and the
+    largest |z_v| at which a bit differs is printed: it is the z_v error of the kernel's own direct-query arithmetic (fp16:
+    the fp16x2 final-layer epilogue `epi_fast`; fp32 models: split precision), which hashrender_trace does not go through."""
+    from paper_2409_10327_b200 import DirSet
+    cfg = gen.make_config(name)
+    m = gen.make_model(cfg)
+    n, S = 6000, 16
+    pix = np.sort(np.random.default_rng(31).choice(cfg.N, n, replace=False))
+    x, n_g, wo = gen.make_points(cfg, pix)
+    d, _ = gen.make_cosine_hemisphere_dirs(cfg, n_g, pix, S, gen._ST_DIR_S)
+    cos = np.einsum("nsk,nk->ns", d.astype(np.float64), n_g.astype(np.float64))
+    keep = (cos > 1e-3).all(axis=1)                                        # every sample strictly above the horizon
+    x, n_g, wo, d, cos = x[keep], n_g[keep], wo[keep], d[keep], cos[keep]
+    n = len(x)
+    pdf = (cos / np.pi).astype(np.float32)
+    Lin = np.zeros((n, S, 3), np.float32); Lin[:, :, 0] = 2.0 ** np.arange(S); Lin[:, :, 1] = 1.0
+    brdf = np.concatenate([n_g, np.ones((n, 3), np.float32), np.full((n, 1), 0.5, np.float32)], 1)
+    o = _oracle(cfg, m, vis_mode=1)
+    feat, _, _ = o.encode(x)
+    _, zv_o, _, _ = o.trace(x, feat, d)
+    r = make_renderer(cfg, m, vis_mode=1, brdf_model=0)
+    rgb = torch.empty((n, 3), device="cuda")
+    r.render_frame(r.make_frame(to_dev(x), to_dev(wo), DirSet(to_dev(d), to_dev(pdf), to_dev(Lin)), flags=3, brdf=to_dev(brdf)), rgb)
+    got = rgb.cpu().numpy().astype(np.float64)
+    code = got[:, 0] * S
+    assert np.abs(code - np.round(code)).max() < 0.2, "pixel value is not an integer code"
+    bits = (np.round(code).astype(np.int64)[:, None] >> np.arange(S)[None, :]) & 1
+    np.testing.assert_allclose(got[:, 1] * S, bits.sum(axis=1), atol=1e-3)      # green counts the visible samples
+    ref_bits = (zv_o > 0).astype(np.int64)
+    diff = bits != ref_bits
+    f16 = cfg.mlp_dtype == "f16"
+    delta = DELTA16 if f16 else DELTA32
+    worst = float(np.abs(zv_o[diff]).max()) if diff.any() else 0.0
+    print(f"[render-kernel visibility bits {name}] path={r.last_path()} queries={bits.size} visible={ref_bits.mean():.3f} "
+          f"flipped={int(diff.sum())} ({diff.mean():.2e}) largest |z_v| at a flip={worst:.3e} (delta={delta:g})")
+    assert r.last_path() == ("tcgen05-f16" if f16 else "tcgen05-f16x3")
+    assert 0.2 <= ref_bits.mean() <= 0.8
+    assert worst < delta, "a visibility bit differs outside the flip band"
+    assert diff.mean() < (0.03 if f16 else 5e-4), "flip fraction"
 
 
 @pytest.mark.parametrize("log2_T", [16, 19, 22, 24])

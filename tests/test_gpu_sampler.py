@@ -121,3 +121,61 @@ def test_sampler_errors(torch):
     with pytest.raises(HashRenderError):
         r.sample_stratified(None, 4, 0, 2, 1, d, p)
     r.sample_stratified(None, 0, 2, 2, 1, d, p)                        # rows == 0: no-op
+
+
+@pytest.mark.parametrize("name", ["C2", "C3"])
+def test_sampled_frame_composition_matches_oracle(torch, name):
+    """bench.py's `e2e_sampled` composition -- hashrender_encode -> decode -> sample_mis (direct set) ->
+    sample_stratified (secondary set about the decoded normal; shared tertiary sphere set) -> render_frame --
+    against the same composition of the oracles (hash-renderer oracle + sampler oracle) from the same x, w_o, env and seeds.
+    (i) strict: the oracle renderer on the rays the GPU generated, at the config's tolerance; (ii) the two compositions end to
+    end: their rays differ by the sampler's fp32 error (GGX rays up to 2e-4, test_sample_mis_matches_oracle), so the bar is
+    10x the config's tolerance and the measured error is printed."""
+    from oracle import sampler as S
+    from oracle.oracle import Oracle
+    from hr_testutil import check_close
+    from paper_2409_10327_b200 import DirSet
+    cfg = gen.make_config(name, S_d=32, S_i=16, S_2=8)
+    m = gen.make_model(cfg)
+    n = 600
+    pix = np.sort(np.random.default_rng(8).choice(cfg.N, n, replace=False))
+    x, _, wo = gen.make_points(cfg, pix)
+    spp, sa, (ta, tb) = cfg.S_d // 2, 4, (4, 2)
+    seeds = (2409, 10327, 7)
+    tol = cfg.tol
+    for vis_mode in (0, 1):
+        r = make_renderer(cfg, m, vis_mode=vis_mode)
+        xd, wod = to_dev(x), to_dev(wo)
+        feat = torch.empty((n, cfg.D), device="cuda"); brdf = torch.empty((n, 7), device="cuda")
+        dd = torch.empty((n, 2 * spp, 3), device="cuda"); pd = torch.empty((n, 2 * spp), device="cuda")
+        ds_ = torch.empty((n, sa * sa, 3), device="cuda"); ps_ = torch.empty((n, sa * sa), device="cuda")
+        dt_ = torch.empty((ta * tb, 3), device="cuda"); pt_ = torch.empty((ta * tb,), device="cuda")
+        r.encode(xd, feat)
+        r.decode(feat, brdf)
+        r.sample_mis(brdf, wod, spp, seeds[0], dd, pd)
+        r.sample_stratified(brdf[:, :3].contiguous(), n, sa, sa, seeds[1], ds_, ps_)
+        r.sample_stratified(None, 1, ta, tb, seeds[2], dt_, pt_)
+        rgb = torch.empty((n, 3), device="cuda")
+        r.render_frame(r.make_frame(xd, wod, DirSet(dd, pd), DirSet(ds_, ps_), DirSet(dt_, pt_), flags=7), rgb)
+        torch.cuda.synchronize()
+        got = rgb.cpu().numpy()
+        o = Oracle.from_gen(cfg, m, vis_mode=vis_mode)
+        delta = (4e-3 if cfg.mlp_dtype == "f16" else 2e-5) if vis_mode else 0.0
+        # (i) the oracle renderer on the GPU's own rays
+        ref = o.render_frame(x, wo, (dd.cpu().numpy(), pd.cpu().numpy()), (ds_.cpu().numpy(), ps_.cpu().numpy()),
+                             (dt_.cpu().numpy(), pt_.cpu().numpy()), flags=7, delta=delta)
+        w1 = check_close(got, ref["rgb"], tol, extra=ref["flipbound"] if vis_mode else None, what=f"sampled frame {name} (GPU rays)")
+        assert np.abs(ref["rgb"]).mean() > 0.05
+        if vis_mode:
+            continue
+        # (ii) the oracle composition from x, w_o alone
+        fo, _, _ = o.encode(x, want_idx=False)
+        bo = o.decode(fo).astype(np.float32)
+        d1, p1, _ = S.sample_mis(m["env"], bo, wo, spp, seeds[0])
+        d2, p2 = S.sample_stratified(np.ascontiguousarray(bo[:, :3]), n, sa, sa, seeds[1])
+        d3, p3 = S.sample_stratified(None, 1, ta, tb, seeds[2])
+        f32 = lambda a: np.ascontiguousarray(a, np.float32)
+        ref2 = o.render_frame(x, wo, (f32(d1), f32(p1)), (f32(d2), f32(p2)), (f32(d3[0]), f32(p3[0])), flags=7)
+        w2 = check_close(got, ref2["rgb"], 10 * tol, what=f"sampled frame {name} (oracle composition)")
+        print(f"[sampled composition {name}] worst err/allowed: on GPU rays {w1:.3f} (tol {tol:g}), oracle composition {w2:.3f} (tol {10 * tol:g})")
+        r.destroy()
