@@ -15,11 +15,11 @@ pytestmark = pytest.mark.gpu
 TOL32, TOL16 = 1e-4, 3e-3
 # |z_v| band in which a hard-visibility flip is legitimate (Q33): <= 3x the largest |z_v(gpu) - z_v(oracle)|
 # the stage-wise tests below measure on the production arithmetic (test_decode_trace_shade_stagewise prints and bounds it).
-DELTA32, DELTA16 = 2e-5, 4e-3
+DELTA32, DELTA16 = 5e-6, 5e-4
 # share of the reference radiance that the hard-mode flip allowance may amount to (mean flipbound / mean |o|): the allowance
-# must stay an exception.  fp16: a sample flips inside |z_v| < 4e-3 while the logits of these synthetic models spread over
-# only +-0.1, so ~5 % of the samples sit in the band.
-FLIPSHARE32, FLIPSHARE16 = 2e-3, 0.12
+# must stay an exception.  fp16: a sample may flip inside |z_v| < 5e-4 (measured error of the fp16 arithmetic: 1.0e-4 stage-wise,
+# 1.3e-4 at the render kernel's own visibility bits) while the logits of these synthetic models spread over only +-0.1.
+FLIPSHARE32, FLIPSHARE16 = 2e-3, 0.05
 
 
 @pytest.fixture(scope="module")
