@@ -467,7 +467,11 @@ __global__ void __launch_bounds__(kRows* G, 1)
                 const float* __restrict__ wts32, FrameP fr, float* __restrict__ rgb, Item* __restrict__ ring,
                 unsigned long long* __restrict__ counters) {
   using CL = Cols<PREC, G>;
+#ifdef HR_LIF
+  constexpr int LIF = HR_LIF;
+#else
   constexpr int LIF = G == 4 ? 2 : 4;               // register budget: 128 per thread at G = 4
+#endif
   using SP = SmemPlan<PREC, TSHARED, G>;
   extern __shared__ uint8_t smem_raw[];
   uint8_t* sp0 = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);
