@@ -184,6 +184,38 @@ const char* hashrender_last_path(const hashrender_t* h);
 
 const char* hashrender_last_error(const hashrender_t* h);
 
+/* ---- The step before the path: the CNN direct-illumination renderer G (Fig. 2, 90-96, 134; Q45-Q51) --------
+ * "The direct illumination renderer G takes rays as input and outputs the material, normal, and primary surface coordinates"
+ * (PAPER.md:80): one forward pass turns the ray map gamma = [o, d_down] of an h x w pixel array into full-resolution
+ * (8h x 8w) maps, written straight into the arrays hr_frame takes.  Architecture: 1x1 conv-norm-act stem (6 -> width), n_res 1x1
+ * conv-norm-act layers in residual blocks of two (x <- x + L2(L1(x))), three super-resolution blocks (bilinear x2, two 3x3
+ * conv-norm-act layers with sr_ch[s] channels, 1x1 output mapping to 11 channels) joined by the output skip; norm = instance
+ * normalisation with affine parameters (eps 1e-5, biased variance), act = exact GELU; output channels [n3 a3 r1 x3 mask1] with the
+ * maps n/||n||, sigma(a), rough_min + (1 - rough_min) sigma(r), x = sigma(.), mask = [. > 0].  The paper's model: width 256,
+ * n_res 28, sr_ch 128/64/32, h = w = 100.
+ * Every convolution is a tcgen05 implicit GEMM fed by TMA; activations travel as fp16 hi + lo pairs with fp32 accumulation and fp32
+ * normalisation / GELU / residual / upsampling, so the result is fp32-grade.  Convolution weights must be fp16-representable.
+ * weights: host, fp32, per layer W[Cout][Cin][k][k], b[Cout] and (conv-norm-act layers) gamma[Cout], beta[Cout], in the order stem,
+ * residual layers, then per block conv a, conv b, output mapping.  create is synchronous and allocates every buffer (about
+ * 1 GB at the paper's size); forward only enqueues kernels on `stream`.  Supported (else HR_ERR_UNSUPPORTED): width a multiple of
+ * 64 up to 256, n_res even, sr_ch[s] = 32 or a multiple of 64 up to 256. */
+typedef struct hr_gnet hr_gnet_t;
+typedef struct {
+  uint32_t h, w;                /* ray array ("downsampled pixel array"); the output image is 8h x 8w */
+  uint32_t width, n_res;        /* 256, 28 */
+  uint32_t sr_ch[3];            /* 128, 64, 32 */
+  float rough_min;              /* 0.09 */
+} hr_gnet_config;
+int hashrender_gbuffer_create(const hr_gnet_config* cfg, const float* weights, uint64_t n_weights, hr_gnet_t** out);
+int hashrender_gbuffer_destroy(hr_gnet_t* h);
+/* rays: DEVICE [h][w][6].  Outputs (DEVICE, each nullable, N = 64 h w pixels in row-major image order): x [N,3], brdf [N,7] = n a r
+ * (post-activation: hr_frame.x / hr_frame.brdf), mask [N] (hr_frame.mask), raw [N,11] (the network's outputs before the maps). */
+int hashrender_gbuffer_forward(hr_gnet_t* h, const float* rays, float* x, float* brdf, uint8_t* mask, float* raw, void* stream);
+/* kernels launched so far; algorithmic flops of one forward (2 N Cout Cin k^2 per convolution, one pass, padding not counted) */
+uint64_t hashrender_gbuffer_launch_count(const hr_gnet_t* h);
+double hashrender_gbuffer_flops(const hr_gnet_t* h);
+const char* hashrender_gbuffer_last_error(const hr_gnet_t* h);
+
 #ifdef __cplusplus
 }
 #endif

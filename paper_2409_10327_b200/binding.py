@@ -16,7 +16,9 @@ _LIB_PATH = os.path.join(os.path.dirname(os.path.abspath(__file__)), "libhashren
 
 EXPORTS = ["hashrender_create", "hashrender_destroy", "hashrender_set_env", "hashrender_encode", "hashrender_decode",
            "hashrender_trace", "hashrender_shade", "hashrender_render_frame", "hashrender_render_frame_host",
-           "hashrender_sample_mis", "hashrender_sample_stratified", "hashrender_denoise", "hashrender_stats", "hashrender_launch_count", "hashrender_last_path", "hashrender_last_error"]
+           "hashrender_sample_mis", "hashrender_sample_stratified", "hashrender_denoise", "hashrender_stats", "hashrender_launch_count", "hashrender_last_path", "hashrender_last_error",
+           "hashrender_gbuffer_create", "hashrender_gbuffer_destroy", "hashrender_gbuffer_forward", "hashrender_gbuffer_launch_count",
+           "hashrender_gbuffer_flops", "hashrender_gbuffer_last_error"]
 
 
 class HashRenderError(RuntimeError):
@@ -41,6 +43,11 @@ class hr_denoise(C.Structure):
     _fields_ = [("H", C.c_uint32), ("W", C.c_uint32), ("rgb", C.c_void_p), ("albedo", C.c_void_p), ("normal", C.c_void_p),
                 ("pos", C.c_void_p), ("cam", C.c_float * 3), ("mask", C.c_void_p), ("iterations", C.c_uint32),
                 ("sigma_z", C.c_float), ("sigma_n", C.c_float), ("sigma_l", C.c_float)]
+
+
+class hr_gnet_config(C.Structure):
+    _fields_ = [("h", C.c_uint32), ("w", C.c_uint32), ("width", C.c_uint32), ("n_res", C.c_uint32), ("sr_ch", C.c_uint32 * 3),
+                ("rough_min", C.c_float)]
 
 
 class hr_frame(C.Structure):
@@ -80,8 +87,19 @@ def load_library(path: str | None = None):
         lib.hashrender_last_path.restype = C.c_char_p
         lib.hashrender_last_error.argtypes = [vp]
         lib.hashrender_last_error.restype = C.c_char_p
+        lib.hashrender_gbuffer_create.argtypes = [C.POINTER(hr_gnet_config), vp, u64, C.POINTER(vp)]
+        lib.hashrender_gbuffer_destroy.argtypes = [vp]
+        lib.hashrender_gbuffer_forward.argtypes = [vp, vp, vp, vp, vp, vp, vp]
+        lib.hashrender_gbuffer_launch_count.argtypes = [vp]
+        lib.hashrender_gbuffer_launch_count.restype = u64
+        lib.hashrender_gbuffer_flops.argtypes = [vp]
+        lib.hashrender_gbuffer_flops.restype = C.c_double
+        lib.hashrender_gbuffer_last_error.argtypes = [vp]
+        lib.hashrender_gbuffer_last_error.restype = C.c_char_p
+        special = ("hashrender_launch_count", "hashrender_last_path", "hashrender_last_error", "hashrender_gbuffer_launch_count",
+                   "hashrender_gbuffer_flops", "hashrender_gbuffer_last_error")
         for name in EXPORTS:
-            if name not in ("hashrender_launch_count", "hashrender_last_path", "hashrender_last_error"):
+            if name not in special:
                 getattr(lib, name).restype = C.c_int
         _lib = lib
     return _lib
@@ -268,3 +286,44 @@ class HashRenderer:
 
     def last_path(self) -> str:
         return self._lib.hashrender_last_path(self._h).decode()
+
+
+class GBufferNet:
+    """Owns one hr_gnet_t handle: the CNN direct renderer G (hashrender_gbuffer_*).  forward() fills the arrays hr_frame takes."""
+
+    def __init__(self, weights, h, w, width=256, n_res=28, sr_ch=(128, 64, 32), rough_min=0.09):
+        self._lib = load_library()
+        weights = np.ascontiguousarray(weights, dtype=np.float32)
+        self.cfg = hr_gnet_config(h=h, w=w, width=width, n_res=n_res, sr_ch=(C.c_uint32 * 3)(*sr_ch), rough_min=rough_min)
+        self.h, self.w, self.N = h, w, 64 * h * w
+        self._h = C.c_void_p()
+        rc = self._lib.hashrender_gbuffer_create(C.byref(self.cfg), _ptr(weights), weights.size, C.byref(self._h))
+        if rc != 0:
+            msg = self._lib.hashrender_gbuffer_last_error(self._h).decode() if self._h else "create failed"
+            if self._h:
+                self._lib.hashrender_gbuffer_destroy(self._h)
+                self._h = C.c_void_p()
+            raise HashRenderError(rc, msg)
+
+    def forward(self, rays, x=None, brdf=None, mask=None, raw=None, stream=None):
+        rc = self._lib.hashrender_gbuffer_forward(self._h, _arg(rays, "rays"), _arg(x, "x"), _arg(brdf, "brdf"), _arg(mask, "mask", "u8", align=1),
+                                                  _arg(raw, "raw"), stream)
+        if rc != 0:
+            raise HashRenderError(rc, self._lib.hashrender_gbuffer_last_error(self._h).decode())
+
+    def launch_count(self) -> int:
+        return int(self._lib.hashrender_gbuffer_launch_count(self._h))
+
+    def flops(self) -> float:
+        return float(self._lib.hashrender_gbuffer_flops(self._h))
+
+    def destroy(self):
+        if getattr(self, "_h", None):
+            self._lib.hashrender_gbuffer_destroy(self._h)
+            self._h = C.c_void_p()
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass

@@ -9,7 +9,7 @@ from concurrent.futures import ThreadPoolExecutor
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(_HERE, "csrc")
-SOURCES = ["hashrender.cu", "hr_wg_p0.cu", "hr_wg_p1.cu"]
+SOURCES = ["hashrender.cu", "hr_wg_p0.cu", "hr_wg_p1.cu", "hr_gnet.cu"]
 LIB = os.path.join(_HERE, "libhashrender.so")
 OBJDIR = os.path.join(_HERE, "build")
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "-Xcompiler", "-fPIC",
