@@ -274,6 +274,89 @@ def run_c4_sweep(args):
                       "hbm_peak_GBps": peaks["hbm"], "clocks": hb["clocks"], "gpu_launches": args.steps, "roofline": hb["roofline"], "sweep": rows}))
 
 
+def measure_gbuffer(steps, peaks, clock_index=None, cpu_rays=40):
+    """The step before the path: one forward pass of the CNN direct renderer G (hashrender_gbuffer_forward; PAPER.md:68, 90-96,
+    134) at the paper's shape, 100 x 100 rays -> 800 x 800 maps of x, n, a, r, mask, random-init weights.  Reports ms / frame, the
+    algorithmic tensor rate (2 N Cout Cin k^2 per convolution, ONE pass: the second pass over the lo halves of the split
+    activations is this implementation's cost, not algorithmic work) against the measured bf16 peak, and the float64 oracle timed
+    beside it on a smaller ray array."""
+    import torch
+    from gen import gnet
+    from paper_2409_10327_b200 import GBufferNet
+    dev = torch.device("cuda", torch.cuda.current_device())
+    blob = gnet.make_gnet(7)
+    rays_h = gnet.make_rays(7, 100, 100)
+    net = GBufferNet(blob, 100, 100)
+    rays = torch.from_numpy(rays_h).to(dev)
+    N = net.N
+    x = torch.empty((N, 3), device=dev); brdf = torch.empty((N, 7), device=dev); mask = torch.empty((N,), device=dev, dtype=torch.uint8)
+    stream = torch.cuda.current_stream().cuda_stream
+    clocks = ClockSampler(clock_index) if clock_index is not None else None
+    if clocks:
+        clocks.start()
+    for _ in range(3):
+        net.forward(rays, x, brdf, mask, stream=stream)
+    torch.cuda.synchronize()
+    l0 = net.launch_count()
+    if clocks:
+        clocks.begin()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(steps):
+        net.forward(rays, x, brdf, mask, stream=stream)
+    e1.record(); torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / steps
+    launches = (net.launch_count() - l0) // steps
+    clk = None
+    if clocks:
+        clocks.end()
+        if len(clocks.in_window()) < 8:
+            t_end = time.time() + 1.0
+            while time.time() < t_end:
+                for _ in range(8):
+                    net.forward(rays, x, brdf, mask, stream=stream)
+                torch.cuda.synchronize()
+            clocks.end("timed region + 1 s untimed continuation of the same launches")
+        clk = clocks.stop()
+    # end to end: the ray map travels host -> device, the maps come back
+    hr_ = torch.from_numpy(rays_h).pin_memory()
+    hx = torch.empty((N, 3)).pin_memory(); hb = torch.empty((N, 7)).pin_memory()
+    def e2e():
+        rd = hr_.to(dev, non_blocking=True)
+        net.forward(rd, x, brdf, mask, stream=stream)
+        hx.copy_(x, non_blocking=True); hb.copy_(brdf, non_blocking=True)
+        torch.cuda.synchronize()
+    e2e()
+    e0.record()
+    for _ in range(3):
+        e2e()
+    e1.record(); torch.cuda.synchronize()
+    e2e_ms = e0.elapsed_time(e1) / 3
+    flops = net.flops()
+    ach = flops / (ms * 1e-3) / 1e12
+    rec = ncu_record("G:k_gconv") or {}
+    out = {"workload": "G: CNN direct renderer forward, 100x100 rays -> 800x800 maps (width 256, 28 residual layers, SR blocks 128/64/32; "
+                       "PAPER.md:134), random-init weights", "ms_per_frame": ms, "kernels_per_frame": launches, "finite": bool(torch.isfinite(x).all()),
+           "e2e_ms_per_frame": e2e_ms, "h2d_bytes_per_step": int(rays_h.nbytes), "d2h_bytes_per_step": int(N * 40),
+           "paper_context": "Model Op. 4.3-5.8 ms on an A100 (PAPER.md:185-193, trained weights; context only)",
+           "roofline": {"bound": "tensor", "achieved": ach, "peak": peaks["tensor_sustained"], "unit": "TFLOP/s", "frac": ach / peaks["tensor_sustained"],
+                        "algorithmic_flops_per_frame": flops, "kernel": "k_gconv (35 launches per frame) + element-wise stages",
+                        "traffic": rec.get("traffic"), "capture": rec.get("capture"),
+                        "peak_source": f"MEASURED_PEAKS.json bf16_tflops_sustained ({peaks['which']})",
+                        "note": "143 GFLOP per frame is 0.1 ms of tensor time: the pass is bound by the 77 dependent launches (every instance "
+                                "norm needs the whole image's statistics) and by the fp32 element-wise stages, not by the MMAs"},
+           "clocks": clk}
+    net.destroy()
+    # the oracle on a smaller ray array (cost is linear in the pixel count)
+    from oracle import gnet_oracle as G
+    t0 = time.perf_counter()
+    G.forward(blob, gnet.make_rays(7, cpu_rays, cpu_rays))
+    dt = time.perf_counter() - t0
+    out["cpu_baseline"] = {"value": dt * (100.0 / cpu_rays) ** 2 * 1e3, "unit": "ms/frame (extrapolated)", "kind": "oracle", "cores": os.cpu_count(),
+                           "sample": f"{cpu_rays}x{cpu_rays} rays -> {8 * cpu_rays}x{8 * cpu_rays} maps in {dt:.1f} s (numpy float64, BLAS threads)"}
+    return out
+
+
 def workload_name(cfg):
     ind = f" + {cfg.S_i} secondary x {cfg.S_2} tertiary (one-bounce indirect)" if cfg.flags & gen.HR_INDIRECT else ""
     return (f"{cfg.name}: 800x800 = {cfg.N} primary points, {cfg.S_d} direct directions{ind}; L={cfg.L} F={cfg.F} T=2^{cfg.log2_T} "
@@ -285,7 +368,7 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--workload", default="C2", choices=["C1", "C2", "C3", "C3a", "C4"])
+    ap.add_argument("--workload", default="C2", choices=["C1", "C2", "C3", "C3a", "C4", "G"])
     ap.add_argument("--full-sweep", action="store_true", help="C4: include 2^26 points")
     ap.add_argument("--c4-log2t", type=int, default=0, help="C4: only this table size (for profiling one point of the sweep)")
     ap.add_argument("--c4-n", type=int, default=0, help="C4: only this many points")
@@ -296,14 +379,26 @@ def main():
     ap.add_argument("--ref-pixels", type=int, default=256, help="pixels per step for --impl reference")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-cpu-all-cores", action="store_true", help="skip the all-host-cores oracle leg")
-    ap.add_argument("--also", default="C1,C3,C4", help="comma-separated workloads measured briefly and reported under `also` ('' = none); "
-                    "C4 = the T = 2^19 and T = 2^24 points of the sweep at 2^24 points")
+    ap.add_argument("--also", default="C1,C3,C4,G", help="comma-separated workloads measured briefly and reported under `also` ('' = none); "
+                    "C4 = the T = 2^19 and T = 2^24 points of the sweep at 2^24 points; G = the CNN direct renderer forward")
     ap.add_argument("--compact", action="store_true", help="headline with the default API flags (zero-weight secondary rays skipped) "
                     "instead of HR_DENSE")
     ap.add_argument("--no-extra", action="store_true", help="skip the `also` measurements")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 0)
-    cfg = gen.make_config(args.workload)
+    if args.workload == "G" and args.impl != "reference":
+        import torch
+        torch.cuda.set_device(0)
+        g = measure_gbuffer(args.steps, load_peaks(), clock_index=0)
+        print(json.dumps({"metric": "G forward ms/frame (100x100 rays -> 800x800 maps)", "value": g["ms_per_frame"], "unit": "ms", "n_gpus": 1,
+                          "steps": args.steps, "warmup": 3, "ms_per_step": g["ms_per_frame"], "higher_is_better": False, "scaling": "weak",
+                          "vs_baseline": None, "dtype": "f16x2 (fp16 hi+lo split activations, fp32 accumulate)", "data": "synthetic",
+                          "config": {"workload": g["workload"]}, "clocks": g["clocks"], "gpu_launches": g["kernels_per_frame"] * args.steps,
+                          "roofline": g["roofline"], "cpu_baseline": g["cpu_baseline"],
+                          "e2e": {"value": g["e2e_ms_per_frame"], "unit": "ms", "h2d_bytes_per_step": g["h2d_bytes_per_step"],
+                                  "d2h_bytes_per_step": g["d2h_bytes_per_step"]}}))
+        return
+    cfg = gen.make_config("C2" if args.workload == "G" else args.workload)
     if args.impl == "reference":
         return run_reference(args, gen.make_config("C2") if args.workload == "C4" else cfg)
     if args.workload == "C4":
@@ -552,6 +647,8 @@ def main():
                                  "executed_queries_per_s": executed_queries(c2, r2["evaluated"]) / (ms2 * 1e-3), "path": r2["path"],
                                  "mean_rgb": r2["mean_rgb"], "achieved_tflops": rf["achieved"], "roofline_frac": rf["frac"],
                                  "roofline_peak": rf["peak"], "roofline": rf, "clocks": r2["clk"]})
+        if "G" in args.also.split(","):
+            line["gbuffer"] = measure_gbuffer(max(args.steps, 5), peaks, clock_index=local)
         if "C4" in args.also.split(","):
             for log2_T in (19, 24):
                 for row in measure_c4(log2_T, [1 << 24], max(args.steps // 2, 3), args.vis_mode, peaks, clock_index=local):

@@ -201,7 +201,7 @@ const char* hashrender_last_error(const hashrender_t* h);
  * 64 up to 256, n_res even, sr_ch[s] = 32 or a multiple of 64 up to 256. */
 typedef struct hr_gnet hr_gnet_t;
 typedef struct {
-  uint32_t h, w;                /* ray array ("downsampled pixel array"); the output image is 8h x 8w */
+  uint32_t h, w;                /* ray array ("downsampled pixel array"), h w <= 65536; the output image is 8h x 8w */
   uint32_t width, n_res;        /* 256, 28 */
   uint32_t sr_ch[3];            /* 128, 64, 32 */
   float rough_min;              /* 0.09 */

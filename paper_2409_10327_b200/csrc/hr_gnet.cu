@@ -132,7 +132,7 @@ int hashrender_gbuffer_create(const hr_gnet_config* cfg, const float* weights, u
   *out = h;
   h->cfg = *cfg;
   const int width = (int)cfg->width, n_res = (int)cfg->n_res;
-  if (cfg->h < 1 || cfg->w < 1 || cfg->h > 4096 || cfg->w > 4096) return gfail(h, HR_ERR_INVALID_ARG, "gbuffer: bad ray-array size");
+  if (cfg->h < 1 || cfg->w < 1 || (uint64_t)cfg->h * cfg->w > (1u << 16)) return gfail(h, HR_ERR_INVALID_ARG, "gbuffer: ray array must hold 1 .. 65536 rays");
   if (width % 64 || width < 64 || width > 256 || n_res % 2 || n_res < 0 || n_res > 256)
     return gfail(h, HR_ERR_UNSUPPORTED, "gbuffer: need width in {64,128,192,256} and an even number of residual layers");
   for (int s = 0; s < 3; ++s)

@@ -190,7 +190,11 @@ __global__ void __launch_bounds__(192, 1)
         wait_ld();
         float v[32], w[32];
 #pragma unroll
-        for (int j = 0; j < 32; ++j) v[j] = __uint_as_float(r[j]) + __ldg(p.bias + c0 + j);
+        for (int j = 0; j < 8; ++j) {
+          const float4 b4 = __ldg(reinterpret_cast<const float4*>(p.bias + c0) + j);
+          v[4 * j] = __uint_as_float(r[4 * j]) + b4.x; v[4 * j + 1] = __uint_as_float(r[4 * j + 1]) + b4.y;
+          v[4 * j + 2] = __uint_as_float(r[4 * j + 2]) + b4.z; v[4 * j + 3] = __uint_as_float(r[4 * j + 3]) + b4.w;
+        }
         if (valid) {
           float4* o = reinterpret_cast<float4*>(p.pre + pix * p.Cout + c0);
 #pragma unroll
@@ -252,11 +256,14 @@ __global__ void __launch_bounds__(256) k_gnorm(NormP p) {
     s_ab[p.C + c] = (float)((double)p.beta[c] - m * a);
   }
   __syncthreads();
-  const int groups = p.C / 8;
-  const long long total = p.N * groups;
-  for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < total; i += (long long)gridDim.x * blockDim.x) {
-    const long long pix = i / groups;
-    const int c0 = (int)(i - pix * groups) * 8;
+  // 32-bit index arithmetic (the host refuses images with 2^31 or more (pixel, 8-channel) groups): 64-bit divisions cost more
+  // than the GELU
+  const uint32_t groups = (uint32_t)p.C / 8u;
+  const uint32_t total = (uint32_t)p.N * groups;
+  for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < total; i += gridDim.x * blockDim.x) {
+    const uint32_t pixu = i / groups;
+    const long long pix = pixu;
+    const int c0 = (int)(i - pixu * groups) * 8;
     const float4 x0 = *reinterpret_cast<const float4*>(p.pre + pix * p.C + c0), x1 = *reinterpret_cast<const float4*>(p.pre + pix * p.C + c0 + 4);
     float v[8] = {x0.x, x0.y, x0.z, x0.w, x1.x, x1.y, x1.z, x1.w};
 #pragma unroll
@@ -278,7 +285,7 @@ __global__ void __launch_bounds__(256) k_gnorm(NormP p) {
 #pragma unroll
     for (int j = 0; j < 8; ++j) split16(v[j], hi[j], lo[j]);
     long long row = pix;
-    if (p.mode == 4) { const long long y = pix / p.W, x = pix - y * p.W; row = (y + 1) * (p.W + 2) + x + 1; }
+    if (p.mode == 4) { const uint32_t y = pixu / (uint32_t)p.W, x = pixu - y * (uint32_t)p.W; row = (long long)(y + 1) * (p.W + 2) + x + 1; }
     __half* o = p.act + row * (2 * p.C) + c0;
     *reinterpret_cast<uint4*>(o) = *reinterpret_cast<const uint4*>(hi);
     *reinterpret_cast<uint4*>(o + p.C) = *reinterpret_cast<const uint4*>(lo);
@@ -302,12 +309,12 @@ __device__ __forceinline__ void up_taps(int j, int n, int& i0, int& i1, float& f
   i0 = (int)s; i1 = min(i0 + 1, n - 1); f = s - (float)i0;
 }
 __global__ void __launch_bounds__(256) k_gupsample(const float* __restrict__ in, __half* __restrict__ act, int h, int w, int C) {
-  const int H = 2 * h, W = 2 * w, groups = C / 8;
-  const long long total = (long long)H * W * groups;
-  for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < total; i += (long long)gridDim.x * blockDim.x) {
-    const long long pix = i / groups;
+  const int H = 2 * h, W = 2 * w;
+  const uint32_t groups = (uint32_t)C / 8u, total = (uint32_t)H * (uint32_t)W * groups;
+  for (uint32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < total; i += gridDim.x * blockDim.x) {
+    const uint32_t pix = i / groups;
     const int c0 = (int)(i - pix * groups) * 8;
-    const int y = (int)(pix / W), x = (int)(pix - (long long)y * W);
+    const int y = (int)(pix / (uint32_t)W), x = (int)(pix - (uint32_t)y * (uint32_t)W);
     int y0, y1, x0, x1; float fy, fx;
     up_taps(y, h, y0, y1, fy); up_taps(x, w, x0, x1, fx);
     const float* p00 = in + ((long long)y0 * w + x0) * C + c0; const float* p01 = in + ((long long)y0 * w + x1) * C + c0;
@@ -340,12 +347,12 @@ __global__ void __launch_bounds__(128) k_gmap(MapP p) {
   extern __shared__ float s_w[];                          // [11][C] + [11]
   for (int i = threadIdx.x; i < kOutCh * p.C + kOutCh; i += blockDim.x) s_w[i] = i < kOutCh * p.C ? p.Wm[i] : p.bm[i - kOutCh * p.C];
   __syncthreads();
-  const long long N = (long long)p.H * p.W;
-  for (long long pix = blockIdx.x * (long long)blockDim.x + threadIdx.x; pix < N; pix += (long long)gridDim.x * blockDim.x) {
+  const uint32_t N = (uint32_t)p.H * (uint32_t)p.W;
+  for (uint32_t pix = blockIdx.x * blockDim.x + threadIdx.x; pix < N; pix += gridDim.x * blockDim.x) {
     float o[kOutCh];
 #pragma unroll
     for (int k = 0; k < kOutCh; ++k) o[k] = s_w[kOutCh * p.C + k];
-    const float4* f = reinterpret_cast<const float4*>(p.feat + pix * p.C);
+    const float4* f = reinterpret_cast<const float4*>(p.feat + (size_t)pix * p.C);
     for (int c = 0; c < p.C / 4; ++c) {
       const float4 v = f[c];
 #pragma unroll
@@ -355,7 +362,7 @@ __global__ void __launch_bounds__(128) k_gmap(MapP p) {
       }
     }
     if (p.prev) {
-      const int y = (int)(pix / p.W), x = (int)(pix - (long long)y * p.W), h = p.H / 2, w = p.W / 2;
+      const int y = (int)(pix / (uint32_t)p.W), x = (int)(pix - (uint32_t)y * (uint32_t)p.W), h = p.H / 2, w = p.W / 2;
       int y0, y1, x0, x1; float fy, fx;
       up_taps(y, h, y0, y1, fy); up_taps(x, w, x0, x1, fx);
       const float* p00 = p.prev + ((long long)y0 * w + x0) * kOutCh; const float* p01 = p.prev + ((long long)y0 * w + x1) * kOutCh;
@@ -368,16 +375,16 @@ __global__ void __launch_bounds__(128) k_gmap(MapP p) {
     }
     if (p.out) {
 #pragma unroll
-      for (int k = 0; k < kOutCh; ++k) p.out[pix * kOutCh + k] = o[k];
+      for (int k = 0; k < kOutCh; ++k) p.out[(size_t)pix * kOutCh + k] = o[k];
     }
     if (p.brdf) {
       const float inv = 1.f / fmaxf(sqrtf(o[0] * o[0] + o[1] * o[1] + o[2] * o[2]), 1e-12f);
-      float* b = p.brdf + pix * 7;
+      float* b = p.brdf + (size_t)pix * 7;
       b[0] = o[0] * inv; b[1] = o[1] * inv; b[2] = o[2] * inv;
       b[3] = sigmoidf_(o[3]); b[4] = sigmoidf_(o[4]); b[5] = sigmoidf_(o[5]);
       b[6] = p.rough_min + (1.f - p.rough_min) * sigmoidf_(o[6]);
     }
-    if (p.x) { p.x[pix * 3] = sigmoidf_(o[7]); p.x[pix * 3 + 1] = sigmoidf_(o[8]); p.x[pix * 3 + 2] = sigmoidf_(o[9]); }
+    if (p.x) { float* xo = p.x + (size_t)pix * 3; xo[0] = sigmoidf_(o[7]); xo[1] = sigmoidf_(o[8]); xo[2] = sigmoidf_(o[9]); }
     if (p.mask) p.mask[pix] = o[10] > 0.f ? 1 : 0;
   }
 }
