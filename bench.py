@@ -259,6 +259,15 @@ def run_c4_sweep(args):
     import torch
     torch.cuda.set_device(0)
     peaks = load_peaks()
+    gran = None
+    if args.l2_fetch_granularity:
+        import ctypes
+        torch.zeros(1, device="cuda")
+        rt = ctypes.CDLL("libcudart.so.12")
+        rc = rt.cudaDeviceSetLimit(5, ctypes.c_size_t(args.l2_fetch_granularity))          # cudaLimitMaxL2FetchGranularity = 0x05
+        got = ctypes.c_size_t(0)
+        rt.cudaDeviceGetLimit(ctypes.byref(got), 5)
+        gran = {"requested": args.l2_fetch_granularity, "rc": rc, "in_effect": got.value}
     rows = []
     Ns = [1 << 20, 1 << 22, 1 << 24] + ([1 << 26] if args.full_sweep else [])
     if args.c4_n:
@@ -271,7 +280,7 @@ def run_c4_sweep(args):
                       "steps": args.steps, "warmup": 3, "ms_per_step": best["ms"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
                       "dtype": "f16", "data": "synthetic", "config": {"workload": "C4 sweep: uniform random points x 1 direction, fp16 L=16 F=2",
                       "points": "generated on device (torch Philox); parity of this call at every table size of the sweep: tests/test_gpu_parity.py::test_c4_sweep_full_size_sampled_points"},
-                      "hbm_peak_GBps": peaks["hbm"], "clocks": hb["clocks"], "gpu_launches": args.steps, "roofline": hb["roofline"], "sweep": rows}))
+                      "l2_fetch_granularity": gran, "hbm_peak_GBps": peaks["hbm"], "clocks": hb["clocks"], "gpu_launches": args.steps, "roofline": hb["roofline"], "sweep": rows}))
 
 
 def measure_gbuffer(steps, peaks, clock_index=None, cpu_rays=40):
@@ -372,6 +381,8 @@ def main():
     ap.add_argument("--full-sweep", action="store_true", help="C4: include 2^26 points")
     ap.add_argument("--c4-log2t", type=int, default=0, help="C4: only this table size (for profiling one point of the sweep)")
     ap.add_argument("--c4-n", type=int, default=0, help="C4: only this many points")
+    ap.add_argument("--l2-fetch-granularity", type=int, default=0, help="probe: cudaDeviceSetLimit(cudaLimitMaxL2FetchGranularity, n) in this "
+                    "process before the measurement (32 / 64 / 128 bytes; 0 = leave the driver default)")
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--vis-mode", type=int, default=1, help="1 = hard visibility (paper-faithful), 0 = soft")
     ap.add_argument("--e2e-steps", type=int, default=3)

@@ -176,34 +176,70 @@ int hashrender_create(const hr_config* cfg, const float* tables, const float* br
   HR_CUDA(h, cudaGetDevice(&dev));
   HR_CUDA(h, cudaDeviceGetAttribute(&h->num_sms, cudaDevAttrMultiProcessorCount, dev));
 
-  // grid parameters
+  // grid parameters + the device layout of the tables (hr_device.cuh GridP): hashed levels keep their T rows; a dense level is stored
+  // with power-of-two strides (row = cx | cy << b | cz << 2b), so one XOR index path serves every level
   GridP& g = h->grid;
   g.L = cfg->L; g.log2_T = cfg->log2_T; g.f16 = cfg->table_dtype; g.dense_mask = 0;
-  for (uint32_t l = 0; l < kMaxL; ++l) g.res[l] = l < cfg->L ? cfg->res[l] : 1;
+  const uint64_t T = 1ull << cfg->log2_T;
+  const size_t esz = cfg->table_dtype == HR_F32 ? 8 : 4;               // bytes per row (F = 2)
+  uint64_t rows_total = 0, lvl_rows[kMaxL], lvl_bits[kMaxL];
+  for (uint32_t l = 0; l < kMaxL; ++l) { g.res[l] = 1; g.pa[l] = g.pb[l] = g.pmask[l] = 0; g.off[l] = 0; lvl_rows[l] = 0; lvl_bits[l] = 0; }
   for (uint32_t l = 0; l < cfg->L; ++l) {
-    const uint64_t s = (uint64_t)cfg->res[l] + 1;
-    if (s * s * s <= (1ull << cfg->log2_T)) g.dense_mask |= 1u << l;
+    g.res[l] = cfg->res[l];
+    const uint64_t sN = (uint64_t)cfg->res[l] + 1;
+    if (sN * sN * sN <= T) {
+      g.dense_mask |= 1u << l;
+      uint32_t bx = 1;
+      while ((1ull << bx) < sN) ++bx;
+      lvl_bits[l] = bx;
+      g.pa[l] = 1u << bx; g.pb[l] = 1u << (2 * bx); g.pmask[l] = 0xFFFFFFFFu;
+      lvl_rows[l] = sN << (2 * bx);                                   // z-slabs 0 .. N
+    } else {
+      g.pa[l] = 2654435761u; g.pb[l] = 805459861u; g.pmask[l] = (uint32_t)(T - 1);
+      lvl_rows[l] = T;
+    }
+    g.off[l] = rows_total * esz;
+    rows_total += (lvl_rows[l] + 3) & ~3ull;                          // keep every level 16-byte aligned
   }
-  // tables: fp32 host -> device float2 / half2
-  const size_t n = (size_t)cfg->L << cfg->log2_T << 1;
-  if (cfg->table_dtype == HR_F32) {
-    HR_CUDA(h, cudaMalloc(&h->d_tables, n * sizeof(float)));
-    HR_CUDA(h, cudaMemcpy(h->d_tables, tables, n * sizeof(float), cudaMemcpyHostToDevice));
-  } else {
-    HR_CUDA(h, cudaMalloc(&h->d_tables, n * sizeof(__half)));
-    const size_t chunk = (size_t)16 << 20;
+  const uint64_t zero_off = rows_total * esz;
+  rows_total += 8;                                                    // zero rows for the null levels l >= L
+  for (uint32_t l = cfg->L; l < kMaxL; ++l) g.off[l] = zero_off;
+  HR_CUDA(h, cudaMalloc(&h->d_tables, rows_total * esz));
+  HR_CUDA(h, cudaMemset(h->d_tables, 0, rows_total * esz));
+  const size_t n = (size_t)cfg->L << cfg->log2_T << 1;                  // floats in the caller's [L][T][2] array
+  {
+    const size_t chunk = (size_t)16 << 20;                            // floats per staged piece (fp16 tables are converted on the device)
     float* st = nullptr;
-    HR_CUDA(h, cudaMalloc(&st, chunk * sizeof(float)));
-    for (size_t o = 0; o < n; o += chunk) {
-      const size_t m = n - o < chunk ? n - o : chunk;
-      cudaError_t e = cudaMemcpy(st, tables + o, m * sizeof(float), cudaMemcpyHostToDevice);
-      if (e == cudaSuccess) {
-        k_f32_to_f16<<<h->num_sms * 8, 256>>>(st, reinterpret_cast<__half*>(h->d_tables) + o, m);
-        e = cudaDeviceSynchronize();
+    if (cfg->table_dtype == HR_F16) HR_CUDA(h, cudaMalloc(&st, chunk * sizeof(float)));
+    std::vector<float> relaid;
+    cudaError_t e = cudaSuccess;
+    for (uint32_t l = 0; l < cfg->L && e == cudaSuccess; ++l) {
+      const float* src = tables + ((size_t)l << cfg->log2_T) * 2;
+      if ((g.dense_mask >> l) & 1u) {                                 // vertex (x, y, z): row x + y s + z s^2 -> row x | y << b | z << 2b
+        const uint64_t sN = (uint64_t)cfg->res[l] + 1, bx = lvl_bits[l];
+        relaid.assign(lvl_rows[l] * 2, 0.f);
+        for (uint64_t z = 0; z < sN; ++z)
+          for (uint64_t y = 0; y < sN; ++y)
+            memcpy(&relaid[((z << (2 * bx)) | (y << bx)) * 2], src + (y * sN + z * sN * sN) * 2, sN * 2 * sizeof(float));
+        src = relaid.data();
       }
-      if (e != cudaSuccess) { cudaFree(st); return fail(h, HR_ERR_CUDA, "table conversion failed: %s", cudaGetErrorString(e)); }
+      const size_t nf = lvl_rows[l] * 2;
+      char* dst = reinterpret_cast<char*>(h->d_tables) + g.off[l];
+      if (cfg->table_dtype == HR_F32) {
+        e = cudaMemcpy(dst, src, nf * sizeof(float), cudaMemcpyHostToDevice);
+      } else {
+        for (size_t o = 0; o < nf && e == cudaSuccess; o += chunk) {
+          const size_t m = nf - o < chunk ? nf - o : chunk;
+          e = cudaMemcpy(st, src + o, m * sizeof(float), cudaMemcpyHostToDevice);
+          if (e == cudaSuccess) {
+            k_f32_to_f16<<<h->num_sms * 8, 256>>>(st, reinterpret_cast<__half*>(dst) + o, m);
+            e = cudaDeviceSynchronize();
+          }
+        }
+      }
     }
     cudaFree(st);
+    if (e != cudaSuccess) return fail(h, HR_ERR_CUDA, "table upload failed: %s", cudaGetErrorString(e));
   }
   g.tables = h->d_tables;
   // weights

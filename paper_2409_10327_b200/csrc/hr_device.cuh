@@ -12,10 +12,20 @@ constexpr int kMaxL = 16;   // levels
 constexpr int kD = 32;      // padded feature width (L*F <= 32, F == 2)
 constexpr int kH = 64;      // hidden width
 
+// Device layout of the tables (hashrender_create re-lays them out once): level l starts `off[l]` bytes into `tables` and the row of
+// grid vertex (cx, cy, cz) is  (cx ^ cy * pa[l] ^ cz * pb[l]) & pmask[l]  for EVERY level.  Hashed levels: pa, pb = the primes of
+// [14], pmask = T - 1, T rows (Q1).  Dense levels: the vertex index is stored with power-of-two strides, pa = 2^b, pb = 2^2b,
+// b = ceil(log2(N + 1)), pmask = ~0: the three terms occupy disjoint bits, so the XOR is the sum cx + cy 2^b + cz 2^2b.  One branch-free
+// index path serves both kinds, and the two x-neighbours of a cell are ADJACENT rows whenever cx is even (bit 0 of the row is
+// bit 0 of cx), so one aligned two-row load brings both (gather8).  The index the ABI exports (hashrender_encode) is still the
+// specified one, x + y (N+1) + z (N+1)^2 or the hash (corner_indices).  Levels l >= L are null: res 1, pa = pb = pmask = 0, off = a
+// block of zero rows.
 struct GridP {
   uint32_t L, log2_T, dense_mask, f16;
   uint32_t res[kMaxL];
-  const void* tables;       // [L][T] of float2 (f16 == 0) or __half2 (f16 == 1)
+  uint32_t pa[kMaxL], pb[kMaxL], pmask[kMaxL];
+  unsigned long long off[kMaxL];
+  const void* tables;       // rows of float2 (f16 == 0) or __half2 (f16 == 1)
 };
 struct EnvP { const float* env; uint32_t He, We; };
 struct ShadeP {
@@ -89,25 +99,49 @@ __device__ __forceinline__ void corner_indices(const Cell& c, uint32_t N, bool d
   }
 }
 
-// Gather of one table row: address = level base + idx * row bytes in ONE integer multiply-add (mad.wide.u32), read-only path.
-__device__ __forceinline__ __half2 gather_h2(const void* level_base, uint32_t idx) {
-  uint32_t v;
-  asm("{\n\t.reg .u64 a;\n\tmad.wide.u32 a, %1, 4, %2;\n\tld.global.nc.b32 %0, [a];\n\t}" : "=r"(v) : "r"(idx), "l"(level_base));
-  return *reinterpret_cast<__half2*>(&v);
+// a3: the 8 corner rows of one level, corner number b0 + 2 b1 + 4 b2 (Q9): one index path for dense and hashed levels, eight
+// independent one-row loads (address = level base + row * row bytes in one mad.wide.u32, read-only path).
+// Measured and not kept: fetching the x-neighbour pair with ONE aligned two-row load (the rows of cx and cx + 1 are adjacent
+// whenever cx is even; a predicated one-row load covers odd cx) -- 6 instead of 8 line requests per level, bit-identical values --
+// was slower everywhere (C2 23.3 -> 25.4 ms, C3 16.7 -> 17.6 ms, C4 at T = 2^19 6.0 -> 6.4 ms, at T = 2^24 13.5 -> 15.2 ms): the
+// selects and predication cost more issue slots than the saved L1 requests give back.
+__device__ __forceinline__ void corner_rows(const GridP& g, int l, const uint32_t (&c0)[3], uint32_t (&i0)[4], uint32_t (&i1)[4]) {
+  const uint32_t pa = g.pa[l], pb = g.pb[l], pm = g.pmask[l];
+  const uint32_t hy0 = c0[1] * pa, hy1 = hy0 + pa, hz0 = c0[2] * pb, hz1 = hz0 + pb;
+  const uint32_t h[4] = {hy0 ^ hz0, hy1 ^ hz0, hy0 ^ hz1, hy1 ^ hz1};
+#pragma unroll
+  for (int j = 0; j < 4; ++j) { i0[j] = (c0[0] ^ h[j]) & pm; i1[j] = ((c0[0] + 1u) ^ h[j]) & pm; }
 }
-__device__ __forceinline__ float2 gather_f2(const void* level_base, uint32_t idx) {
-  float2 v;
-  asm("{\n\t.reg .u64 a;\n\tmad.wide.u32 a, %2, 8, %3;\n\tld.global.nc.v2.f32 {%0, %1}, [a];\n\t}" : "=f"(v.x), "=f"(v.y) : "r"(idx), "l"(level_base));
-  return v;
+__device__ __forceinline__ void gather8_h2(const GridP& g, int l, const uint32_t (&c0)[3], uint32_t (&v)[8]) {
+  uint32_t i0[4], i1[4];
+  corner_rows(g, l, c0, i0, i1);
+  const char* lb = reinterpret_cast<const char*>(g.tables) + g.off[l];
+#pragma unroll
+  for (int j = 0; j < 4; ++j) {
+    asm("{\n\t.reg .u64 p;\n\tmad.wide.u32 p, %1, 4, %2;\n\tld.global.nc.b32 %0, [p];\n\t}" : "=r"(v[2 * j]) : "r"(i0[j]), "l"(lb));
+    asm("{\n\t.reg .u64 p;\n\tmad.wide.u32 p, %1, 4, %2;\n\tld.global.nc.b32 %0, [p];\n\t}" : "=r"(v[2 * j + 1]) : "r"(i1[j]), "l"(lb));
+  }
+}
+__device__ __forceinline__ void gather8_f2(const GridP& g, int l, const uint32_t (&c0)[3], float2 (&v)[8]) {
+  uint32_t i0[4], i1[4];
+  corner_rows(g, l, c0, i0, i1);
+  const char* lb = reinterpret_cast<const char*>(g.tables) + g.off[l];
+#pragma unroll
+  for (int j = 0; j < 4; ++j) {
+    asm("{\n\t.reg .u64 p;\n\tmad.wide.u32 p, %2, 8, %3;\n\tld.global.nc.v2.f32 {%0, %1}, [p];\n\t}" : "=f"(v[2 * j].x), "=f"(v[2 * j].y) : "r"(i0[j]), "l"(lb));
+    asm("{\n\t.reg .u64 p;\n\tmad.wide.u32 p, %2, 8, %3;\n\tld.global.nc.v2.f32 {%0, %1}, [p];\n\t}" : "=f"(v[2 * j + 1].x), "=f"(v[2 * j + 1].y) : "r"(i1[j]), "l"(lb));
+  }
 }
 template <bool F16>
-__device__ __forceinline__ const void* level_base(const void* tables, uint32_t log2_T, int l) {
-  return reinterpret_cast<const char*>(tables) + (((size_t)l << log2_T) << (F16 ? 2 : 3));
-}
-template <bool F16>
-__device__ __forceinline__ float2 table_load(const void* lbase, uint32_t idx) {
-  if (F16) return __half22float2(gather_h2(lbase, idx));
-  return gather_f2(lbase, idx);
+__device__ __forceinline__ void gather8(const GridP& g, int l, const uint32_t (&c0)[3], float2 (&v)[8]) {
+  if constexpr (F16) {
+    uint32_t r[8];
+    gather8_h2(g, l, c0, r);
+#pragma unroll
+    for (int k = 0; k < 8; ++k) v[k] = __half22float2(*reinterpret_cast<const __half2*>(&r[k]));
+  } else {
+    gather8_f2(g, l, c0, v);
+  }
 }
 
 // a3/a4: gather 8 corners of one level and interpolate.  Corner number b0 + 2 b1 + 4 b2 (Q9).
@@ -116,13 +150,11 @@ __device__ __forceinline__ float2 encode_level(const GridP& g, int l, float x, f
                                                uint32_t* idx_out, float* w_out) {
   const uint32_t N = g.res[l];
   const Cell c = cell_of(N, x, y, z);
-  uint32_t idx[8];
-  corner_indices(c, N, (g.dense_mask >> l) & 1u, g.log2_T, idx);
   float2 v[8];
-  const void* lb = level_base<F16>(g.tables, g.log2_T, l);
-#pragma unroll
-  for (int k = 0; k < 8; ++k) v[k] = table_load<F16>(lb, idx[k]);
-  if (idx_out) {
+  gather8<F16>(g, l, c.c0, v);
+  if (idx_out) {                                              // the SPECIFIED index (Q1, Q3), not the device row
+    uint32_t idx[8];
+    corner_indices(c, N, (g.dense_mask >> l) & 1u, g.log2_T, idx);
 #pragma unroll
     for (int k = 0; k < 8; ++k) idx_out[k] = idx[k];
   }

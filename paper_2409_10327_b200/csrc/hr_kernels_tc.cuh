@@ -143,17 +143,15 @@ template <bool F16>
 __device__ __forceinline__ void gather_level(const GridP& g, int l, float x, float y, float z, LevelTaps<F16>& t) {
   const uint32_t N = g.res[l];
   const Cell cl = cell_of_clamped(N, x, y, z);                 // callers pass x' = sec_hit(...), already in [0,1]^3
-  uint32_t idx[8];
-  corner_indices(cl, N, (g.dense_mask >> l) & 1u, g.log2_T, idx);
-  const void* lb = level_base<F16>(g.tables, g.log2_T, l);
   if constexpr (F16) {
+    uint32_t r[8];
+    gather8_h2(g, l, cl.c0, r);
 #pragma unroll
-    for (int k = 0; k < 8; ++k) t.v[k] = gather_h2(lb, idx[k]);
+    for (int k = 0; k < 8; ++k) t.v[k] = *reinterpret_cast<const __half2*>(&r[k]);
 #pragma unroll
     for (int d = 0; d < 3; ++d) t.w[d] = __float2half2_rn(cl.w[d]);
   } else {
-#pragma unroll
-    for (int k = 0; k < 8; ++k) t.v[k] = gather_f2(lb, idx[k]);
+    gather8_f2(g, l, cl.c0, t.v);
 #pragma unroll
     for (int d = 0; d < 3; ++d) t.w[d] = cl.w[d];
   }

@@ -76,6 +76,7 @@ __device__ __forceinline__ void tmem_stN(uint32_t taddr, const uint32_t (&r)[4])
 __device__ __forceinline__ void tmem_stN(uint32_t taddr, const uint32_t (&r)[2]) {
   asm volatile("tcgen05.st.sync.aligned.32x32b.x2.b32 [%0], {%1,%2};" ::"r"(taddr), "r"(r[0]), "r"(r[1]) : "memory");
 }
+__device__ __forceinline__ void tmem_stN(uint32_t taddr, const uint32_t (&r)[1]) { tmem_st1(taddr, r[0]); }
 __device__ __forceinline__ void wg_sync(const WgCtx& c) { asm volatile("bar.sync %0, 128;" ::"r"(c.bar_id) : "memory"); }
 
 // One 128 x N layer of the WG: D = A W^T (+ bias K-step).  A = `ksteps` K-steps of fp16 at column a_col; split_a: a lo
@@ -327,14 +328,48 @@ __device__ __forceinline__ void load_D_h2(uint32_t tD, uint32_t (&Ph)[kH / 2]) {
   }
 }
 
-// f = H(x) in fp32 -> A columns 0..15 (hi) | 16..31 (lo)
+// One level of the fp32 encode in two halves, so that the caller can put a whole tertiary query between the gathers and
+// their first use (the arithmetic is encode_level's).
+template <bool F16TAB> struct Taps32;
+template <> struct Taps32<false> { float2 v[8]; float w[3]; __device__ __forceinline__ float2 tap(int k) const { return v[k]; } };
+template <> struct Taps32<true> {                          // fp16 rows stay packed (one register each) until they are interpolated
+  uint32_t r[8]; float w[3];
+  __device__ __forceinline__ float2 tap(int k) const { return __half22float2(*reinterpret_cast<const __half2*>(&r[k])); }
+};
+template <bool F16TAB>
+__device__ __forceinline__ void gather32(const GridP& g, int l, float x, float y, float z, Taps32<F16TAB>& t) {
+  const uint32_t N = g.res[l];
+  const Cell c = cell_of(N, x, y, z);
+  if constexpr (F16TAB) gather8_h2(g, l, c.c0, t.r); else gather8_f2(g, l, c.c0, t.v);
+  t.w[0] = c.w[0]; t.w[1] = c.w[1]; t.w[2] = c.w[2];
+}
+// trilinear interpolation of the taps: the arithmetic (and its order) is encode_level's
+template <bool F16TAB>
+__device__ __forceinline__ float2 lerp32(const Taps32<F16TAB>& t) {
+  const float wx[2] = {1.f - t.w[0], t.w[0]}, wy[2] = {1.f - t.w[1], t.w[1]}, wz[2] = {1.f - t.w[2], t.w[2]};
+  float2 f = make_float2(0.f, 0.f);
+#pragma unroll
+  for (int k = 0; k < 8; ++k) {
+    const float wt = wx[k & 1] * wy[(k >> 1) & 1] * wz[(k >> 2) & 1];
+    const float2 v = t.tap(k);
+    f.x = fmaf(wt, v.x, f.x);
+    f.y = fmaf(wt, v.y, f.y);
+  }
+  return f;
+}
+// f = H(x) in fp32 -> A columns 0..15 (hi) | 16..31 (lo), LIF levels per TMEM store
 template <bool F16TAB, int LIF>
 __device__ __forceinline__ void encode_split_to(uint32_t tA, const GridP& g, float x, float y, float z, float* scr = nullptr) {
 #pragma unroll 1
-  for (int l0 = 0; l0 < kMaxL; l0 += LIF) {               // LIF levels (8 LIF gathers) in flight
+  for (int l0 = 0; l0 < kMaxL; l0 += LIF) {
     uint32_t hi[LIF], lo[LIF];
 #pragma unroll
     for (int q = 0; q < LIF; ++q) {
+      // The branch is kept although null levels (GridP) would read zeros without it: it keeps each level's eight gathers
+      // and their interpolation in a block of their own.  Without it the compiler hoists all 8 LIF gathers of the group above the
+      // first use, and that burst is SLOWER (k_trace_wg, C4 at 2^24 points: T = 2^19 5.8 -> 7.5 ms, T = 2^24 13.5 -> 16.1 ms;
+      // written out as explicit gather / interpolate phases: 7.7 / 16.8 ms) -- L1 serves a warp's 32 divergent lines one per
+      // cycle, and 16 warps x 32 loads queue behind each other instead of overlapping with the interpolation of the others.
       hi[q] = 0u; lo[q] = 0u;
       if (l0 + q < (int)g.L) {
         const float2 v = encode_level<F16TAB>(g, l0 + q, x, y, z, nullptr, nullptr);
@@ -355,40 +390,18 @@ __device__ __forceinline__ void encode_fast_to(uint32_t tA, const GridP& g, floa
   for (int l0 = 0; l0 < kMaxL; l0 += LIF) {               // LIF levels (8 LIF gathers) in flight
     LevelTaps<F16TAB> t[LIF];
 #pragma unroll
-    for (int q = 0; q < LIF; ++q)
-      if (l0 + q < (int)g.L) gather_level<F16TAB>(g, l0 + q, x, y, z, t[q]);
+    for (int q = 0; q < LIF; ++q) gather_level<F16TAB>(g, l0 + q, x, y, z, t[q]);
     uint32_t f[LIF];
 #pragma unroll
-    for (int q = 0; q < LIF; ++q) f[q] = l0 + q < (int)g.L ? lerp_level(t[q]) : 0u;
+    for (int q = 0; q < LIF; ++q) f[q] = lerp_level(t[q]);
     tmem_stN(tA + l0, f);
   }
 }
 
-// One level of the fp32 encode in two halves, so that the caller can put a whole tertiary query between the gathers and
-// their first use (the arithmetic is encode_level's).
-template <bool F16TAB> struct Taps32 { float2 v[8]; float w[3]; };
-template <bool F16TAB>
-__device__ __forceinline__ void gather32(const GridP& g, int l, float x, float y, float z, Taps32<F16TAB>& t) {
-  const uint32_t N = g.res[l];
-  const Cell c = cell_of(N, x, y, z);
-  uint32_t idx[8];
-  corner_indices(c, N, (g.dense_mask >> l) & 1u, g.log2_T, idx);
-  const void* lb = level_base<F16TAB>(g.tables, g.log2_T, l);
-#pragma unroll
-  for (int k = 0; k < 8; ++k) t.v[k] = table_load<F16TAB>(lb, idx[k]);
-  t.w[0] = c.w[0]; t.w[1] = c.w[1]; t.w[2] = c.w[2];
-}
 // interpolate, split, store the level's fp16x2 words to TMEM columns tF + l (hi) and tF + 16 + l (lo)
 template <bool F16TAB>
 __device__ __forceinline__ void finish32(uint32_t tF, int l, const Taps32<F16TAB>& t) {
-  const float wx[2] = {1.f - t.w[0], t.w[0]}, wy[2] = {1.f - t.w[1], t.w[1]}, wz[2] = {1.f - t.w[2], t.w[2]};
-  float2 f = make_float2(0.f, 0.f);
-#pragma unroll
-  for (int k = 0; k < 8; ++k) {
-    const float wt = wx[k & 1] * wy[(k >> 1) & 1] * wz[(k >> 2) & 1];
-    f.x = fmaf(wt, t.v[k].x, f.x);
-    f.y = fmaf(wt, t.v[k].y, f.y);
-  }
+  const float2 f = lerp32(t);
   uint32_t hi, lo;
   split_pair(f.x, f.y, hi, lo);
   asm volatile("tcgen05.st.sync.aligned.32x32b.x1.b32 [%0], {%1};" ::"r"(tF + l), "r"(hi) : "memory");
@@ -470,7 +483,11 @@ __global__ void __launch_bounds__(kRows* G, 1)
 #ifdef HR_LIF
   constexpr int LIF = HR_LIF;
 #else
-  constexpr int LIF = G == 4 ? 2 : 4;               // register budget: 128 per thread at G = 4
+  // levels whose gathers are issued together in the encodes of this kernel.  One: a level's eight gathers, then its interpolation,
+  // then the next level.  Measured (C3 dense / compacted, C2 compacted, ms): LIF 1 15.65 / 7.61 / 10.87, LIF 2 (G = 4) and
+  // 4 (G = 3) 16.12 / 7.72 / 11.36, LIF 4 at G = 4 19.99 / 9.62: L1 serves a warp's 32 divergent lines one per cycle, so a
+  // burst of gathers from every warp queues up instead of overlapping with the other warps' arithmetic.
+  constexpr int LIF = 1;
 #endif
   using SP = SmemPlan<PREC, TSHARED, G>;
   extern __shared__ uint8_t smem_raw[];
@@ -604,17 +621,11 @@ __global__ void __launch_bounds__(kRows* G, 1)
       float3 L;
       Taps32<F16TAB> taps;                                            // PREC 1: fp32 taps; PREC 0: fp16x2 taps (only one survives)
       LevelTaps<F16TAB> htaps;
-      // levels l >= g.L do not exist (their table slice would lie past the allocation): no gather, zero features
+      // levels l >= g.L are null levels of the device layout (zero rows, GridP): they gather zeros, never past the allocation
       auto pre_gather = [&](int l) {
-        if (l >= (int)g.L) return;
         if constexpr (PREC == 1) gather32<F16TAB>(g, l, nx, ny, nz, taps); else gather_level<F16TAB>(g, l, nx, ny, nz, htaps);
       };
       auto pre_finish = [&](int l) {
-        if (l >= (int)g.L) {
-          tmem_st1(tF + l, 0u);
-          if constexpr (PREC == 1) tmem_st1(tF + 16 + l, 0u);
-          return;
-        }
         if constexpr (PREC == 1) finish32<F16TAB>(tF, l, taps);
         else tmem_st1(tF + l, lerp_level(htaps));
       };
@@ -792,6 +803,11 @@ __global__ void __launch_bounds__(kRows* G, 1)
 // x 32 outstanding loads per SM keep the gather pipeline full when the table spills from L2 to HBM.  t is an output, so the
 // fp32 epilogue is used (features hi/lo split for P, fp16 h1).
 constexpr int kTraceG = 4;
+#ifdef HR_TRACE_LIF
+constexpr int kTraceLIF = HR_TRACE_LIF;
+#else
+constexpr int kTraceLIF = 4;
+#endif
 template <int PREC> constexpr size_t trace_smem() {
   return 1024 + (size_t)kHiTileBytes * (PREC ? 2 : 1) + kOnesBytes + (size_t)kTraceG * kH * kRows * 4 + 8 * kMaxG + 16;
 }
@@ -872,7 +888,7 @@ __global__ void __launch_bounds__(kRows* kTraceG, 1)
     float px = 0.f, py = 0.f, pz = 0.f;
     if (x) { px = __ldg(x + 3 * i); py = __ldg(x + 3 * i + 1); pz = __ldg(x + 3 * i + 2); }
     if (feat) feat_split_to<4>(tA, g, feat + i * D);
-    else encode_split_to<F16TAB, 4>(tA, g, px, py, pz);
+    else encode_split_to<F16TAB, kTraceLIF>(tA, g, px, py, pz);
     issue_layer<PREC, G>(c, 0, 0, 2, true, 0, 2);                     // P = W1f f + b1, split-precision f
     wait_layer(c);
     store_D_f4(tD, Ps4);
