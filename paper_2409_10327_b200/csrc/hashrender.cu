@@ -204,6 +204,13 @@ int hashrender_create(const hr_config* cfg, const float* tables, const float* br
   const uint64_t zero_off = rows_total * esz;
   rows_total += 8;                                                    // zero rows for the null levels l >= L
   for (uint32_t l = cfg->L; l < kMaxL; ++l) g.off[l] = zero_off;
+  {
+    int l2 = 0;
+    HR_CUDA(h, cudaDeviceGetAttribute(&l2, cudaDevAttrL2CacheSize, dev));
+    uint64_t hashed = 0;
+    for (uint32_t l = 0; l < cfg->L; ++l) if (!((g.dense_mask >> l) & 1u)) hashed += lvl_rows[l] * esz;
+    g.l2_hint = hashed > 2ull * (uint64_t)l2 ? 1u : 0u;                // measured: helps at 448 MB of hashed levels, hurts at 128 MB (hr_device.cuh)
+  }
   HR_CUDA(h, cudaMalloc(&h->d_tables, rows_total * esz));
   HR_CUDA(h, cudaMemset(h->d_tables, 0, rows_total * esz));
   const size_t n = (size_t)cfg->L << cfg->log2_T << 1;                  // floats in the caller's [L][T][2] array

@@ -26,7 +26,21 @@ struct GridP {
   uint32_t pa[kMaxL], pb[kMaxL], pmask[kMaxL];
   unsigned long long off[kMaxL];
   const void* tables;       // rows of float2 (f16 == 0) or __half2 (f16 == 1)
+  uint32_t l2_hint;         // hashed levels > 2 x L2: their gathers carry an evict-first policy, dense levels evict-last (k_trace_wg)
 };
+// L2 eviction policies for tables far larger than the L2 (BASELINE configs[4], T = 2^24): the hashed levels are a random stream over
+// hundreds of MB that no cache can hold, the dense levels are ~70 MB that every point reads.  Hashed rows are fetched evict-first
+// and dense rows evict-last, so the stream does not push the dense levels out.  Measured with k_trace_wg at 2^24 points: T = 2^24
+// (448 MB of hashed levels) 13.5 -> 12.6 ms; evict-first alone 12.7, evict-last alone 13.4 (no effect); at T = 2^22 (128 MB of
+// hashed levels, about the size of the L2) the hint LOSES, 11.45 -> 12.15 ms, so it is applied only when the hashed levels exceed
+// twice the L2 (hashrender_create).
+struct L2Pol { unsigned long long first, last; };
+__device__ __forceinline__ L2Pol make_l2pol() {
+  L2Pol p;
+  asm("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p.first));
+  asm("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p.last));
+  return p;
+}
 struct EnvP { const float* env; uint32_t He, We; };
 struct ShadeP {
   float near_t, far_t, rough_min, f0;
@@ -122,6 +136,18 @@ __device__ __forceinline__ void gather8_h2(const GridP& g, int l, const uint32_t
     asm("{\n\t.reg .u64 p;\n\tmad.wide.u32 p, %1, 4, %2;\n\tld.global.nc.b32 %0, [p];\n\t}" : "=r"(v[2 * j + 1]) : "r"(i1[j]), "l"(lb));
   }
 }
+// the same with an L2 eviction policy per level (hashed: evict-first, dense: evict-last)
+__device__ __forceinline__ void gather8_h2_hint(const GridP& g, int l, const uint32_t (&c0)[3], uint32_t (&v)[8], const L2Pol& pol) {
+  uint32_t i0[4], i1[4];
+  corner_rows(g, l, c0, i0, i1);
+  const char* lb = reinterpret_cast<const char*>(g.tables) + g.off[l];
+  const unsigned long long cp = g.pmask[l] == 0xFFFFFFFFu ? pol.last : pol.first;
+#pragma unroll
+  for (int j = 0; j < 4; ++j) {
+    asm("{\n\t.reg .u64 p;\n\tmad.wide.u32 p, %1, 4, %2;\n\tld.global.nc.L2::cache_hint.b32 %0, [p], %3;\n\t}" : "=r"(v[2 * j]) : "r"(i0[j]), "l"(lb), "l"(cp));
+    asm("{\n\t.reg .u64 p;\n\tmad.wide.u32 p, %1, 4, %2;\n\tld.global.nc.L2::cache_hint.b32 %0, [p], %3;\n\t}" : "=r"(v[2 * j + 1]) : "r"(i1[j]), "l"(lb), "l"(cp));
+  }
+}
 __device__ __forceinline__ void gather8_f2(const GridP& g, int l, const uint32_t (&c0)[3], float2 (&v)[8]) {
   uint32_t i0[4], i1[4];
   corner_rows(g, l, c0, i0, i1);
@@ -147,11 +173,18 @@ __device__ __forceinline__ void gather8(const GridP& g, int l, const uint32_t (&
 // a3/a4: gather 8 corners of one level and interpolate.  Corner number b0 + 2 b1 + 4 b2 (Q9).
 template <bool F16>
 __device__ __forceinline__ float2 encode_level(const GridP& g, int l, float x, float y, float z,
-                                               uint32_t* idx_out, float* w_out) {
+                                               uint32_t* idx_out, float* w_out, const L2Pol* pol = nullptr) {
   const uint32_t N = g.res[l];
   const Cell c = cell_of(N, x, y, z);
   float2 v[8];
-  gather8<F16>(g, l, c.c0, v);
+  if (F16 && pol) {
+    uint32_t r[8];
+    gather8_h2_hint(g, l, c.c0, r, *pol);
+#pragma unroll
+    for (int k = 0; k < 8; ++k) v[k] = __half22float2(*reinterpret_cast<const __half2*>(&r[k]));
+  } else {
+    gather8<F16>(g, l, c.c0, v);
+  }
   if (idx_out) {                                              // the SPECIFIED index (Q1, Q3), not the device row
     uint32_t idx[8];
     corner_indices(c, N, (g.dense_mask >> l) & 1u, g.log2_T, idx);

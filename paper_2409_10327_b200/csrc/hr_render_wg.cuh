@@ -359,7 +359,8 @@ __device__ __forceinline__ float2 lerp32(const Taps32<F16TAB>& t) {
 }
 // f = H(x) in fp32 -> A columns 0..15 (hi) | 16..31 (lo), LIF levels per TMEM store
 template <bool F16TAB, int LIF>
-__device__ __forceinline__ void encode_split_to(uint32_t tA, const GridP& g, float x, float y, float z, float* scr = nullptr) {
+__device__ __forceinline__ void encode_split_to(uint32_t tA, const GridP& g, float x, float y, float z, float* scr = nullptr,
+                                                const L2Pol* pol = nullptr) {
 #pragma unroll 1
   for (int l0 = 0; l0 < kMaxL; l0 += LIF) {
     uint32_t hi[LIF], lo[LIF];
@@ -372,7 +373,7 @@ __device__ __forceinline__ void encode_split_to(uint32_t tA, const GridP& g, flo
       // cycle, and 16 warps x 32 loads queue behind each other instead of overlapping with the interpolation of the others.
       hi[q] = 0u; lo[q] = 0u;
       if (l0 + q < (int)g.L) {
-        const float2 v = encode_level<F16TAB>(g, l0 + q, x, y, z, nullptr, nullptr);
+        const float2 v = encode_level<F16TAB>(g, l0 + q, x, y, z, nullptr, nullptr, pol);
         split_pair(v.x, v.y, hi[q], lo[q]);
         if (scr) { scr[(2 * (l0 + q)) * kRows] = v.x; scr[(2 * (l0 + q) + 1) * kRows] = v.y; }
       } else if (scr) {
@@ -834,7 +835,7 @@ __device__ __forceinline__ void feat_split_to(uint32_t tA, const GridP& g, const
 // PREC = 0: fp16 models (fp16 h1, one MMA pass).  PREC = 1: fp32 models in hi/lo split precision -- exactly the arithmetic
 // k_render_wg<PREC = 1> runs for its direct / secondary queries (h1_dir<true>, three passes, epi_precise), so hashrender_trace
 // on an fp32 model checks z_v, t, x' of the production path stage by stage.  feat != nullptr: the caller's features replace H(x).
-template <bool F16TAB, int PREC>
+template <bool F16TAB, int PREC, bool HINT = false>
 __global__ void __launch_bounds__(kRows* kTraceG, 1)
     k_trace_wg(const __grid_constant__ GridP g, ShadeP sp, const __grid_constant__ TcConst cw, const uint8_t* __restrict__ wtiles,
                const float* __restrict__ x, const float* __restrict__ feat, unsigned long long N, DirsetP ds, float* __restrict__ vis,
@@ -881,6 +882,8 @@ __global__ void __launch_bounds__(kRows* kTraceG, 1)
   float4* Ps4 = s_P + (size_t)wgi * (kH / 4) * kRows + c.t;
   const unsigned long long ntiles = (N + kRows - 1) / kRows;
   const uint32_t D = g.L * 2u;
+  L2Pol pol;
+  if constexpr (HINT) pol = make_l2pol();
   for (unsigned long long tile = (unsigned long long)blockIdx.x * G + wgi; tile < ntiles; tile += (unsigned long long)gridDim.x * G) {
     const unsigned long long i_raw = tile * kRows + c.t;
     const bool valid = i_raw < N;
@@ -888,6 +891,7 @@ __global__ void __launch_bounds__(kRows* kTraceG, 1)
     float px = 0.f, py = 0.f, pz = 0.f;
     if (x) { px = __ldg(x + 3 * i); py = __ldg(x + 3 * i + 1); pz = __ldg(x + 3 * i + 2); }
     if (feat) feat_split_to<4>(tA, g, feat + i * D);
+    else if constexpr (HINT) encode_split_to<F16TAB, kTraceLIF>(tA, g, px, py, pz, nullptr, &pol);
     else encode_split_to<F16TAB, kTraceLIF>(tA, g, px, py, pz);
     issue_layer<PREC, G>(c, 0, 0, 2, true, 0, 2);                     // P = W1f f + b1, split-precision f
     wait_layer(c);
@@ -923,12 +927,17 @@ inline cudaError_t launch_trace_one(const GridP& g, const ShadeP& sp, const TcCo
                                     float* xsec, int num_sms, cudaStream_t st) {
   const unsigned long long need = ((N + kRows - 1) / kRows + kTraceG - 1) / kTraceG;
   const int grid = (int)(need < (unsigned long long)num_sms ? need : (unsigned long long)num_sms);
-  k_trace_wg<F16TAB, PREC><<<grid, kRows * kTraceG, trace_smem<PREC>(), st>>>(g, sp, cw, d_tiles, x, feat, N, ds, vis, zv, t, xsec);
+  if (F16TAB && g.l2_hint && !feat)
+    k_trace_wg<F16TAB, PREC, F16TAB><<<grid, kRows * kTraceG, trace_smem<PREC>(), st>>>(g, sp, cw, d_tiles, x, feat, N, ds, vis, zv, t, xsec);
+  else
+    k_trace_wg<F16TAB, PREC><<<grid, kRows * kTraceG, trace_smem<PREC>(), st>>>(g, sp, cw, d_tiles, x, feat, N, ds, vis, zv, t, xsec);
   return cudaGetLastError();
 }
 // the opt-in to > 48 KB of dynamic shared memory is per device: hashrender_create calls this for the handle's device
 template <bool F16TAB, int PREC>
 inline cudaError_t trace_attr() {
+  cudaError_t e = cudaFuncSetAttribute(k_trace_wg<F16TAB, PREC, F16TAB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)trace_smem<PREC>());
+  if (e != cudaSuccess) return e;
   return cudaFuncSetAttribute(k_trace_wg<F16TAB, PREC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)trace_smem<PREC>());
 }
 
