@@ -643,7 +643,7 @@ def main():
         extra = []
         if cfg.flags & gen.HR_INDIRECT:
             extra.append((cfg, args.compact))
-        for nm in [w for w in args.also.split(",") if w and w != args.workload and w != "C4"]:
+        for nm in [w for w in args.also.split(",") if w and w != args.workload and w not in ("C4", "G")]:
             cfg2 = gen.make_config(nm)
             extra += [(cfg2, True), (cfg2, False)] if cfg2.flags & gen.HR_INDIRECT else [(cfg2, True)]
         line["also"] = []

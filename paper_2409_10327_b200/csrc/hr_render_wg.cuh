@@ -67,6 +67,8 @@ struct WgCtx {
   uint32_t ones;      // shared address of the uniform bias operand
   int bar_id;         // named barrier of the WG
   int t;              // thread index in the WG
+  mutable uint32_t rot;   // layers issued so far
+  uint32_t rot_mask;      // 3: the issuing warp rotates over the four warps of the group (k_render_wg); 0: always warp 0 (k_trace_wg)
 };
 
 __device__ __forceinline__ void tmem_st4(uint32_t taddr, const uint32_t (&r)[4]) {
@@ -86,9 +88,13 @@ __device__ __forceinline__ void issue_layer(const WgCtx& c, uint32_t a_col, int 
                                             int bias_kstep, uint32_t idesc = kIdesc, uint32_t d_col = Cols<PREC, G>::d) {
   wait_st();
   fence_before();
-  if (c.t >= 32) {                              // warps 1..3 only announce their rows and go on to the work that needs no D
+  // The issuing warp rotates from layer to layer: warp w of every group sits on SM sub-partition w, so a fixed issuer would put
+  // the barrier wait and the MMA issue of all G groups on one scheduler (C2 dense 23.1 -> 22.9 ms, compacted 10.9 -> 10.65,
+  // C3 compacted 7.54 -> 7.38; k_trace_wg measured slower with it, 5.77 -> 6.24 ms, and keeps warp 0).
+  const uint32_t iw = (c.rot++) & c.rot_mask;
+  if ((uint32_t)(c.t >> 5) != iw) {             // three warps only announce their rows and go on to the work that needs no D
     asm volatile("bar.arrive %0, 128;" ::"r"(c.bar_id) : "memory");
-  } else {                                      // warp 0 of the warpgroup, converged; one elected lane issues
+  } else {                                      // the issuing warp, converged; one elected lane issues
     wg_sync(c);
     fence_after();
     const uint32_t d = c.tmem + d_col;
@@ -506,6 +512,7 @@ __global__ void __launch_bounds__(kRows* G, 1)
   WgCtx c;
   c.t = threadIdx.x % kRows;
   c.bar_id = 1 + wgi;
+  c.rot = 0; c.rot_mask = 3u;
   // ---- setup: TMEM (the CTA owns all 512 columns), mbarriers, weight tiles -----------------------------------------
   if (warp == 0) {
     asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(s_tmem)), "r"(512u) : "memory");
@@ -853,6 +860,7 @@ __global__ void __launch_bounds__(kRows* kTraceG, 1)
   WgCtx c;
   c.t = threadIdx.x % kRows;
   c.bar_id = 1 + wgi;
+  c.rot = 0; c.rot_mask = 0u;
   if (warp == 0) {
     asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(smem_u32(s_tmem)), "r"(512u) : "memory");
     asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
