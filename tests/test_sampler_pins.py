@@ -132,6 +132,60 @@ def test_vndf_samples_follow_their_pdf_and_are_reflections():
     assert np.median(Lm @ mirror) > 0.9998 and np.quantile(Lm @ mirror, 0.05) > 0.997    # GGX tails are long, the bulk is tight
 
 
+def _dvis_textbook(n, alpha, v, h):
+    """Distribution of visible normals as Heitz (2014, 2018) defines it, written out in world space with numpy:
+    D_vis(h) = G1(v) max(0, v.h) D(h) / (v.n),  D(h) = a^2 / (pi ((n.h)^2 (a^2 - 1) + 1)^2),
+    G1(v) = 2 (n.v) / ((n.v) + sqrt(a^2 + (1 - a^2)(n.v)^2))."""
+    nh = h @ n; nv = v @ n
+    D = alpha ** 2 / (PI * (nh ** 2 * (alpha ** 2 - 1) + 1) ** 2) * (nh > 0)
+    G1 = 2 * nv / (nv + np.sqrt(alpha ** 2 + (1 - alpha ** 2) * nv ** 2))
+    return G1 * np.maximum(h @ v, 0) * D / nv
+
+
+@pytest.mark.parametrize("rough,vz", [(0.5, 0.8), (0.8, 0.35)])
+def test_vndf_against_rejection_sampling_of_the_textbook_density(rough, vz):
+    """A check that shares nothing with the sampler's construction (the oracle stretches / projects / unstretches, Heitz 2018):
+    (i) the oracle's pdf equals the closed form D_vis(h) / (4 v.h) written out independently in world space;
+    (ii) half vectors drawn by REJECTION from D_vis (uniform-hemisphere proposals) and reflected give the same histogram of
+    directions as the oracle's sampler -- a shared misreading of the density, the frame or the reflection cannot pass both."""
+    rng = np.random.default_rng(7)
+    n = np.array([0.36, -0.48, 0.8])
+    t = np.cross(n, [0, 0, 1.0]); t /= np.linalg.norm(t); b = np.cross(n, t)
+    v = vz * n + np.sqrt(1 - vz * vz) * (0.6 * t + 0.8 * b)
+    alpha = rough * rough                                                  # PAPER.md:122 "alpha = Roughness^2"
+    # (i) pdf of the reflected direction
+    L = rng.standard_normal((4000, 3)); L /= np.linalg.norm(L, axis=1, keepdims=True)
+    H = L + v; H /= np.linalg.norm(H, axis=1, keepdims=True)
+    ref = _dvis_textbook(n, alpha, v, H) / (4 * np.maximum(H @ v, 1e-300))
+    got = S.ggx_pdf(n, rough, v, L)
+    ok = (H @ n > 1e-6)
+    np.testing.assert_allclose(got[ok], ref[ok], rtol=1e-9, atol=1e-12)
+    # (ii) rejection sampling of h ~ D_vis, proposal uniform on the hemisphere about n (density 1 / 2 pi)
+    M = 2 * PI * alpha ** 2 / (PI * alpha ** 4) / vz * 1.02                # 2 pi max D_vis: D <= 1/(pi a^2), G1 (v.h) <= 1
+    keep = []
+    while sum(len(k) for k in keep) < 120000:
+        z = rng.random(2_000_000); ph = 2 * PI * rng.random(2_000_000)
+        r = np.sqrt(1 - z * z)
+        h = r[:, None] * np.cos(ph)[:, None] * t + r[:, None] * np.sin(ph)[:, None] * b + z[:, None] * n
+        f = 2 * PI * _dvis_textbook(n, alpha, v, h)
+        assert f.max() <= M
+        keep.append(h[rng.random(len(h)) * M < f])
+    h = np.concatenate(keep)
+    Lr = 2 * (h @ v)[:, None] * h - v                                      # reflect the view direction about h
+    m = 350
+    g = (np.arange(m) + 0.5) / m
+    u = np.stack(np.meshgrid(g, g, indexing="ij"), -1).reshape(-1, 2)
+    Lo = S.ggx_sample(n, rough, v, u)
+
+    def cell(x):
+        th = np.arccos(np.clip(x @ n, -1, 1)); ph = np.arctan2(x @ b, x @ t)
+        return (np.minimum((th / PI * 10).astype(int), 9)) * 10 + np.minimum(((ph + PI) / (2 * PI) * 10).astype(int), 9)
+    e1 = np.bincount(cell(Lr), minlength=100) / len(Lr)
+    e2 = np.bincount(cell(Lo), minlength=100) / len(Lo)
+    assert np.abs(e1 - e2).max() < 6e-3, np.abs(e1 - e2).max()
+    assert e1.max() > 0.05                                                 # the histogram has structure to compare
+
+
 # ---------------------------------------------------------------------------------------------- stratified sets
 def test_stratified_hemisphere_and_sphere():
     rng = np.random.default_rng(4)
