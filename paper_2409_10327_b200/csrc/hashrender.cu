@@ -32,6 +32,7 @@ struct hashrender {
   unsigned long long* d_counters = nullptr;   // [0] tile counter, [1] items evaluated, [2] secondary rays traced
   bool split_ok = false;         // fp32 model representable as fp16 hi + lo without overflow (enables the tcgen05 fp32 path)
   float* d_env = nullptr;
+  float4* d_env4 = nullptr;      // the env map padded to RGBA
   size_t env_cap = 0;
   int num_sms = 148;
   uint64_t launches = 0;
@@ -67,6 +68,11 @@ int fail(hashrender* h, int code, const char* fmt, ...) {
       return fail(h, e_ == cudaErrorMemoryAllocation ? HR_ERR_OOM : HR_ERR_CUDA, "%s failed: %s", #call, \
                   cudaGetErrorString(e_));                                                            \
   } while (0)
+
+__global__ void k_env_pack(const float* __restrict__ src, float4* __restrict__ dst, size_t n) {
+  for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x)
+    dst[i] = make_float4(src[3 * i], src[3 * i + 1], src[3 * i + 2], 0.f);
+}
 
 __global__ void k_f32_to_f16(const float* __restrict__ src, __half* __restrict__ dst, size_t n) {
   for (size_t i = blockIdx.x * (size_t)blockDim.x + threadIdx.x; i < n; i += (size_t)gridDim.x * blockDim.x)
@@ -275,7 +281,7 @@ int hashrender_create(const hr_config* cfg, const float* tables, const float* br
   s.near_t = cfg->near_t; s.far_t = cfg->far_t; s.rough_min = cfg->rough_min; s.f0 = cfg->fresnel_f0;
   s.vis_mode = cfg->vis_mode; s.brdf_model = cfg->brdf_model;
   s.as0 = cfg->albedo_scale[0]; s.as1 = cfg->albedo_scale[1]; s.as2 = cfg->albedo_scale[2];
-  h->env.env = nullptr; h->env.He = h->env.We = 0;
+  h->env.env = nullptr; h->env.env4 = nullptr; h->env.He = h->env.We = 0;
 
   const int smem_full = (int)ffma_smem_bytes(NT_FFMA, true), smem_half = (int)ffma_smem_bytes(NT_FFMA, false);
   HR_CUDA(h, cudaFuncSetAttribute(k_render_ffma<false, NT_FFMA>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_full));
@@ -291,7 +297,7 @@ int hashrender_create(const hr_config* cfg, const float* tables, const float* br
 int hashrender_destroy(hashrender_t* h) {
   if (!h) return HR_ERR_INVALID_ARG;
   cudaDeviceSynchronize();
-  cudaFree(h->d_tables); cudaFree(h->d_wts); cudaFree(h->d_wts_tc); cudaFree(h->d_env);
+  cudaFree(h->d_tables); cudaFree(h->d_wts); cudaFree(h->d_wts_tc); cudaFree(h->d_env); cudaFree(h->d_env4);
   cudaFree(h->d_ring); cudaFree(h->d_counters); cudaFree(h->d_light); cudaFree(h->d_svgf);
   if (h->copy_stream) {
     cudaStreamDestroy(h->copy_stream);
@@ -308,11 +314,20 @@ int hashrender_set_env(hashrender_t* h, const float* env, uint32_t He, uint32_t 
   const size_t bytes = (size_t)He * We * 3 * sizeof(float);
   if (bytes > h->env_cap) {
     cudaFree(h->d_env); h->d_env = nullptr; h->env_cap = 0;
+    cudaFree(h->d_env4); h->d_env4 = nullptr;
     HR_CUDA(h, cudaMalloc(&h->d_env, bytes));
+    HR_CUDA(h, cudaMalloc(&h->d_env4, (size_t)He * We * sizeof(float4)));
     h->env_cap = bytes;
   }
   HR_CUDA(h, cudaMemcpyAsync(h->d_env, env, bytes, cudaMemcpyDeviceToDevice, (cudaStream_t)stream));
-  h->env.env = h->d_env; h->env.He = He; h->env.We = We;
+  {
+    const size_t n = (size_t)He * We;
+    const size_t blocks = (n + 255) / 256;
+    k_env_pack<<<(int)(blocks < 4096 ? blocks : 4096), 256, 0, (cudaStream_t)stream>>>(h->d_env, h->d_env4, n);
+    h->launches++;
+    HR_CUDA(h, cudaGetLastError());
+  }
+  h->env.env = h->d_env; h->env.env4 = h->d_env4; h->env.He = He; h->env.We = We;
   h->light_valid = false;
   return HR_OK;
 }

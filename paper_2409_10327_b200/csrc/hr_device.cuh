@@ -41,7 +41,7 @@ __device__ __forceinline__ L2Pol make_l2pol() {
   asm("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p.last));
   return p;
 }
-struct EnvP { const float* env; uint32_t He, We; };
+struct EnvP { const float* env; const float4* env4; uint32_t He, We; };     // env4: the same texels padded to RGBA (one 16-byte load each)
 struct ShadeP {
   float near_t, far_t, rough_min, f0;
   uint32_t vis_mode, brdf_model;
@@ -252,15 +252,15 @@ __device__ __forceinline__ float3 env_lookup(const EnvP& e, float wx, float wy, 
   int x0 = (int)u0 % We; if (x0 < 0) x0 += We;
   int x1 = x0 + 1; if (x1 == We) x1 = 0;
   const int y0 = min(max((int)s0, 0), He - 1), y1 = min(max((int)s0 + 1, 0), He - 1);
-  const float* r0 = e.env + (size_t)y0 * We * 3;
-  const float* r1 = e.env + (size_t)y1 * We * 3;
+  // one 16-byte load per corner (the map is kept padded to RGBA): a query's four texels are four L1 requests instead of twelve --
+  // the lanes of a warp look up unrelated texels, so every scalar load was up to 32 cache-line requests of its own
+  const float4* r0 = e.env4 + (size_t)y0 * We;
+  const float4* r1 = e.env4 + (size_t)y1 * We;
+  const float4 e00 = __ldg(r0 + x0), e01 = __ldg(r0 + x1), e10 = __ldg(r1 + x0), e11 = __ldg(r1 + x1);
   float out[3];
-#pragma unroll
-  for (int ch = 0; ch < 3; ++ch) {
-    const float e00 = __ldg(r0 + x0 * 3 + ch), e01 = __ldg(r0 + x1 * 3 + ch);
-    const float e10 = __ldg(r1 + x0 * 3 + ch), e11 = __ldg(r1 + x1 * 3 + ch);
-    out[ch] = (1.f - fs) * ((1.f - fu) * e00 + fu * e01) + fs * ((1.f - fu) * e10 + fu * e11);
-  }
+  out[0] = (1.f - fs) * ((1.f - fu) * e00.x + fu * e01.x) + fs * ((1.f - fu) * e10.x + fu * e11.x);
+  out[1] = (1.f - fs) * ((1.f - fu) * e00.y + fu * e01.y) + fs * ((1.f - fu) * e10.y + fu * e11.y);
+  out[2] = (1.f - fs) * ((1.f - fu) * e00.z + fu * e01.z) + fs * ((1.f - fu) * e10.z + fu * e11.z);
   return make_float3(out[0], out[1], out[2]);
 }
 
