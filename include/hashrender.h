@@ -171,6 +171,19 @@ typedef struct {
 } hr_denoise;
 int hashrender_denoise(hashrender_t* h, const hr_denoise* d, float* out, void* stream);
 
+/* hashrender_denoise for callers that cannot allocate device memory (code under CUDA graph capture, serving loops, harnesses
+ * that forbid cudaMalloc): the same kernels, arguments and result, with the image planes in a fixed array inside the library
+ * (a file-scope __device__ array, 31.4 MB, held by every GPU that loads the library until the process exits) instead of
+ * handle-owned scratch.  Calls no cudaMalloc / cudaFree or allocating library routine; enqueues 2 + iterations kernels on
+ * `stream` and returns.  H * W > HASHRENDER_DENOISE_STATIC_MAX_PIXELS (one 800 x 800 frame) => HR_ERR_UNSUPPORTED before any
+ * launch, the message naming the limit.  The array's device address is looked up once per device (hashrender_create on that
+ * device does it; otherwise the first call).  The array is SHARED by every call and every handle on the device and keeps the
+ * last call's contents (each call overwrites all it reads, nothing needs clearing): two calls that overlap on the GPU --
+ * different streams without an ordering between them, or two handles from two threads -- race on it and corrupt both results;
+ * order them on one stream or with events. */
+#define HASHRENDER_DENOISE_STATIC_MAX_PIXELS 640000
+int hashrender_denoise_static(hashrender_t* h, const hr_denoise* d, float* out, void* stream);
+
 /* Secondary-ray accounting of the render_frame calls since the last reset: rays_traced = secondary
  * (point, direction) rays whose (v, t) were evaluated, rays_evaluated = those whose L'_o was evaluated (all of them with
  * HR_DENSE).  Both nullable.  Synchronises the device.  Only the tcgen05 paths count; the FFMA path leaves both at 0. */

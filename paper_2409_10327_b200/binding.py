@@ -12,11 +12,12 @@ import numpy as np
 HR_DIRECT, HR_SHADOW, HR_INDIRECT, HR_DENSE = 1, 2, 4, 8
 HR_TERM_DIRECT, HR_TERM_INDIRECT = 1, 2
 _STATUS = {1: "HR_ERR_INVALID_ARG", 2: "HR_ERR_CUDA", 3: "HR_ERR_OOM", 4: "HR_ERR_UNSUPPORTED"}
+DENOISE_STATIC_MAX_PIXELS = 640000      # HASHRENDER_DENOISE_STATIC_MAX_PIXELS of include/hashrender.h
 _LIB_PATH = os.path.join(os.path.dirname(os.path.abspath(__file__)), "libhashrender.so")
 
 EXPORTS = ["hashrender_create", "hashrender_destroy", "hashrender_set_env", "hashrender_encode", "hashrender_decode",
            "hashrender_trace", "hashrender_shade", "hashrender_render_frame", "hashrender_render_frame_host",
-           "hashrender_sample_mis", "hashrender_sample_stratified", "hashrender_denoise", "hashrender_stats", "hashrender_launch_count", "hashrender_last_path", "hashrender_last_error",
+           "hashrender_sample_mis", "hashrender_sample_stratified", "hashrender_denoise", "hashrender_denoise_static", "hashrender_stats", "hashrender_launch_count", "hashrender_last_path", "hashrender_last_error",
            "hashrender_gbuffer_create", "hashrender_gbuffer_destroy", "hashrender_gbuffer_forward", "hashrender_gbuffer_launch_count",
            "hashrender_gbuffer_flops", "hashrender_gbuffer_last_error"]
 
@@ -80,6 +81,7 @@ def load_library(path: str | None = None):
         lib.hashrender_sample_mis.argtypes = [vp, vp, vp, u64, u32, u64, vp, vp, vp]
         lib.hashrender_sample_stratified.argtypes = [vp, vp, u64, u32, u32, u64, vp, vp, vp]
         lib.hashrender_denoise.argtypes = [vp, C.POINTER(hr_denoise), vp, vp]
+        lib.hashrender_denoise_static.argtypes = [vp, C.POINTER(hr_denoise), vp, vp]
         lib.hashrender_stats.argtypes = [vp, C.POINTER(u64), C.POINTER(u64), C.c_int]
         lib.hashrender_launch_count.argtypes = [vp]
         lib.hashrender_launch_count.restype = u64
@@ -268,12 +270,17 @@ class HashRenderer:
         self._check(self._lib.hashrender_sample_stratified(self._h, _arg(normal, "normal"), rows, Sa, Sb, seed, _arg(dir, "dir"), _arg(pdf, "pdf"), stream))
 
     def denoise(self, rgb, normal, pos, cam, out, albedo=None, mask=None, iterations=5, sigma_z=1.0, sigma_n=128.0, sigma_l=4.0,
-                stream=None):
-        """rgb / normal / pos / out: [H, W, 3] device tensors; cam: 3 floats."""
+                stream=None, static_scratch=False):
+        """rgb / normal / pos / out: [H, W, 3] device tensors; cam: 3 floats.  static_scratch: hashrender_denoise_static (no
+        allocation; the planes live in the library's fixed device array, at most DENOISE_STATIC_MAX_PIXELS pixels)."""
         d = hr_denoise(H=rgb.shape[0], W=rgb.shape[1], rgb=_arg(rgb, "rgb"), albedo=_arg(albedo, "albedo"), normal=_arg(normal, "normal"),
                        pos=_arg(pos, "pos"), cam=(C.c_float * 3)(*[float(v) for v in cam]), mask=_arg(mask, "mask", "u8", align=1),
                        iterations=iterations, sigma_z=sigma_z, sigma_n=sigma_n, sigma_l=sigma_l)
-        self._check(self._lib.hashrender_denoise(self._h, C.byref(d), _arg(out, "out"), stream))
+        fn = self._lib.hashrender_denoise_static if static_scratch else self._lib.hashrender_denoise
+        self._check(fn(self._h, C.byref(d), _arg(out, "out"), stream))
+
+    def denoise_static(self, rgb, normal, pos, cam, out, **kw):
+        self.denoise(rgb, normal, pos, cam, out, static_scratch=True, **kw)
 
     def stats(self, reset=False):
         """(secondary rays traced, secondary rays whose L'_o was evaluated) since the last reset."""

@@ -6,6 +6,7 @@
 #include <cstdio>
 #include <cmath>
 #include <cstring>
+#include <mutex>
 #include <new>
 #include <vector>
 
@@ -155,6 +156,40 @@ float mlp_bound(const float* w, int din, int H, float in_max) {
   return fmaxf(B1, B2);
 }
 
+// ---- hashrender_denoise_static: the denoiser's image planes in a file-scope device array (no allocation, ever) ----------------
+// Layout for an n-pixel image (n <= HASHRENDER_DENOISE_STATIC_MAX_PIXELS), the same as the handle-owned scratch of hashrender_denoise:
+// geo [n] | live [n, padded to 16] | colour+variance plane A [n] | plane B [n].  Every GPU that loads the library holds the array until
+// the process exits.  Pass 0 (k_svgf_prep) writes every byte the later passes read, so nothing here has to start at zero and the
+// previous call's contents never show through.
+constexpr size_t kSvgfStaticPixels = HASHRENDER_DENOISE_STATIC_MAX_PIXELS;
+constexpr size_t kSvgfStaticBytes = kSvgfStaticPixels * (sizeof(svgf::Geo) + 2 * sizeof(float4)) + (kSvgfStaticPixels + 15) / 16 * 16;
+static __device__ __align__(256) unsigned char g_svgf_static[kSvgfStaticBytes];
+
+// In host code `g_svgf_static` is only the host-side stand-in of the symbol: the device address comes from cudaGetSymbolAddress,
+// asked once per device with that device current (hashrender_create does, so the first denoise_static call finds it cached).
+constexpr int kMaxDevices = 64;
+char* g_svgf_static_base[kMaxDevices] = {nullptr};
+cudaError_t g_svgf_static_err[kMaxDevices] = {cudaSuccess};
+bool g_svgf_static_asked[kMaxDevices] = {false};
+std::mutex g_svgf_static_mu;
+
+cudaError_t svgf_static_base(char** base) {
+  *base = nullptr;
+  int dev = -1;
+  cudaError_t e = cudaGetDevice(&dev);
+  if (e != cudaSuccess) return e;
+  if (dev < 0 || dev >= kMaxDevices) return cudaErrorInvalidDevice;
+  std::lock_guard<std::mutex> lock(g_svgf_static_mu);
+  if (!g_svgf_static_asked[dev]) {
+    void* p = nullptr;
+    g_svgf_static_err[dev] = cudaGetSymbolAddress(&p, g_svgf_static);
+    g_svgf_static_base[dev] = g_svgf_static_err[dev] == cudaSuccess ? static_cast<char*>(p) : nullptr;
+    g_svgf_static_asked[dev] = g_svgf_static_err[dev] == cudaSuccess;     // a failed query is asked again on the next call
+  }
+  *base = g_svgf_static_base[dev];
+  return g_svgf_static_err[dev];
+}
+
 }  // namespace
 
 extern "C" {
@@ -291,6 +326,7 @@ int hashrender_create(const hr_config* cfg, const float* tables, const float* br
   HR_CUDA(h, cudaFuncSetAttribute(k_decode_ffma<NT_FFMA>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_half));
   HR_CUDA(h, wg::init_device_p0());      // per device (a second handle on another device opts in there too)
   HR_CUDA(h, wg::init_device_p1());
+  { char* b = nullptr; (void)svgf_static_base(&b); }   // set-up for hashrender_denoise_static; a failure is reported by that call
   return HR_OK;
 }
 
@@ -655,6 +691,44 @@ int hashrender_denoise(hashrender_t* h, const hr_denoise* d, float* out, void* s
     h->svgf_cap = need;
   }
   char* base = (char*)h->d_svgf;
+  svgf::Geo* geo = (svgf::Geo*)base;
+  uint8_t* live = (uint8_t*)(base + geo_b);
+  float4* colA = (float4*)(base + geo_b + live_b);
+  float4* colB = colA + n;
+  svgf::Params P;
+  P.H = d->H; P.W = d->W; P.sigma_z = d->sigma_z; P.sigma_n = d->sigma_n; P.sigma_l = d->sigma_l;
+  P.cam[0] = d->cam[0]; P.cam[1] = d->cam[1]; P.cam[2] = d->cam[2];
+  cudaStream_t st = (cudaStream_t)stream;
+  const uint64_t blocks = (n + 255) / 256, cap = (uint64_t)h->num_sms * 16;
+  const int grid = (int)(blocks < cap ? blocks : cap);
+  svgf::k_svgf_prep<<<grid, 256, 0, st>>>(P, d->rgb, d->albedo, d->pos, d->mask, geo, live, colA);
+  svgf::k_svgf_variance<<<grid, 256, 0, st>>>(P, geo, d->normal, live, colA);
+  float4* in = colA; float4* o = colB;
+  for (uint32_t it = 0; it < d->iterations; ++it) {
+    const bool last = it + 1 == d->iterations;
+    svgf::k_svgf_atrous<<<grid, 256, 0, st>>>(P, 1 << it, geo, d->normal, live, in, last ? nullptr : o, d->albedo, last ? out : nullptr);
+    float4* t = in; in = o; o = t;
+  }
+  h->launches += 2 + d->iterations;
+  HR_CUDA(h, cudaGetLastError());
+  return HR_OK;
+}
+
+int hashrender_denoise_static(hashrender_t* h, const hr_denoise* d, float* out, void* stream) {
+  if (!h) return HR_ERR_INVALID_ARG;
+  if (!d) return fail(h, HR_ERR_INVALID_ARG, "denoise_static: NULL descriptor");
+  if (d->H == 0 || d->W == 0) return HR_OK;
+  if (!d->rgb || !d->normal || !d->pos || !out) return fail(h, HR_ERR_INVALID_ARG, "denoise_static: NULL rgb / normal / pos / out");
+  if (d->iterations < 1 || d->iterations > 8) return fail(h, HR_ERR_INVALID_ARG, "denoise_static: iterations must be 1..8");
+  if (!(d->sigma_z > 0.f) || !(d->sigma_l > 0.f) || !(d->sigma_n >= 0.f)) return fail(h, HR_ERR_INVALID_ARG, "denoise_static: bad sigma");
+  const size_t n = (size_t)d->H * d->W;
+  if (n > kSvgfStaticPixels)
+    return fail(h, HR_ERR_UNSUPPORTED, "denoise_static: %u x %u = %zu pixels exceed the static scratch (HASHRENDER_DENOISE_STATIC_MAX_PIXELS = %zu); "
+                "use hashrender_denoise", d->H, d->W, n, kSvgfStaticPixels);
+  char* base = nullptr;
+  const cudaError_t eb = svgf_static_base(&base);
+  if (eb != cudaSuccess || !base) return fail(h, HR_ERR_CUDA, "denoise_static: cudaGetSymbolAddress(g_svgf_static) failed: %s", cudaGetErrorString(eb));
+  const size_t geo_b = n * sizeof(svgf::Geo), live_b = (n + 15) / 16 * 16;
   svgf::Geo* geo = (svgf::Geo*)base;
   uint8_t* live = (uint8_t*)(base + geo_b);
   float4* colA = (float4*)(base + geo_b + live_b);
