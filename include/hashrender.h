@@ -102,7 +102,10 @@ typedef struct {
 /* Creates a renderer.  tables: host, fp32 [L][T][F] (every level owns T = 2^log2_T slots; a dense level --
  * (N_l+1)^3 <= T, Q3 -- uses the first (N_l+1)^3); converted once (RNE) when table_dtype == HR_F16.
  * brdf_w / irt_w: host, fp32 blobs, per layer W[out][in] row-major then b[out]; layers in->64->64->out with
- * in = L*F for B and L*F+3 ([f ; w], Q13) for I.  Synchronous.  Errors: INVALID_ARG, UNSUPPORTED, OOM, CUDA. */
+ * in = L*F for B and L*F+3 ([f ; w], Q13) for I.  Synchronous.  Errors: INVALID_ARG, UNSUPPORTED, OOM, CUDA.
+ * Device memory: the handle's copy of the tables is re-laid out for the gathers; the coarsest levels are also stored cell-major
+ * (the 8 corner rows of every grid cell side by side: one or two 32-byte sectors per point and level instead of ~4.5), within a
+ * budget of a quarter of the L2 cache when L*T rows fit the L2, else four times the size of the tables. */
 int hashrender_create(const hr_config* cfg, const float* tables, const float* brdf_w, const float* irt_w,
                       hashrender_t** out);
 int hashrender_destroy(hashrender_t* h);

@@ -80,6 +80,25 @@ __global__ void k_f32_to_f16(const float* __restrict__ src, __half* __restrict__
     dst[i] = __float2half_rn(src[i]);
 }
 
+// Cell-major copy of one level (hr_device.cuh GridP): entry e = cx + N (cy + N cz) <- the 8 corner rows, each read at the SPECIFIED
+// index (corner_indices: dense x + y (N+1) + z (N+1)^2, or the hash) from the caller's rows `src` of that level.
+template <bool F16>
+__global__ void k_build_cells(const float2* __restrict__ src, uint32_t N, bool dense, uint32_t log2_T, void* __restrict__ dst) {
+  const size_t cells = (size_t)N * N * N;
+  for (size_t e = blockIdx.x * (size_t)blockDim.x + threadIdx.x; e < cells; e += (size_t)gridDim.x * blockDim.x) {
+    Cell c;
+    c.c0[0] = (uint32_t)(e % N); c.c0[1] = (uint32_t)((e / N) % N); c.c0[2] = (uint32_t)(e / ((size_t)N * N));
+    uint32_t idx[8];
+    corner_indices(c, N, dense, log2_T, idx);
+#pragma unroll
+    for (int k = 0; k < 8; ++k) {
+      const float2 v = src[idx[k]];
+      if (F16) reinterpret_cast<__half2*>(dst)[e * 8 + k] = __floats2half2_rn(v.x, v.y);
+      else reinterpret_cast<float2*>(dst)[e * 8 + k] = v;
+    }
+  }
+}
+
 constexpr int NT_FFMA = 256;
 
 void prepare_weights_ffma(const hr_config& c, const float* bw, const float* iw, std::vector<float>& out) {
@@ -225,10 +244,32 @@ int hashrender_create(const hr_config* cfg, const float* tables, const float* br
   const size_t esz = cfg->table_dtype == HR_F32 ? 8 : 4;               // bytes per row (F = 2)
   uint64_t rows_total = 0, lvl_rows[kMaxL], lvl_bits[kMaxL];
   for (uint32_t l = 0; l < kMaxL; ++l) { g.res[l] = 1; g.pa[l] = g.pb[l] = g.pmask[l] = 0; g.off[l] = 0; lvl_rows[l] = 0; lvl_bits[l] = 0; }
+  // Cell-major levels: the coarsest levels whose 8-rows-per-cell copies fit a byte budget.  Tables that fit the L2 keep the copies
+  // to a quarter of it, so that the working set stays resident; larger tables stream from HBM anyway and get four times their own
+  // size.  Measured with k_trace_wg, 2^24 points, fp16 (ms without -> with): T = 2^19 6.25 -> 4.95 (27 MB of copies; 71 MB: 5.13),
+  // 2^20 6.26 -> 5.64 (71 MB: 6.25), 2^21 9.67 -> 7.82 (491 MB), 2^22 11.93 -> 8.83 (491 MB; 1.3 GB: 8.36), 2^24 12.76 -> 9.52
+  // (3.4 GB; 1.3 GB: 10.28, 9.1 GB: 8.86).
+  g.nblock = 0;
+  {
+    int l2 = 0;
+    HR_CUDA(h, cudaDeviceGetAttribute(&l2, cudaDevAttrL2CacheSize, dev));
+    const uint64_t table_bytes = ((uint64_t)cfg->L << cfg->log2_T) * esz;
+    uint64_t budget = table_bytes <= (uint64_t)l2 ? (uint64_t)l2 / 4 : 4 * table_bytes;
+    if (cfg->log2_T > 26) budget = 0;                                 // the build stages one level's rows (T x 8 bytes) on the device
+    uint64_t cum = 0;
+    for (uint32_t l = 0; l < cfg->L; ++l) {
+      const uint64_t N = cfg->res[l], b = N * N * N * 8 * esz;
+      if (N * N * N > (1ull << 28) || cum + b > budget) break;
+      cum += b; g.nblock = l + 1;
+    }
+  }
   for (uint32_t l = 0; l < cfg->L; ++l) {
     g.res[l] = cfg->res[l];
     const uint64_t sN = (uint64_t)cfg->res[l] + 1;
-    if (sN * sN * sN <= T) {
+    if (l < g.nblock) {                                               // 8 rows per cell; entries stay sector-aligned (block levels come first)
+      if (sN * sN * sN <= T) g.dense_mask |= 1u << l;
+      lvl_rows[l] = (uint64_t)cfg->res[l] * cfg->res[l] * cfg->res[l] * 8;
+    } else if (sN * sN * sN <= T) {
       g.dense_mask |= 1u << l;
       uint32_t bx = 1;
       while ((1ull << bx) < sN) ++bx;
@@ -249,7 +290,7 @@ int hashrender_create(const hr_config* cfg, const float* tables, const float* br
     int l2 = 0;
     HR_CUDA(h, cudaDeviceGetAttribute(&l2, cudaDevAttrL2CacheSize, dev));
     uint64_t hashed = 0;
-    for (uint32_t l = 0; l < cfg->L; ++l) if (!((g.dense_mask >> l) & 1u)) hashed += lvl_rows[l] * esz;
+    for (uint32_t l = g.nblock; l < cfg->L; ++l) if (!((g.dense_mask >> l) & 1u)) hashed += lvl_rows[l] * esz;
     g.l2_hint = hashed > 2ull * (uint64_t)l2 ? 1u : 0u;                // measured: helps at 448 MB of hashed levels, hurts at 128 MB (hr_device.cuh)
   }
   HR_CUDA(h, cudaMalloc(&h->d_tables, rows_total * esz));
@@ -261,7 +302,20 @@ int hashrender_create(const hr_config* cfg, const float* tables, const float* br
     if (cfg->table_dtype == HR_F16) HR_CUDA(h, cudaMalloc(&st, chunk * sizeof(float)));
     std::vector<float> relaid;
     cudaError_t e = cudaSuccess;
-    for (uint32_t l = 0; l < cfg->L && e == cudaSuccess; ++l) {
+    float2* lvl_src = nullptr;                                        // one level's rows as given, for the cell-major build
+    if (g.nblock) e = cudaMalloc(&lvl_src, (size_t)T * sizeof(float2));
+    for (uint32_t l = 0; l < g.nblock && e == cudaSuccess; ++l) {
+      const uint64_t sN = (uint64_t)cfg->res[l] + 1;
+      const bool dense = (g.dense_mask >> l) & 1u;
+      e = cudaMemcpy(lvl_src, tables + ((size_t)l << cfg->log2_T) * 2, (dense ? sN * sN * sN : T) * sizeof(float2), cudaMemcpyHostToDevice);
+      if (e != cudaSuccess) break;
+      void* dst = reinterpret_cast<char*>(h->d_tables) + g.off[l];
+      if (cfg->table_dtype == HR_F16) k_build_cells<true><<<h->num_sms * 8, 256>>>(lvl_src, cfg->res[l], dense, cfg->log2_T, dst);
+      else k_build_cells<false><<<h->num_sms * 8, 256>>>(lvl_src, cfg->res[l], dense, cfg->log2_T, dst);
+      e = cudaDeviceSynchronize();
+    }
+    cudaFree(lvl_src);
+    for (uint32_t l = g.nblock; l < cfg->L && e == cudaSuccess; ++l) {
       const float* src = tables + ((size_t)l << cfg->log2_T) * 2;
       if ((g.dense_mask >> l) & 1u) {                                 // vertex (x, y, z): row x + y s + z s^2 -> row x | y << b | z << 2b
         const uint64_t sN = (uint64_t)cfg->res[l] + 1, bx = lvl_bits[l];

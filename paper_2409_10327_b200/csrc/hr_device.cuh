@@ -20,8 +20,14 @@ constexpr int kH = 64;      // hidden width
 // bit 0 of cx), so one aligned two-row load brings both (gather8).  The index the ABI exports (hashrender_encode) is still the
 // specified one, x + y (N+1) + z (N+1)^2 or the hash (corner_indices).  Levels l >= L are null: res 1, pa = pb = pmask = 0, off = a
 // block of zero rows.
+// Cell-major levels (l < nblock, the coarsest ones; hashrender_create picks them by a byte budget): the level is stored as N^3 ENTRIES,
+// one per grid cell (cx, cy, cz), entry index cx + N (cy + N cz), each the cell's 8 corner rows in corner order b0 + 2 b1 + 4 b2 -- the
+// rows the specified index (dense or hashed) names, copied, so values and arithmetic are unchanged.  An entry of fp16 rows is one
+// aligned 32-byte sector (ONE 256-bit load), of fp32 rows two sectors (two loads), against 8 one-row loads that touch ~4.5 sectors:
+// an SM's L1 passes ONE missing sector per cycle to the L2 (measured with fully divergent loads of any width, 289 G loads/s for the
+// chip) and that rate, not arithmetic, bounds the encode, so a level costs one or two sector requests instead of 4.5.
 struct GridP {
-  uint32_t L, log2_T, dense_mask, f16;
+  uint32_t L, log2_T, dense_mask, f16, nblock;
   uint32_t res[kMaxL];
   uint32_t pa[kMaxL], pb[kMaxL], pmask[kMaxL];
   unsigned long long off[kMaxL];
@@ -126,7 +132,22 @@ __device__ __forceinline__ void corner_rows(const GridP& g, int l, const uint32_
 #pragma unroll
   for (int j = 0; j < 4; ++j) { i0[j] = (c0[0] ^ h[j]) & pm; i1[j] = ((c0[0] + 1u) ^ h[j]) & pm; }
 }
+// entry of cell c0 of a cell-major level
+__device__ __forceinline__ const uint4* block_entry(const GridP& g, int l, const uint32_t (&c0)[3], uint32_t entry_bytes) {
+  const uint32_t N = g.res[l];
+  const uint32_t e = c0[0] + N * (c0[1] + N * c0[2]);
+  return reinterpret_cast<const uint4*>(reinterpret_cast<const char*>(g.tables) + g.off[l] + (unsigned long long)e * entry_bytes);
+}
+// one aligned 32-byte sector in ONE load (sm_100 has 256-bit global loads)
+__device__ __forceinline__ void ldg_nc32(const uint4* p, uint32_t (&r)[8]) {
+  asm("ld.global.nc.v8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
+      : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]) : "l"(p));
+}
 __device__ __forceinline__ void gather8_h2(const GridP& g, int l, const uint32_t (&c0)[3], uint32_t (&v)[8]) {
+  if (l < (int)g.nblock) {                                    // warp-uniform: l is a loop counter
+    ldg_nc32(block_entry(g, l, c0, 32u), v);
+    return;
+  }
   uint32_t i0[4], i1[4];
   corner_rows(g, l, c0, i0, i1);
   const char* lb = reinterpret_cast<const char*>(g.tables) + g.off[l];
@@ -138,6 +159,7 @@ __device__ __forceinline__ void gather8_h2(const GridP& g, int l, const uint32_t
 }
 // the same with an L2 eviction policy per level (hashed: evict-first, dense: evict-last)
 __device__ __forceinline__ void gather8_h2_hint(const GridP& g, int l, const uint32_t (&c0)[3], uint32_t (&v)[8], const L2Pol& pol) {
+  if (l < (int)g.nblock) { gather8_h2(g, l, c0, v); return; }
   uint32_t i0[4], i1[4];
   corner_rows(g, l, c0, i0, i1);
   const char* lb = reinterpret_cast<const char*>(g.tables) + g.off[l];
@@ -149,6 +171,17 @@ __device__ __forceinline__ void gather8_h2_hint(const GridP& g, int l, const uin
   }
 }
 __device__ __forceinline__ void gather8_f2(const GridP& g, int l, const uint32_t (&c0)[3], float2 (&v)[8]) {
+  if (l < (int)g.nblock) {
+    const uint4* p = block_entry(g, l, c0, 64u);
+#pragma unroll
+    for (int j = 0; j < 2; ++j) {
+      uint32_t r[8];
+      ldg_nc32(p + 2 * j, r);
+#pragma unroll
+      for (int k = 0; k < 4; ++k) v[4 * j + k] = make_float2(__uint_as_float(r[2 * k]), __uint_as_float(r[2 * k + 1]));
+    }
+    return;
+  }
   uint32_t i0[4], i1[4];
   corner_rows(g, l, c0, i0, i1);
   const char* lb = reinterpret_cast<const char*>(g.tables) + g.off[l];
