@@ -186,6 +186,45 @@ def ncu_record(key):
     return json.load(open(pth)).get(key)
 
 
+_GATHER = None
+
+
+def gather_model():
+    """The L1 roofline of the hash-grid gathers, measured live with hashrender_probe_gather (fully divergent loads from a 32 MiB,
+    L2-resident table, 160 KiB of shared memory requested as the render kernels do): an SM passes one missing 32-byte sector per
+    `c_sector + c_load` cycles when every load has a sector of its own, and every further load of the same sector costs `c_load`.
+    cycles per point = c_sector * sectors + c_load * loads."""
+    global _GATHER
+    if _GATHER is None:
+        from paper_2409_10327_b200.binding import probe_gather
+        rows = {}
+        for name, (w, grp) in {"4B x1": (4, 1), "4B x2 per sector": (4, 2), "4B x4 per sector": (4, 4), "4B x8 per sector": (4, 8),
+                               "8B x1": (8, 1), "32B x1": (32, 1)}.items():
+            per_cycle, per_s = probe_gather(32 << 20, w, grp, 160 << 10)
+            rows[name] = {"loads_per_cycle_per_sm": per_cycle, "loads_per_s": per_s}
+        c1 = 1.0 / rows["4B x1"]["loads_per_cycle_per_sm"]              # cycles per load = per sector
+        c2 = 2.0 / rows["4B x2 per sector"]["loads_per_cycle_per_sm"]   # cycles per sector with two loads in it
+        c_load = c2 - c1
+        _GATHER = {"probe": rows, "c_sector": c1 - c_load, "c_load": c_load,
+                   "l1_hit": probe_gather(16 << 10, 4, 1, 160 << 10)[0]}
+    return _GATHER
+
+
+def gather_floor(n_points, levels, cell_major, rows_per_sector, sm_mhz, num_sms=148):
+    """L1 floor of the encode of n_points: cell-major levels cost one sector and one load (fp16) or two and two (fp32 rows),
+    the others 8 loads in 4 x-pairs, each pair in one sector unless it straddles a sector boundary."""
+    gm = gather_model()
+    per_entry = 1 if rows_per_sector == 8 else 2
+    sectors = cell_major * per_entry + (levels - cell_major) * 4 * (1 + 1.0 / rows_per_sector)
+    loads = cell_major * per_entry + (levels - cell_major) * 8
+    cyc = gm["c_sector"] * sectors + gm["c_load"] * loads
+    ms = n_points * cyc / num_sms / (sm_mhz * 1e3)
+    return {"sectors_per_point": sectors, "loads_per_point": loads, "c_sector": gm["c_sector"], "c_load": gm["c_load"],
+            "cycles_per_point": cyc, "floor_ms": ms, "sm_mhz": sm_mhz,
+            "probe_loads_per_cycle_per_sm": gm["probe"]["4B x1"]["loads_per_cycle_per_sm"],
+            "probe_loads_per_s": gm["probe"]["4B x1"]["loads_per_s"]}
+
+
 C4_ALG_BYTES = 16 * 8 * 4 + 24 + 8      # per point: 128 gathers x one fp16 pair + position / direction in + (v, t) out (SURVEY 8(d))
 
 
@@ -245,6 +284,15 @@ def measure_c4(log2_T, Ns, steps, vis_mode, peaks, clock_index=None):
         if rec.get("traffic"):
             roof["traffic_GBps"] = rec["traffic"] / (ms * 1e-3) / 1e9
             roof["traffic_frac_of_peak"] = roof["traffic_GBps"] / peaks["hbm"]
+        nblock, dev_bytes = r.table_layout()
+        mhz = (clk or {}).get("sm_mhz") or 1900.0
+        l1 = gather_floor(N, 16, nblock, 8, mhz)
+        l1["frac"] = l1["floor_ms"] / ms
+        l1["note"] = ("floor of the encode's gathers alone at the L1 sector-request rate measured by hashrender_probe_gather; it binds while "
+                      "the table is L2-resident (T <= 2^20), HBM traffic binds beyond")
+        roof["l1_gather"] = l1
+        roof["cell_major_levels"] = nblock
+        roof["device_table_MiB"] = dev_bytes / 2 ** 20
         rows.append({"log2_T": log2_T, "table_MiB": 16 * (1 << log2_T) * 4 / 2 ** 20, "N": N, "ms": ms, "points_per_s": N / (ms * 1e-3),
                      "useful_gather_GBps": useful / (ms * 1e-3) / 1e9, "sector_GBps_upper": useful * 8 / (ms * 1e-3) / 1e9,
                      "path": path, "roofline": roof, "clocks": clk})
@@ -377,7 +425,7 @@ def main():
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=10)
     ap.add_argument("--warmup", type=int, default=3)
-    ap.add_argument("--workload", default="C2", choices=["C1", "C2", "C3", "C3a", "C4", "G"])
+    ap.add_argument("--workload", default="C2", choices=["C1", "C2", "C3", "C3a", "C4", "G", "probe"])
     ap.add_argument("--full-sweep", action="store_true", help="C4: include 2^26 points")
     ap.add_argument("--c4-log2t", type=int, default=0, help="C4: only this table size (for profiling one point of the sweep)")
     ap.add_argument("--c4-n", type=int, default=0, help="C4: only this many points")
@@ -409,7 +457,18 @@ def main():
                           "e2e": {"value": g["e2e_ms_per_frame"], "unit": "ms", "h2d_bytes_per_step": g["h2d_bytes_per_step"],
                                   "d2h_bytes_per_step": g["d2h_bytes_per_step"]}}))
         return
-    cfg = gen.make_config("C2" if args.workload == "G" else args.workload)
+    if args.workload == "probe" and args.impl != "reference":
+        import torch
+        torch.cuda.set_device(0)
+        torch.zeros(1, device="cuda")
+        gm = gather_model()
+        print(json.dumps({"metric": "divergent-gather rate of an SM's L1 (hashrender_probe_gather)", "value": gm["probe"]["4B x1"]["loads_per_s"],
+                          "unit": "loads/s", "n_gpus": 1, "higher_is_better": True, "data": "synthetic",
+                          "config": {"workload": "512 threads per SM, 8 independent pseudo-random slots in flight per thread, 32 MiB table "
+                                                 "(L2-resident), 160 KiB dynamic shared memory"},
+                          "probe": gm["probe"], "c_sector": gm["c_sector"], "c_load": gm["c_load"], "l1_hit_loads_per_cycle_per_sm": gm["l1_hit"]}))
+        return
+    cfg = gen.make_config("C2" if args.workload in ("G", "probe") else args.workload)
     if args.impl == "reference":
         return run_reference(args, gen.make_config("C2") if args.workload == "C4" else cfg)
     if args.workload == "C4":
@@ -484,7 +543,8 @@ def main():
         total_ms = hd.max_over_ranks(total_ms, dev)
         assert torch.isfinite(rgb).all()
         out = dict(total_ms=total_ms, per=per, launches=launches, clk=clk, path=r.last_path(), mean_rgb=float(rgb.mean().item()),
-                   traced=traced // max(steps, 1), evaluated=(evaluated // max(steps, 1)) if traced else None)
+                   traced=traced // max(steps, 1), evaluated=(evaluated // max(steps, 1)) if traced else None,
+                   cell_major=r.table_layout()[0], device_table_MiB=r.table_layout()[1] / 2 ** 20)
         # end to end through the public host-buffer entry point: pinned host inputs, H2D + D2H inside the timed region
         if e2e_steps:
             pin = lambda a: torch.from_numpy(a).pin_memory().numpy()
@@ -577,7 +637,7 @@ def main():
     value = world * cfg.queries / (ms * 1e-3)
     kernel_ms = float(np.mean(res["per"]))          # the step is ONE kernel launch: its duration is the step's
 
-    def roofline(cfg, path, kernel_ms, evaluated):
+    def roofline(cfg, path, kernel_ms, evaluated, res=None):
         flops = algorithmic_flops(cfg, evaluated)
         ach = flops / (kernel_ms * 1e-3) / 1e12
         if path.startswith("tcgen05"):
@@ -605,9 +665,23 @@ def main():
             roof[k] = rec.get(k)
         if rec.get("warp_inst"):                               # thread instructions per executed query, from the capture's dense frame
             roof["thread_inst_per_query"] = rec["warp_inst"] * 32 / cfg.queries
+        if res is not None and path.startswith("tcgen05") and world == 1:
+            # the second roofline of this kernel: the L1 sector-request rate of the encode's gathers (every primary point and every
+            # evaluated secondary hit is encoded once), measured live by hashrender_probe_gather
+            ind = bool(cfg.flags & gen.HR_INDIRECT)
+            ev = (cfg.N * cfg.S_i if evaluated is None else evaluated) if ind else 0
+            mhz = (res.get("clk") or {}).get("sm_mhz") or 1900.0
+            l1 = gather_floor(cfg.N + ev, cfg.L, res["cell_major"], 8 if cfg.table_dtype == "f16" else 4, mhz)
+            l1["frac"] = l1["floor_ms"] / kernel_ms
+            l1["encoded_points"] = cfg.N + ev
+            l1["note"] = ("time the encode's gathers alone need at the measured L1 rate for divergent loads; the kernel cannot run faster than "
+                          "max(this, the issue-slot floor), and its gathers and MMA round trips overlap only partly")
+            roof["l1_gather"] = l1
+            roof["cell_major_levels"] = res["cell_major"]
+            roof["device_table_MiB"] = res["device_table_MiB"]
         return roof
 
-    roof = roofline(cfg, res["path"], kernel_ms, res["evaluated"])
+    roof = roofline(cfg, res["path"], kernel_ms, res["evaluated"], res)
     dt = {"tcgen05-f16": "f16", "tcgen05-f16x3": "f16x3 (fp16 hi+lo split operands, three tcgen05 passes, fp32 accumulate)"}.get(res["path"], "f32")
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": max(args.warmup, 3),
@@ -651,7 +725,7 @@ def main():
             st = max(args.steps // 2, 3)
             r2, _ = measure(c2, st, 3, 0, ClockSampler(local), dense=dense)
             ms2 = r2["total_ms"] / st
-            rf = roofline(c2, r2["path"], ms2, r2["evaluated"])
+            rf = roofline(c2, r2["path"], ms2, r2["evaluated"], r2)
             line["also"].append({"workload": workload_name(c2), "secondary_rays": "dense" if dense else "compacted", "ms_per_frame": ms2,
                                  "frame_equivalent_queries_per_s": c2.queries / (ms2 * 1e-3),
                                  "executed_queries_per_frame": executed_queries(c2, r2["evaluated"]),

@@ -192,6 +192,19 @@ int hashrender_denoise_static(hashrender_t* h, const hr_denoise* d, float* out, 
  * HR_DENSE).  Both nullable.  Synchronises the device.  Only the tcgen05 paths count; the FFMA path leaves both at 0. */
 int hashrender_stats(hashrender_t* h, uint64_t* rays_traced, uint64_t* rays_evaluated, int reset);
 
+/* Layout of the handle's device copy of the tables: how many of the coarsest levels are stored cell-major (see hashrender_create)
+ * and the bytes the copy takes.  Both nullable. */
+int hashrender_table_layout(const hashrender_t* h, uint32_t* cell_major_levels, uint64_t* device_table_bytes);
+
+/* Measurement aid, no handle: the rate at which the current device serves fully divergent global loads -- the roofline of the
+ * hash-grid gathers.  512 threads per SM draw pseudo-random slots of a scratch table of `table_bytes`
+ * (a power of two, 4 KiB .. 8 GiB; allocated and freed inside the call) and load `group` consecutive words of `width` bytes
+ * from each: (width, group) = (4,1) (8,1) (32,1) one load per 32-byte sector, (4,2) (4,4) (4,8) that many loads per sector.
+ * smem_bytes of dynamic shared memory are requested, which sets the L1 left beside it.  Outputs (host): loads per SM clock
+ * cycle and SM, loads per second for the chip.  Synchronous.  Errors: INVALID_ARG, UNSUPPORTED (other width / group), OOM, CUDA. */
+int hashrender_probe_gather(uint64_t table_bytes, uint32_t width, uint32_t group, uint32_t smem_bytes,
+                            double* loads_per_cycle_per_sm, double* loads_per_s);
+
 /* Number of kernels this handle has launched so far (for launch accounting in benchmarks). */
 uint64_t hashrender_launch_count(const hashrender_t* h);
 

@@ -17,7 +17,7 @@ _LIB_PATH = os.path.join(os.path.dirname(os.path.abspath(__file__)), "libhashren
 
 EXPORTS = ["hashrender_create", "hashrender_destroy", "hashrender_set_env", "hashrender_encode", "hashrender_decode",
            "hashrender_trace", "hashrender_shade", "hashrender_render_frame", "hashrender_render_frame_host",
-           "hashrender_sample_mis", "hashrender_sample_stratified", "hashrender_denoise", "hashrender_denoise_static", "hashrender_stats", "hashrender_launch_count", "hashrender_last_path", "hashrender_last_error",
+           "hashrender_sample_mis", "hashrender_sample_stratified", "hashrender_denoise", "hashrender_denoise_static", "hashrender_table_layout", "hashrender_probe_gather", "hashrender_stats", "hashrender_launch_count", "hashrender_last_path", "hashrender_last_error",
            "hashrender_gbuffer_create", "hashrender_gbuffer_destroy", "hashrender_gbuffer_forward", "hashrender_gbuffer_launch_count",
            "hashrender_gbuffer_flops", "hashrender_gbuffer_last_error"]
 
@@ -83,6 +83,8 @@ def load_library(path: str | None = None):
         lib.hashrender_denoise.argtypes = [vp, C.POINTER(hr_denoise), vp, vp]
         lib.hashrender_denoise_static.argtypes = [vp, C.POINTER(hr_denoise), vp, vp]
         lib.hashrender_stats.argtypes = [vp, C.POINTER(u64), C.POINTER(u64), C.c_int]
+        lib.hashrender_table_layout.argtypes = [vp, C.POINTER(C.c_uint32), C.POINTER(u64)]
+        lib.hashrender_probe_gather.argtypes = [u64, C.c_uint32, C.c_uint32, C.c_uint32, C.POINTER(C.c_double), C.POINTER(C.c_double)]
         lib.hashrender_launch_count.argtypes = [vp]
         lib.hashrender_launch_count.restype = u64
         lib.hashrender_last_path.argtypes = [vp]
@@ -288,11 +290,27 @@ class HashRenderer:
         self._check(self._lib.hashrender_stats(self._h, C.byref(a), C.byref(b), 1 if reset else 0))
         return a.value, b.value
 
+    def table_layout(self):
+        """(number of cell-major levels, bytes of the device copy of the tables)."""
+        a, b = C.c_uint32(), C.c_uint64()
+        self._check(self._lib.hashrender_table_layout(self._h, C.byref(a), C.byref(b)))
+        return a.value, b.value
+
     def launch_count(self) -> int:
         return int(self._lib.hashrender_launch_count(self._h))
 
     def last_path(self) -> str:
         return self._lib.hashrender_last_path(self._h).decode()
+
+
+def probe_gather(table_bytes, width=4, group=1, smem_bytes=0):
+    """hashrender_probe_gather on the current device: (loads per cycle and SM, loads per second)."""
+    lib = load_library()
+    a, b = C.c_double(), C.c_double()
+    rc = lib.hashrender_probe_gather(table_bytes, width, group, smem_bytes, C.byref(a), C.byref(b))
+    if rc != 0:
+        raise HashRenderError(rc, "hashrender_probe_gather")
+    return a.value, b.value
 
 
 class GBufferNet:

@@ -26,6 +26,7 @@ struct hashrender {
   ShadeP shade;
   EnvP env;
   void* d_tables = nullptr;
+  uint64_t table_bytes = 0;      // size of the device copy of the tables (all layouts)
   float* d_wts = nullptr;        // prepared fp32 weights (hr_kernels_ffma.cuh layout)
   uint8_t* d_wts_tc = nullptr;   // fp16 UMMA weight tiles, hi then lo halves (hr_render_wg.cuh)
   std::vector<uint8_t> h_wts_tc; // host copy of [TcConst | hi tiles | lo tiles]; TcConst is passed by value at launch
@@ -175,6 +176,67 @@ float mlp_bound(const float* w, int din, int H, float in_max) {
   return fmaxf(B1, B2);
 }
 
+// ---- hashrender_probe_gather: the rate at which an SM's L1 serves fully divergent loads (the roofline of the encode) -----------
+// Every thread draws pseudo-random slots of a table and loads `group` consecutive W-byte words of each (group = 1: every load its own
+// 32-byte sector; 2 / 4 / 8: that many loads per sector, as the corner rows of an x-pair are), eight independent slots in flight.
+__device__ __forceinline__ uint32_t probe_mix(uint32_t x) { x ^= x >> 16; x *= 0x7feb352du; x ^= x >> 15; x *= 0x846ca68bu; x ^= x >> 16; return x; }
+template <int W> __device__ __forceinline__ uint32_t probe_ld(const uint8_t* p);
+template <> __device__ __forceinline__ uint32_t probe_ld<4>(const uint8_t* p) { uint32_t v; asm volatile("ld.global.nc.b32 %0, [%1];" : "=r"(v) : "l"(p)); return v; }
+template <> __device__ __forceinline__ uint32_t probe_ld<8>(const uint8_t* p) {
+  uint32_t a, b; asm volatile("ld.global.nc.v2.b32 {%0, %1}, [%2];" : "=r"(a), "=r"(b) : "l"(p)); return a ^ b;
+}
+template <> __device__ __forceinline__ uint32_t probe_ld<32>(const uint8_t* p) {
+  uint32_t r[8];
+  asm volatile("ld.global.nc.v8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
+               : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]) : "l"(p));
+  return r[0] ^ r[1] ^ r[2] ^ r[3] ^ r[4] ^ r[5] ^ r[6] ^ r[7];
+}
+template <int W, int GROUP>
+__global__ void k_probe_gather(const uint8_t* __restrict__ tab, uint32_t mask, int iters, uint32_t* sink, unsigned long long* cycles) {
+  constexpr int IF = 8;                                               // independent slots in flight per thread
+  uint32_t s = probe_mix(blockIdx.x * blockDim.x + threadIdx.x + 1u), acc = 0;
+  const long long t0 = clock64();
+  for (int it = 0; it < iters; ++it) {
+    uint32_t v[IF * GROUP];
+#pragma unroll
+    for (int q = 0; q < IF; ++q) {
+      s = probe_mix(s + q + 1u);
+#pragma unroll
+      for (int e = 0; e < GROUP; ++e) v[q * GROUP + e] = probe_ld<W>(tab + (size_t)(((s & mask) & ~(uint32_t)(GROUP - 1)) + e) * W);
+    }
+#pragma unroll
+    for (int q = 0; q < IF * GROUP; ++q) acc += v[q];
+  }
+  const long long t1 = clock64();
+  if (acc == 0x12345u) sink[0] = acc;
+  if (threadIdx.x == 0) atomicAdd(cycles, (unsigned long long)(t1 - t0));
+}
+template <int W, int GROUP>
+cudaError_t run_probe(const uint8_t* tab, uint64_t bytes, int smem, int sms, uint32_t* sink, unsigned long long* cyc, double* per_cycle, double* per_s) {
+  const uint32_t mask = (uint32_t)(bytes / W - 1);
+  const int threads = 512, iters = 2048 / GROUP;
+  cudaError_t e = cudaFuncSetAttribute(k_probe_gather<W, GROUP>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+  if (e != cudaSuccess) return e;
+  k_probe_gather<W, GROUP><<<sms, threads, smem>>>(tab, mask, 16, sink, cyc);           // warm-up
+  cudaMemset(cyc, 0, 8);
+  cudaEvent_t a, b;
+  cudaEventCreate(&a); cudaEventCreate(&b);
+  cudaEventRecord(a);
+  k_probe_gather<W, GROUP><<<sms, threads, smem>>>(tab, mask, iters, sink, cyc);
+  cudaEventRecord(b);
+  e = cudaEventSynchronize(b);
+  float ms = 0.f;
+  cudaEventElapsedTime(&ms, a, b);
+  cudaEventDestroy(a); cudaEventDestroy(b);
+  if (e != cudaSuccess) return e;
+  unsigned long long c = 0;
+  e = cudaMemcpy(&c, cyc, 8, cudaMemcpyDeviceToHost);
+  const double loads = (double)threads * iters * 8 * GROUP;
+  *per_cycle = loads / ((double)c / sms);
+  *per_s = loads * sms / (ms * 1e-3);
+  return e;
+}
+
 // ---- hashrender_denoise_static: the denoiser's image planes in a file-scope device array (no allocation, ever) ----------------
 // Layout for an n-pixel image (n <= HASHRENDER_DENOISE_STATIC_MAX_PIXELS), the same as the handle-owned scratch of hashrender_denoise:
 // geo [n] | live [n, padded to 16] | colour+variance plane A [n] | plane B [n].  Every GPU that loads the library holds the array until
@@ -294,6 +356,7 @@ int hashrender_create(const hr_config* cfg, const float* tables, const float* br
     g.l2_hint = hashed > 2ull * (uint64_t)l2 ? 1u : 0u;                // measured: helps at 448 MB of hashed levels, hurts at 128 MB (hr_device.cuh)
   }
   HR_CUDA(h, cudaMalloc(&h->d_tables, rows_total * esz));
+  h->table_bytes = rows_total * esz;
   HR_CUDA(h, cudaMemset(h->d_tables, 0, rows_total * esz));
   const size_t n = (size_t)cfg->L << cfg->log2_T << 1;                  // floats in the caller's [L][T][2] array
   {
@@ -803,6 +866,40 @@ int hashrender_denoise_static(hashrender_t* h, const hr_denoise* d, float* out, 
   }
   h->launches += 2 + d->iterations;
   HR_CUDA(h, cudaGetLastError());
+  return HR_OK;
+}
+
+int hashrender_probe_gather(uint64_t table_bytes, uint32_t width, uint32_t group, uint32_t smem_bytes, double* loads_per_cycle_per_sm,
+                            double* loads_per_s) {
+  if (!loads_per_cycle_per_sm || !loads_per_s || table_bytes < 4096 || (table_bytes & (table_bytes - 1)) || table_bytes > (1ull << 33))
+    return HR_ERR_INVALID_ARG;
+  int dev = 0, sms = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return HR_ERR_CUDA;
+  uint8_t* tab = nullptr; uint32_t* sink = nullptr; unsigned long long* cyc = nullptr;
+  if (cudaMalloc(&tab, table_bytes) != cudaSuccess) return HR_ERR_OOM;
+  cudaError_t e = cudaMalloc(&sink, 4);
+  if (e == cudaSuccess) e = cudaMalloc(&cyc, 8);
+  if (e == cudaSuccess) e = cudaMemset(tab, 1, table_bytes);
+  int rc = HR_OK;
+  if (e == cudaSuccess) {
+    const int sm = (int)smem_bytes;
+    if (width == 4 && group == 1) e = run_probe<4, 1>(tab, table_bytes, sm, sms, sink, cyc, loads_per_cycle_per_sm, loads_per_s);
+    else if (width == 4 && group == 2) e = run_probe<4, 2>(tab, table_bytes, sm, sms, sink, cyc, loads_per_cycle_per_sm, loads_per_s);
+    else if (width == 4 && group == 4) e = run_probe<4, 4>(tab, table_bytes, sm, sms, sink, cyc, loads_per_cycle_per_sm, loads_per_s);
+    else if (width == 4 && group == 8) e = run_probe<4, 8>(tab, table_bytes, sm, sms, sink, cyc, loads_per_cycle_per_sm, loads_per_s);
+    else if (width == 8 && group == 1) e = run_probe<8, 1>(tab, table_bytes, sm, sms, sink, cyc, loads_per_cycle_per_sm, loads_per_s);
+    else if (width == 32 && group == 1) e = run_probe<32, 1>(tab, table_bytes, sm, sms, sink, cyc, loads_per_cycle_per_sm, loads_per_s);
+    else rc = HR_ERR_UNSUPPORTED;
+  }
+  cudaFree(tab); cudaFree(sink); cudaFree(cyc);
+  if (e != cudaSuccess) return e == cudaErrorMemoryAllocation ? HR_ERR_OOM : HR_ERR_CUDA;
+  return rc;
+}
+
+int hashrender_table_layout(const hashrender_t* h, uint32_t* cell_major_levels, uint64_t* device_table_bytes) {
+  if (!h) return HR_ERR_INVALID_ARG;
+  if (cell_major_levels) *cell_major_levels = h->grid.nblock;
+  if (device_table_bytes) *device_table_bytes = h->table_bytes;
   return HR_OK;
 }
 

@@ -1,0 +1,88 @@
+"""The device layout of the tables (cell-major copies of the coarsest levels, hashrender_table_layout) and the gather probe.
+The values a cell-major level returns are checked by every encode / trace / frame parity test (the layout is the default); this
+file checks that those tests really run through BOTH kinds of cell-major level -- dense ones and hashed ones -- and that the
+budget rule of hashrender_create holds."""
+import numpy as np
+import pytest
+
+import gen
+from hr_testutil import make_renderer, to_dev
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def torch():
+    import torch
+    assert torch.cuda.is_available()
+    return torch
+
+
+def _expected_cell_major(cfg, res, l2_bytes):
+    esz = 8 if cfg.table_dtype == "f32" else 4
+    table = cfg.L * cfg.T * esz
+    budget = l2_bytes // 4 if table <= l2_bytes else 4 * table
+    n, cum = 0, 0
+    for N in res:
+        b = int(N) ** 3 * 8 * esz
+        if cum + b > budget:
+            break
+        cum += b
+        n += 1
+    return n, cum
+
+
+@pytest.mark.parametrize("name,over", [("C0", {}), ("C3", {"N": 640000}), ("C4", {"log2_T": 16}), ("C4", {"log2_T": 22})])
+def test_cell_major_levels_follow_the_budget_and_cover_hashed_levels(torch, name, over):
+    cfg = gen.make_config(name, **over)
+    model = gen.make_model(cfg)
+    r = make_renderer(cfg, model)
+    nblock, dev_bytes = r.table_layout()
+    l2 = torch.cuda.get_device_properties(0).L2_cache_size
+    res = [int(v) for v in model["res"]]
+    want, cum = _expected_cell_major(cfg, res, l2)
+    assert nblock == want and 1 <= nblock <= cfg.L
+    assert dev_bytes >= cum
+    hashed = [l for l in range(nblock) if (res[l] + 1) ** 3 > cfg.T]
+    dense = [l for l in range(nblock) if (res[l] + 1) ** 3 <= cfg.T]
+    if name in ("C0", "C4"):
+        assert hashed and dense, "the parity tests on this config must cover dense AND hashed cell-major levels"
+    # the cell-major copy returns exactly the rows the specified index names: features at random points against
+    # interpolating the caller's table at the indices hashrender_encode reports
+    rng = np.random.default_rng(7)
+    x = rng.random((4096, 3), dtype=np.float32)
+    x[:8] = [[0, 0, 0], [1, 1, 1], [1, 0, 0], [0, 1, 0], [0, 0, 1], [1, 1, 0], [0.5, 1, 1], [1, 0.25, 1]]
+    feat = torch.empty((4096, 2 * cfg.L), device="cuda")
+    idx = torch.empty((4096, cfg.L, 8), device="cuda", dtype=torch.int32)
+    w = torch.empty((4096, cfg.L, 3), device="cuda")
+    r.encode(to_dev(x), feat, idx=idx, w=w)
+    torch.cuda.synchronize()
+    idx_h, w_h, f_h = idx.cpu().numpy().astype(np.int64), w.cpu().numpy(), feat.cpu().numpy()
+    tab = model["tables"].astype(np.float32)
+    if cfg.table_dtype == "f16":
+        tab = tab.astype(np.float16).astype(np.float32)
+    for l in range(nblock):
+        rows = tab[l][idx_h[:, l, :]]                                 # [n, 8, 2]
+        wx, wy, wz = w_h[:, l, 0], w_h[:, l, 1], w_h[:, l, 2]
+        f = np.zeros((4096, 2), np.float32)
+        for k in range(8):
+            wt = ((wx if k & 1 else np.float32(1) - wx) * (wy if k & 2 else np.float32(1) - wy)).astype(np.float32)
+            wt = (wt * (wz if k & 4 else np.float32(1) - wz)).astype(np.float32)
+            f = (f.astype(np.float64) + wt[:, None].astype(np.float64) * rows[:, k, :].astype(np.float64))   # fma: one rounding
+            f = f.astype(np.float32)
+        # (the fp64 emulation of fmaf can differ from it by a double rounding: one ulp of the feature; a wrong row is O(table scale))
+        np.testing.assert_allclose(f, f_h[:, 2 * l:2 * l + 2], rtol=0, atol=3e-7 * float(np.abs(tab[l]).max()), err_msg=f"level {l}")
+    r.destroy()
+
+
+def test_probe_gather_reports_a_sane_rate(torch):
+    from paper_2409_10327_b200.binding import HashRenderError, probe_gather
+    miss, per_s = probe_gather(32 << 20, 4, 1, 160 << 10)              # L2-resident table, L1 misses
+    pair, _ = probe_gather(32 << 20, 4, 2, 160 << 10)
+    hit, _ = probe_gather(16 << 10, 4, 1, 160 << 10)                   # L1-resident table
+    print(f"probe: {miss:.3f} loads/cycle/SM on misses ({per_s / 1e9:.0f} G loads/s), {pair:.3f} with two loads per sector, {hit:.3f} on L1 hits")
+    assert 0.5 < miss < 1.3 and miss < pair < 2.0 * miss + 0.1 and hit > 2.0 * miss
+    with pytest.raises(HashRenderError):
+        probe_gather(3000, 4, 1, 0)                                    # not a power of two
+    with pytest.raises(HashRenderError):
+        probe_gather(1 << 20, 16, 3, 0)                                # unsupported shape
