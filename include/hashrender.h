@@ -105,7 +105,8 @@ typedef struct {
  * in = L*F for B and L*F+3 ([f ; w], Q13) for I.  Synchronous.  Errors: INVALID_ARG, UNSUPPORTED, OOM, CUDA.
  * Device memory: the handle's copy of the tables is re-laid out for the gathers; the coarsest levels are also stored cell-major
  * (the 8 corner rows of every grid cell side by side: one or two 32-byte sectors per point and level instead of ~4.5), within a
- * budget of a quarter of the L2 cache when L*T rows fit the L2, else four times the size of the tables. */
+ * budget of a quarter of the L2 cache when L*T rows fit the L2, else four times the size of the tables, and never more than a
+ * quarter of the device memory free at the call (hashrender_table_layout reports what was built). */
 int hashrender_create(const hr_config* cfg, const float* tables, const float* brdf_w, const float* irt_w,
                       hashrender_t** out);
 int hashrender_destroy(hashrender_t* h);

@@ -317,6 +317,9 @@ int hashrender_create(const hr_config* cfg, const float* tables, const float* br
     HR_CUDA(h, cudaDeviceGetAttribute(&l2, cudaDevAttrL2CacheSize, dev));
     const uint64_t table_bytes = ((uint64_t)cfg->L << cfg->log2_T) * esz;
     uint64_t budget = table_bytes <= (uint64_t)l2 ? (uint64_t)l2 / 4 : 4 * table_bytes;
+    size_t mem_free = 0, mem_total = 0;
+    HR_CUDA(h, cudaMemGetInfo(&mem_free, &mem_total));
+    if (budget > mem_free / 4) budget = mem_free / 4;                 // the copies are an optimisation: never crowd out the caller
     if (cfg->log2_T > 26) budget = 0;                                 // the build stages one level's rows (T x 8 bytes) on the device
     uint64_t cum = 0;
     for (uint32_t l = 0; l < cfg->L; ++l) {

@@ -21,7 +21,7 @@ def torch():
 def _expected_cell_major(cfg, res, l2_bytes):
     esz = 8 if cfg.table_dtype == "f32" else 4
     table = cfg.L * cfg.T * esz
-    budget = l2_bytes // 4 if table <= l2_bytes else 4 * table
+    budget = l2_bytes // 4 if table <= l2_bytes else 4 * table      # (the free-memory cap of hashrender_create is far away on a test box)
     n, cum = 0, 0
     for N in res:
         b = int(N) ** 3 * 8 * esz
