@@ -481,7 +481,9 @@ template <int PREC, bool TSHARED, int G> struct SmemPlan {
 
 // ---------------------------------------------------------------------------------------------------- the kernel
 // counters[0]: next tile (zeroed before every launch); [1]: items evaluated; [2]: secondary rays traced (dense count)
-template <bool F16TAB, int PREC, bool TSHARED, int G>
+// IND = false: frames without the indirect term (BASELINE configs[1]): phases B and C are compiled out, which takes the
+// split-precision kernel from 168 to <= 128 registers and lets four warpgroups share an SM instead of three.
+template <bool F16TAB, int PREC, bool TSHARED, int G, bool IND = true>
 __global__ void __launch_bounds__(kRows* G, 1)
     k_render_wg(const __grid_constant__ GridP g, EnvP env, ShadeP sp, const __grid_constant__ TcConst cw, const uint8_t* __restrict__ wtiles,
                 const float* __restrict__ wts32, FrameP fr, float* __restrict__ rgb, Item* __restrict__ ring,
@@ -526,7 +528,7 @@ __global__ void __launch_bounds__(kRows* G, 1)
     for (int i = threadIdx.x; i < (int)(SP::tiles / 16); i += kRows * G) dst[i] = __ldg(src + i);
   }
   fill_ones(s_ones, kRows * G);
-  const bool indirect = (fr.flags & 4u) && fr.s.S && fr.t.S;
+  const bool indirect = IND && (fr.flags & 4u) && fr.s.S && fr.t.S;
   if (indirect && TSHARED) {                    // shared tertiary set: Q_k = W1w . w'_k; per k: radiance, pdf, direction
     for (int e = threadIdx.x; e < (int)fr.t.S * kH; e += kRows * G) {
       const int k = e / kH, q = e % kH;
@@ -740,7 +742,7 @@ __global__ void __launch_bounds__(kRows* G, 1)
     }
 
     // ---- phases B + C: secondary rays -> work items -> L'_o -----------------------------------------------------------
-    if (S_i > 0) {
+    if constexpr (IND) if (S_i > 0) {
       const float wscale = 1.f / ((float)S_i * (float)S2);
       for (int j0 = 0; j0 < S_i; j0 += kChunkJ) {
         const int j1 = min(j0 + kChunkJ, S_i);
@@ -973,11 +975,11 @@ inline void prepare_weights(const hr_config& cfg, const float* bw, const float* 
 
 inline bool frame_supported(const FrameP& fr) { return !(fr.flags & 4u) || fr.t.stride != 0 || fr.t.S <= (uint32_t)kMaxS2; }
 
-template <bool F16TAB, int PREC, bool TSHARED, int G>
+template <bool F16TAB, int PREC, bool TSHARED, int G, bool IND = true>
 inline cudaError_t launch_one(const GridP& g, const EnvP& env, const ShadeP& sp, const TcConst& cw, const uint8_t* d_tiles,
                               const float* wts32, const FrameP& fr, float* rgb, Item* ring, unsigned long long* counters, int num_sms, cudaStream_t st) {
   using SP = SmemPlan<PREC, TSHARED, G>;
-  auto kern = k_render_wg<F16TAB, PREC, TSHARED, G>;
+  auto kern = k_render_wg<F16TAB, PREC, TSHARED, G, IND>;
   cudaError_t e = cudaMemsetAsync(counters, 0, 8, st);                // the tile counter; the statistics keep accumulating
   if (e != cudaSuccess) return e;
   const unsigned long long tiles = (fr.N + kRows - 1) / kRows;
@@ -987,9 +989,9 @@ inline cudaError_t launch_one(const GridP& g, const EnvP& env, const ShadeP& sp,
   return cudaGetLastError();
 }
 
-template <bool F16TAB, int PREC, bool TSHARED, int G>
+template <bool F16TAB, int PREC, bool TSHARED, int G, bool IND = true>
 inline cudaError_t render_attr() {
-  return cudaFuncSetAttribute(k_render_wg<F16TAB, PREC, TSHARED, G>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+  return cudaFuncSetAttribute(k_render_wg<F16TAB, PREC, TSHARED, G, IND>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                               (int)SmemPlan<PREC, TSHARED, G>::bytes);
 }
 

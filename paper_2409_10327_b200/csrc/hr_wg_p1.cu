@@ -14,6 +14,10 @@ cudaError_t launch_p1(bool f16tab, const GridP& g, const EnvP& env, const ShadeP
   const TcConst& cw = *reinterpret_cast<const TcConst*>(tc_const);
   Item* rg = reinterpret_cast<Item*>(ring);
   const bool tsh = fr.t.stride == 0;
+  if (!((fr.flags & 4u) && fr.s.S && fr.t.S)) {                  // no indirect term: the direct-only kernel, four warpgroups per SM
+    if (f16tab) return launch_one<true, 1, true, 4, false>(g, env, sp, cw, d_tiles, wts32, fr, rgb, rg, counters, num_sms, st);
+    return launch_one<false, 1, true, 4, false>(g, env, sp, cw, d_tiles, wts32, fr, rgb, rg, counters, num_sms, st);
+  }
   if (f16tab) {
     if (tsh) return launch_one<true, 1, true, HR_G_P1>(g, env, sp, cw, d_tiles, wts32, fr, rgb, rg, counters, num_sms, st);
     return launch_one<true, 1, false, 2>(g, env, sp, cw, d_tiles, wts32, fr, rgb, rg, counters, num_sms, st);
@@ -32,6 +36,8 @@ cudaError_t launch_trace_p1(bool f16tab, const GridP& g, const ShadeP& sp, const
 
 cudaError_t init_device_p1() {
   cudaError_t e;
+  if ((e = render_attr<true, 1, true, 4, false>()) != cudaSuccess) return e;
+  if ((e = render_attr<false, 1, true, 4, false>()) != cudaSuccess) return e;
   if ((e = render_attr<true, 1, true, HR_G_P1>()) != cudaSuccess) return e;
   if ((e = render_attr<true, 1, false, 2>()) != cudaSuccess) return e;
   if ((e = render_attr<false, 1, true, HR_G_P1>()) != cudaSuccess) return e;
