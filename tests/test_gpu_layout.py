@@ -86,3 +86,32 @@ def test_probe_gather_reports_a_sane_rate(torch):
         probe_gather(3000, 4, 1, 0)                                    # not a power of two
     with pytest.raises(HashRenderError):
         probe_gather(1 << 20, 16, 3, 0)                                # unsupported shape
+
+
+@pytest.mark.parametrize("over", [dict(L=3, log2_T=5, base_res=1, max_res=6),            # res 1, 2, 6: a one-cell level, dense and hashed mixed
+                                  dict(L=4, log2_T=3, base_res=2, max_res=40),           # T = 8 rows: every level hashed, heavy collisions
+                                  dict(L=16, log2_T=10, base_res=16, max_res=2048, table_dtype="f16", mlp_dtype="f16")])
+def test_degenerate_grids_encode_bit_exact(torch, over):
+    """Tiny tables and coarse grids: all (or the first six) levels end up cell-major, most of them hashed with many cells
+    sharing a row.  Indices and fractional positions bit-exact against the oracle, features to rounding."""
+    from hr_testutil import check_close
+    from oracle.oracle import Oracle
+    cfg = gen.make_config("C0", table_scale=0.5, **over)
+    m = gen.make_model(cfg)
+    o = Oracle.from_gen(cfg, m)
+    rng = np.random.default_rng(11)
+    n = 3000
+    x = rng.random((n, 3), dtype=np.float32)
+    x[:6] = [[0, 0, 0], [1, 1, 1], [1, 0, 0.5], [0.5, 0.5, 0.5], [0.999999, 1e-7, 1], [-0.5, 2.0, 0.25]]     # clamped (Q6)
+    feat_o, idx_o, w_o = o.encode(x)
+    r = make_renderer(cfg, m)
+    nblock, _ = r.table_layout()
+    assert nblock == (cfg.L if cfg.L <= 4 else 6)                    # the 16-level grid: levels 0-5 fit the budget, T = 1024 rows hash the rest
+    feat = torch.empty((n, cfg.D), device="cuda"); idx = torch.empty((n, cfg.L, 8), device="cuda", dtype=torch.int32)
+    w = torch.empty((n, cfg.L, 3), device="cuda")
+    r.encode(to_dev(x), feat, idx, w)
+    torch.cuda.synchronize()
+    assert np.array_equal(idx.cpu().numpy().view(np.uint32), idx_o)
+    assert np.array_equal(w.cpu().numpy(), w_o)
+    check_close(feat.cpu().numpy(), feat_o, 2e-6, what=f"encode {over}")
+    r.destroy()
