@@ -809,14 +809,16 @@ __global__ void __launch_bounds__(kRows* G, 1)
 
 // ---------------------------------------------------------------------------------------------------- trace kernel
 // hashrender_trace with the encode fused (a1-a4, a6, a7) for fp16 models -- the kernel of the encode + IRT sweep
-// (BASELINE.json configs[4]).  Same warpgroup scheme with G = 4 and four levels (32 gathers) in flight per thread: 16 warps
-// x 32 outstanding loads per SM keep the gather pipeline full when the table spills from L2 to HBM.  t is an output, so the
-// fp32 epilogue is used (features hi/lo split for P, fp16 h1).
+// (BASELINE.json configs[4]).  Same warpgroup scheme with G = 4.  t is an output, so the fp32 epilogue is used (features hi/lo
+// split for P, fp16 h1).  Levels whose gathers are in flight together: two, and one in the instantiation for tables far beyond
+// the L2 (HINT).  Measured at 2^24 points with the cell-major levels (ms at T = 2^16 / 2^19 / 2^22 / 2^24): one level 4.36 / 4.80 /
+// 8.73 / 9.25, two 4.31 / 4.70 / 8.57 / 9.53, four 4.46 / 4.92 / 8.83 / 9.48.  (Before the cell-major levels four was best:
+// 16 warps x 32 outstanding loads; a cell-major level is one load, so four levels no longer means 32.)
 constexpr int kTraceG = 4;
 #ifdef HR_TRACE_LIF
-constexpr int kTraceLIF = HR_TRACE_LIF;
+constexpr int kTraceLIF = HR_TRACE_LIF, kTraceLIFHint = HR_TRACE_LIF;
 #else
-constexpr int kTraceLIF = 4;
+constexpr int kTraceLIF = 2, kTraceLIFHint = 1;
 #endif
 template <int PREC> constexpr size_t trace_smem() {
   return 1024 + (size_t)kHiTileBytes * (PREC ? 2 : 1) + kOnesBytes + (size_t)kTraceG * kH * kRows * 4 + 8 * kMaxG + 16;
@@ -901,7 +903,7 @@ __global__ void __launch_bounds__(kRows* kTraceG, 1)
     float px = 0.f, py = 0.f, pz = 0.f;
     if (x) { px = __ldg(x + 3 * i); py = __ldg(x + 3 * i + 1); pz = __ldg(x + 3 * i + 2); }
     if (feat) feat_split_to<4>(tA, g, feat + i * D);
-    else if constexpr (HINT) encode_split_to<F16TAB, kTraceLIF>(tA, g, px, py, pz, nullptr, &pol);
+    else if constexpr (HINT) encode_split_to<F16TAB, kTraceLIFHint>(tA, g, px, py, pz, nullptr, &pol);
     else encode_split_to<F16TAB, kTraceLIF>(tA, g, px, py, pz);
     issue_layer<PREC, G>(c, 0, 0, 2, true, 0, 2);                     // P = W1f f + b1, split-precision f
     wait_layer(c);
