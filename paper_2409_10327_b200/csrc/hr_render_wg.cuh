@@ -492,11 +492,12 @@ __global__ void __launch_bounds__(kRows* G, 1)
 #ifdef HR_LIF
   constexpr int LIF = HR_LIF;
 #else
-  // levels whose gathers are issued together in the encodes of this kernel.  One: a level's eight gathers, then its interpolation,
-  // then the next level.  Measured (C3 dense / compacted, C2 compacted, ms): LIF 1 15.65 / 7.61 / 10.87, LIF 2 (G = 4) and
-  // 4 (G = 3) 16.12 / 7.72 / 11.36, LIF 4 at G = 4 19.99 / 9.62: L1 serves a warp's 32 divergent lines one per cycle, so a
-  // burst of gathers from every warp queues up instead of overlapping with the other warps' arithmetic.
-  constexpr int LIF = 1;
+  // levels whose gathers are issued together in the encodes of this kernel.  Two since the coarsest levels are cell-major (one
+  // load each): same box, C3 dense 15.22 -> 15.00 ms, C2 dense 23.13 -> 23.07, compacted frames and C1 unchanged.  Before the
+  // cell-major levels one level at a time was best (C3 dense / compacted, C2 compacted, ms: LIF 1 15.65 / 7.61 / 10.87, LIF 2
+  // (G = 4) and 4 (G = 3) 16.12 / 7.72 / 11.36, LIF 4 at G = 4 19.99 / 9.62): the L1 passes one missing sector per cycle to the L2,
+  // so a burst of gathers from every warp queues up instead of overlapping with the other warps' arithmetic.
+  constexpr int LIF = 2;
 #endif
   using SP = SmemPlan<PREC, TSHARED, G>;
   extern __shared__ uint8_t smem_raw[];
