@@ -210,13 +210,22 @@ def gather_model():
     return _GATHER
 
 
+def gather_counts(levels, cell_major, rows_per_sector):
+    """(32-byte sectors, load instructions) one point's encode touches: a cell-major level is one sector and one 256-bit load
+    (fp16 rows, 8 per sector) or two and two (fp32 rows, 4 per sector); any other level is 8 one-row loads in 4 x-pairs, and the two
+    rows of a pair -- rows s and s ^ m with m = cx ^ (cx + 1) = 1, 3, 7, ... -- share a sector unless m >= rows_per_sector, which
+    happens for one cell in rows_per_sector.  Checked against a count over the oracle's indices in tests/test_gen_recipe.py."""
+    per_entry = 1 if rows_per_sector == 8 else 2
+    sectors = cell_major * per_entry + (levels - cell_major) * 4 * (1 + 1.0 / rows_per_sector)
+    loads = cell_major * per_entry + (levels - cell_major) * 8
+    return sectors, loads
+
+
 def gather_floor(n_points, levels, cell_major, rows_per_sector, sm_mhz, num_sms=148):
     """L1 floor of the encode of n_points: cell-major levels cost one sector and one load (fp16) or two and two (fp32 rows),
     the others 8 loads in 4 x-pairs, each pair in one sector unless it straddles a sector boundary."""
     gm = gather_model()
-    per_entry = 1 if rows_per_sector == 8 else 2
-    sectors = cell_major * per_entry + (levels - cell_major) * 4 * (1 + 1.0 / rows_per_sector)
-    loads = cell_major * per_entry + (levels - cell_major) * 8
+    sectors, loads = gather_counts(levels, cell_major, rows_per_sector)
     cyc = gm["c_sector"] * sectors + gm["c_load"] * loads
     ms = n_points * cyc / num_sms / (sm_mhz * 1e3)
     return {"sectors_per_point": sectors, "loads_per_point": loads, "c_sector": gm["c_sector"], "c_load": gm["c_load"],

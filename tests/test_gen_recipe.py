@@ -45,3 +45,28 @@ def test_hard_visibility_is_balanced(name, over):
     if zs is not None:
         fs = (zs > 0).mean()
         assert 0.3 <= fs <= 0.7, fs
+
+
+def test_bench_gather_counts_match_a_count_over_the_oracle_indices():
+    """bench.py's L1 roofline of the encode (roofline.l1_gather) prices `sectors` and `loads` per point.  For the levels that are
+    not cell-major the device row of a hashed level IS the specified index, so the sectors a point touches can be counted from
+    the oracle's corner indices: distinct (index // rows per sector) among a level's 8 corners, averaged over random points."""
+    import importlib.util
+    from oracle.oracle import Oracle
+    spec = importlib.util.spec_from_file_location("bench", os.path.join(os.path.dirname(GOLD), "..", "bench.py"))
+    bench = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(bench)
+    cfg = gen.make_config("C4")                                        # fp16 rows: 8 per 32-byte sector
+    m = gen.make_model(cfg)
+    o = Oracle.from_gen(cfg, m)
+    x = np.random.default_rng(5).random((20000, 3), dtype=np.float32)
+    _, idx, _ = o.encode(x)
+    hashed = [l for l in range(cfg.L) if (int(m["res"][l]) + 1) ** 3 > cfg.T]
+    for rows_per_sector in (8, 4):
+        counted = np.mean([[len(set((idx[i, l] // rows_per_sector).tolist())) for l in hashed] for i in range(0, 20000, 10)])
+        model_sectors, model_loads = bench.gather_counts(1, 0, rows_per_sector)
+        assert model_loads == 8
+        assert abs(counted - model_sectors) < 0.05 * model_sectors, (rows_per_sector, counted, model_sectors)
+    # cell-major levels: one entry = 8 rows = exactly one sector of fp16 rows, two of fp32 rows
+    assert bench.gather_counts(16, 16, 8) == (16, 16) and bench.gather_counts(16, 16, 4) == (32, 32)
+    assert bench.gather_counts(16, 6, 8) == (6 + 10 * 4.5, 6 + 80)
