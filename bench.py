@@ -212,12 +212,14 @@ def gather_model():
 
 def gather_counts(levels, cell_major, rows_per_sector):
     """(32-byte sectors, load instructions) one point's encode touches: a cell-major level is one sector and one 256-bit load
-    (fp16 rows, 8 per sector) or two and two (fp32 rows, 4 per sector); any other level is 8 one-row loads in 4 x-pairs, and the two
-    rows of a pair -- rows s and s ^ m with m = cx ^ (cx + 1) = 1, 3, 7, ... -- share a sector unless m >= rows_per_sector, which
-    happens for one cell in rows_per_sector.  Checked against a count over the oracle's indices in tests/test_gen_recipe.py."""
+    (fp16 rows, 8 per sector) or two and two (fp32 rows, 4 per sector); any other level is 4 x-pairs, and the two rows of a pair --
+    rows s and s ^ m with m = cx ^ (cx + 1) = 1, 3, 7, ... -- share a sector unless m >= rows_per_sector, which happens for one
+    cell in rows_per_sector.  Loads of such a level: 8 one-row loads for fp32 rows; for fp16 rows one two-row load per pair plus a
+    one-row load of the neighbour when cx is odd (hr_device.cuh gather8_h2): 6 on average.  The sector count is checked against a
+    count over the oracle's indices in tests/test_gen_recipe.py."""
     per_entry = 1 if rows_per_sector == 8 else 2
     sectors = cell_major * per_entry + (levels - cell_major) * 4 * (1 + 1.0 / rows_per_sector)
-    loads = cell_major * per_entry + (levels - cell_major) * 8
+    loads = cell_major * per_entry + (levels - cell_major) * (6 if rows_per_sector == 8 else 8)
     return sectors, loads
 
 

@@ -119,12 +119,9 @@ __device__ __forceinline__ void corner_indices(const Cell& c, uint32_t N, bool d
   }
 }
 
-// a3: the 8 corner rows of one level, corner number b0 + 2 b1 + 4 b2 (Q9): one index path for dense and hashed levels, eight
-// independent one-row loads (address = level base + row * row bytes in one mad.wide.u32, read-only path).
-// Measured and not kept: fetching the x-neighbour pair with ONE aligned two-row load (the rows of cx and cx + 1 are adjacent
-// whenever cx is even; a predicated one-row load covers odd cx) -- 6 instead of 8 line requests per level, bit-identical values --
-// was slower everywhere (C2 23.3 -> 25.4 ms, C3 16.7 -> 17.6 ms, C4 at T = 2^19 6.0 -> 6.4 ms, at T = 2^24 13.5 -> 15.2 ms): the
-// selects and predication cost more issue slots than the saved L1 requests give back.
+// a3: the 8 corner rows of one level, corner number b0 + 2 b1 + 4 b2 (Q9): one index path for dense and hashed levels (address =
+// level base + row * row bytes in one mad.wide.u32, read-only path).  fp32 rows: eight independent one-row loads.  fp16 rows: the
+// x-neighbour pair comes with one aligned two-row load when cx is even (gather8_h2).
 __device__ __forceinline__ void corner_rows(const GridP& g, int l, const uint32_t (&c0)[3], uint32_t (&i0)[4], uint32_t (&i1)[4]) {
   const uint32_t pa = g.pa[l], pb = g.pb[l], pm = g.pmask[l];
   const uint32_t hy0 = c0[1] * pa, hy1 = hy0 + pa, hz0 = c0[2] * pb, hz1 = hz0 + pb;
@@ -151,10 +148,21 @@ __device__ __forceinline__ void gather8_h2(const GridP& g, int l, const uint32_t
   uint32_t i0[4], i1[4];
   corner_rows(g, l, c0, i0, i1);
   const char* lb = reinterpret_cast<const char*>(g.tables) + g.off[l];
+  // The aligned 8-byte word of row i0 always holds row i0 ^ 1, and that IS the x-neighbour when cx is even (bit 0 of a row is bit 0
+  // of cx on every level): one 8-byte load serves the pair, a predicated one-row load fetches the neighbour for odd cx.  6 loads per
+  // level instead of 8 on average; each costs the L1 0.35 cycles (hashrender_probe_gather).  Same box: C3 dense 15.00 -> 14.50 ms,
+  // compacted 7.16 -> 7.04, C4 at T = 2^19 4.71 -> 4.64.  (Before the cell-major levels the same idea LOST -- C3 16.7 -> 17.6 -- and
+  // for 8-byte fp32 rows it still does, C2 23.05 -> 24.35: the 16-byte pair words cost the split-precision kernel registers it
+  // does not have.  gather8_f2 keeps one load per row.)
+  const bool odd = c0[0] & 1u;
 #pragma unroll
   for (int j = 0; j < 4; ++j) {
-    asm("{\n\t.reg .u64 p;\n\tmad.wide.u32 p, %1, 4, %2;\n\tld.global.nc.b32 %0, [p];\n\t}" : "=r"(v[2 * j]) : "r"(i0[j]), "l"(lb));
-    asm("{\n\t.reg .u64 p;\n\tmad.wide.u32 p, %1, 4, %2;\n\tld.global.nc.b32 %0, [p];\n\t}" : "=r"(v[2 * j + 1]) : "r"(i1[j]), "l"(lb));
+    uint32_t lo, hi, nb = 0u;
+    asm("{\n\t.reg .u64 p;\n\tmad.wide.u32 p, %2, 4, %3;\n\tld.global.nc.v2.b32 {%0, %1}, [p];\n\t}" : "=r"(lo), "=r"(hi) : "r"(i0[j] & ~1u), "l"(lb));
+    if (odd) asm("{\n\t.reg .u64 p;\n\tmad.wide.u32 p, %1, 4, %2;\n\tld.global.nc.b32 %0, [p];\n\t}" : "=r"(nb) : "r"(i1[j]), "l"(lb));
+    const bool up = i0[j] & 1u;
+    v[2 * j] = up ? hi : lo;
+    v[2 * j + 1] = odd ? nb : (up ? lo : hi);
   }
 }
 // the same with an L2 eviction policy per level (hashed: evict-first, dense: evict-last)
