@@ -358,6 +358,11 @@ int hashrender_create(const hr_config* cfg, const float* tables, const float* br
     for (uint32_t l = g.nblock; l < cfg->L; ++l) if (!((g.dense_mask >> l) & 1u)) hashed += lvl_rows[l] * esz;
     g.l2_hint = hashed > 2ull * (uint64_t)l2 ? 1u : 0u;                // measured: helps at 448 MB of hashed levels, hurts at 128 MB (hr_device.cuh)
   }
+  {
+    int l2 = 0;
+    HR_CUDA(h, cudaDeviceGetAttribute(&l2, cudaDevAttrL2CacheSize, dev));
+    g.pair_loads = (cfg->table_dtype == HR_F16 && rows_total * esz <= (uint64_t)l2 / 2) ? 1u : 0u;   // L2-resident on both dies' halves
+  }
   HR_CUDA(h, cudaMalloc(&h->d_tables, rows_total * esz));
   h->table_bytes = rows_total * esz;
   HR_CUDA(h, cudaMemset(h->d_tables, 0, rows_total * esz));

@@ -33,6 +33,7 @@ struct GridP {
   unsigned long long off[kMaxL];
   const void* tables;       // rows of float2 (f16 == 0) or __half2 (f16 == 1)
   uint32_t l2_hint;         // hashed levels > 2 x L2: their gathers carry an evict-first policy, dense levels evict-last (k_trace_wg)
+  uint32_t pair_loads;      // fp16 rows, device copy of the tables L2-resident: x-neighbour pairs come with one two-row load (gather8_h2)
 };
 // L2 eviction policies for tables far larger than the L2 (BASELINE configs[4], T = 2^24): the hashed levels are a random stream over
 // hundreds of MB that no cache can hold, the dense levels are ~70 MB that every point reads.  Hashed rows are fetched evict-first
@@ -140,6 +141,7 @@ __device__ __forceinline__ void ldg_nc32(const uint4* p, uint32_t (&r)[8]) {
   asm("ld.global.nc.v8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
       : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]) : "l"(p));
 }
+template <int PAIR = -1>                      // -1: g.pair_loads decides at run time; 0 / 1: the caller's kernel was chosen by it
 __device__ __forceinline__ void gather8_h2(const GridP& g, int l, const uint32_t (&c0)[3], uint32_t (&v)[8]) {
   if (l < (int)g.nblock) {                                    // warp-uniform: l is a loop counter
     ldg_nc32(block_entry(g, l, c0, 32u), v);
@@ -154,6 +156,16 @@ __device__ __forceinline__ void gather8_h2(const GridP& g, int l, const uint32_t
   // compacted 7.16 -> 7.04, C4 at T = 2^19 4.71 -> 4.64.  (Before the cell-major levels the same idea LOST -- C3 16.7 -> 17.6 -- and
   // for 8-byte fp32 rows it still does, C2 23.05 -> 24.35: the 16-byte pair words cost the split-precision kernel registers it
   // does not have.  gather8_f2 keeps one load per row.)
+  // Only while the tables are L2-resident (g.pair_loads, set by hashrender_create): with tables that spill to HBM the same loads
+  // LOSE (k_trace_wg at T = 2^22, 2^24 points: 8.56 -> 9.23 ms on one box), and one load per row stays.
+  if (PAIR == 0 || (PAIR < 0 && !g.pair_loads)) {
+#pragma unroll
+    for (int j = 0; j < 4; ++j) {
+      asm("{\n\t.reg .u64 p;\n\tmad.wide.u32 p, %1, 4, %2;\n\tld.global.nc.b32 %0, [p];\n\t}" : "=r"(v[2 * j]) : "r"(i0[j]), "l"(lb));
+      asm("{\n\t.reg .u64 p;\n\tmad.wide.u32 p, %1, 4, %2;\n\tld.global.nc.b32 %0, [p];\n\t}" : "=r"(v[2 * j + 1]) : "r"(i1[j]), "l"(lb));
+    }
+    return;
+  }
   const bool odd = c0[0] & 1u;
 #pragma unroll
   for (int j = 0; j < 4; ++j) {
@@ -167,7 +179,7 @@ __device__ __forceinline__ void gather8_h2(const GridP& g, int l, const uint32_t
 }
 // the same with an L2 eviction policy per level (hashed: evict-first, dense: evict-last)
 __device__ __forceinline__ void gather8_h2_hint(const GridP& g, int l, const uint32_t (&c0)[3], uint32_t (&v)[8], const L2Pol& pol) {
-  if (l < (int)g.nblock) { gather8_h2(g, l, c0, v); return; }
+  if (l < (int)g.nblock) { gather8_h2<0>(g, l, c0, v); return; }
   uint32_t i0[4], i1[4];
   corner_rows(g, l, c0, i0, i1);
   const char* lb = reinterpret_cast<const char*>(g.tables) + g.off[l];
@@ -199,11 +211,11 @@ __device__ __forceinline__ void gather8_f2(const GridP& g, int l, const uint32_t
     asm("{\n\t.reg .u64 p;\n\tmad.wide.u32 p, %2, 8, %3;\n\tld.global.nc.v2.f32 {%0, %1}, [p];\n\t}" : "=f"(v[2 * j + 1].x), "=f"(v[2 * j + 1].y) : "r"(i1[j]), "l"(lb));
   }
 }
-template <bool F16>
+template <bool F16, int PAIR = -1>
 __device__ __forceinline__ void gather8(const GridP& g, int l, const uint32_t (&c0)[3], float2 (&v)[8]) {
   if constexpr (F16) {
     uint32_t r[8];
-    gather8_h2(g, l, c0, r);
+    gather8_h2<PAIR>(g, l, c0, r);
 #pragma unroll
     for (int k = 0; k < 8; ++k) v[k] = __half22float2(*reinterpret_cast<const __half2*>(&r[k]));
   } else {
@@ -212,7 +224,7 @@ __device__ __forceinline__ void gather8(const GridP& g, int l, const uint32_t (&
 }
 
 // a3/a4: gather 8 corners of one level and interpolate.  Corner number b0 + 2 b1 + 4 b2 (Q9).
-template <bool F16>
+template <bool F16, int PAIR = -1>
 __device__ __forceinline__ float2 encode_level(const GridP& g, int l, float x, float y, float z,
                                                uint32_t* idx_out, float* w_out, const L2Pol* pol = nullptr) {
   const uint32_t N = g.res[l];
@@ -224,7 +236,7 @@ __device__ __forceinline__ float2 encode_level(const GridP& g, int l, float x, f
 #pragma unroll
     for (int k = 0; k < 8; ++k) v[k] = __half22float2(*reinterpret_cast<const __half2*>(&r[k]));
   } else {
-    gather8<F16>(g, l, c.c0, v);
+    gather8<F16, PAIR>(g, l, c.c0, v);
   }
   if (idx_out) {                                              // the SPECIFIED index (Q1, Q3), not the device row
     uint32_t idx[8];

@@ -364,7 +364,7 @@ __device__ __forceinline__ float2 lerp32(const Taps32<F16TAB>& t) {
   return f;
 }
 // f = H(x) in fp32 -> A columns 0..15 (hi) | 16..31 (lo), LIF levels per TMEM store
-template <bool F16TAB, int LIF>
+template <bool F16TAB, int LIF, int PAIR = -1>
 __device__ __forceinline__ void encode_split_to(uint32_t tA, const GridP& g, float x, float y, float z, float* scr = nullptr,
                                                 const L2Pol* pol = nullptr) {
 #pragma unroll 1
@@ -379,7 +379,7 @@ __device__ __forceinline__ void encode_split_to(uint32_t tA, const GridP& g, flo
       // cycle, and 16 warps x 32 loads queue behind each other instead of overlapping with the interpolation of the others.
       hi[q] = 0u; lo[q] = 0u;
       if (l0 + q < (int)g.L) {
-        const float2 v = encode_level<F16TAB>(g, l0 + q, x, y, z, nullptr, nullptr, pol);
+        const float2 v = encode_level<F16TAB, PAIR>(g, l0 + q, x, y, z, nullptr, nullptr, pol);
         split_pair(v.x, v.y, hi[q], lo[q]);
         if (scr) { scr[(2 * (l0 + q)) * kRows] = v.x; scr[(2 * (l0 + q) + 1) * kRows] = v.y; }
       } else if (scr) {
@@ -815,11 +815,13 @@ __global__ void __launch_bounds__(kRows* G, 1)
 // the L2 (HINT).  Measured at 2^24 points with the cell-major levels (ms at T = 2^16 / 2^19 / 2^22 / 2^24): one level 4.36 / 4.80 /
 // 8.73 / 9.25, two 4.31 / 4.70 / 8.57 / 9.53, four 4.46 / 4.92 / 8.83 / 9.48.  (Before the cell-major levels four was best:
 // 16 warps x 32 outstanding loads; a cell-major level is one load, so four levels no longer means 32.)
+// With the paired loads of the L2-resident fp16 tables (6 loads per level, MODE 2) four levels are best again: T = 2^16 4.12 -> 4.07,
+// 2^19 4.65 -> 4.52 (same box).
 constexpr int kTraceG = 4;
 #ifdef HR_TRACE_LIF
-constexpr int kTraceLIF = HR_TRACE_LIF, kTraceLIFHint = HR_TRACE_LIF;
+constexpr int kTraceLIF = HR_TRACE_LIF, kTraceLIFHint = HR_TRACE_LIF, kTraceLIFRes = HR_TRACE_LIF;
 #else
-constexpr int kTraceLIF = 2, kTraceLIFHint = 1;
+constexpr int kTraceLIF = 2, kTraceLIFHint = 1, kTraceLIFRes = 4;
 #endif
 template <int PREC> constexpr size_t trace_smem() {
   return 1024 + (size_t)kHiTileBytes * (PREC ? 2 : 1) + kOnesBytes + (size_t)kTraceG * kH * kRows * 4 + 8 * kMaxG + 16;
@@ -847,7 +849,8 @@ __device__ __forceinline__ void feat_split_to(uint32_t tA, const GridP& g, const
 // PREC = 0: fp16 models (fp16 h1, one MMA pass).  PREC = 1: fp32 models in hi/lo split precision -- exactly the arithmetic
 // k_render_wg<PREC = 1> runs for its direct / secondary queries (h1_dir<true>, three passes, epi_precise), so hashrender_trace
 // on an fp32 model checks z_v, t, x' of the production path stage by stage.  feat != nullptr: the caller's features replace H(x).
-template <bool F16TAB, int PREC, bool HINT = false>
+// MODE 0: tables beyond the L2; 1: far beyond it (L2 policies on the gathers); 2: L2-resident fp16 tables (paired loads)
+template <bool F16TAB, int PREC, int MODE = 0>
 __global__ void __launch_bounds__(kRows* kTraceG, 1)
     k_trace_wg(const __grid_constant__ GridP g, ShadeP sp, const __grid_constant__ TcConst cw, const uint8_t* __restrict__ wtiles,
                const float* __restrict__ x, const float* __restrict__ feat, unsigned long long N, DirsetP ds, float* __restrict__ vis,
@@ -896,6 +899,7 @@ __global__ void __launch_bounds__(kRows* kTraceG, 1)
   const unsigned long long ntiles = (N + kRows - 1) / kRows;
   const uint32_t D = g.L * 2u;
   L2Pol pol;
+  constexpr bool HINT = MODE == 1;
   if constexpr (HINT) pol = make_l2pol();
   for (unsigned long long tile = (unsigned long long)blockIdx.x * G + wgi; tile < ntiles; tile += (unsigned long long)gridDim.x * G) {
     const unsigned long long i_raw = tile * kRows + c.t;
@@ -904,7 +908,8 @@ __global__ void __launch_bounds__(kRows* kTraceG, 1)
     float px = 0.f, py = 0.f, pz = 0.f;
     if (x) { px = __ldg(x + 3 * i); py = __ldg(x + 3 * i + 1); pz = __ldg(x + 3 * i + 2); }
     if (feat) feat_split_to<4>(tA, g, feat + i * D);
-    else if constexpr (HINT) encode_split_to<F16TAB, kTraceLIFHint>(tA, g, px, py, pz, nullptr, &pol);
+    else if constexpr (HINT) encode_split_to<F16TAB, kTraceLIFHint, 0>(tA, g, px, py, pz, nullptr, &pol);
+    else if constexpr (MODE == 2) encode_split_to<F16TAB, kTraceLIFRes, 1>(tA, g, px, py, pz);
     else encode_split_to<F16TAB, kTraceLIF>(tA, g, px, py, pz);
     issue_layer<PREC, G>(c, 0, 0, 2, true, 0, 2);                     // P = W1f f + b1, split-precision f
     wait_layer(c);
@@ -941,7 +946,9 @@ inline cudaError_t launch_trace_one(const GridP& g, const ShadeP& sp, const TcCo
   const unsigned long long need = ((N + kRows - 1) / kRows + kTraceG - 1) / kTraceG;
   const int grid = (int)(need < (unsigned long long)num_sms ? need : (unsigned long long)num_sms);
   if (F16TAB && g.l2_hint && !feat)
-    k_trace_wg<F16TAB, PREC, F16TAB><<<grid, kRows * kTraceG, trace_smem<PREC>(), st>>>(g, sp, cw, d_tiles, x, feat, N, ds, vis, zv, t, xsec);
+    k_trace_wg<F16TAB, PREC, F16TAB ? 1 : 0><<<grid, kRows * kTraceG, trace_smem<PREC>(), st>>>(g, sp, cw, d_tiles, x, feat, N, ds, vis, zv, t, xsec);
+  else if (F16TAB && g.pair_loads && !feat)
+    k_trace_wg<F16TAB, PREC, F16TAB ? 2 : 0><<<grid, kRows * kTraceG, trace_smem<PREC>(), st>>>(g, sp, cw, d_tiles, x, feat, N, ds, vis, zv, t, xsec);
   else
     k_trace_wg<F16TAB, PREC><<<grid, kRows * kTraceG, trace_smem<PREC>(), st>>>(g, sp, cw, d_tiles, x, feat, N, ds, vis, zv, t, xsec);
   return cudaGetLastError();
@@ -949,7 +956,9 @@ inline cudaError_t launch_trace_one(const GridP& g, const ShadeP& sp, const TcCo
 // the opt-in to > 48 KB of dynamic shared memory is per device: hashrender_create calls this for the handle's device
 template <bool F16TAB, int PREC>
 inline cudaError_t trace_attr() {
-  cudaError_t e = cudaFuncSetAttribute(k_trace_wg<F16TAB, PREC, F16TAB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)trace_smem<PREC>());
+  cudaError_t e = cudaFuncSetAttribute(k_trace_wg<F16TAB, PREC, F16TAB ? 1 : 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)trace_smem<PREC>());
+  if (e != cudaSuccess) return e;
+  e = cudaFuncSetAttribute(k_trace_wg<F16TAB, PREC, F16TAB ? 2 : 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)trace_smem<PREC>());
   if (e != cudaSuccess) return e;
   return cudaFuncSetAttribute(k_trace_wg<F16TAB, PREC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)trace_smem<PREC>());
 }
